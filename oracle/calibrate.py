@@ -1,0 +1,48 @@
+"""eps_d calibration for the DSSJ configs -- TEST INFRASTRUCTURE (oracle side).
+
+A reduced form of the paper's sampled cumulative distance histogram
+(section 3.5.3): the radius at which a sample's pooled pair
+distances reach the target selectivity s = mean neighbours per point
+(PAPER.md:221).  Recipe in DESIGN.md "Input recipe".
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import dist_row
+
+
+def eps_per_dimension(X, masks, target_neighbours, seed, n_query_sample=1000,
+                      n_cand_sample=None, max_masks_per_dim=64):
+    """-> eps [n_masks] fp64: every mask of popcount d gets eps_d, the pooled
+    sample quantile at target_neighbours/(N-1) of D over (sampled query,
+    sampled candidate != query) pairs of up to max_masks_per_dim masks of that d."""
+    X = np.ascontiguousarray(X, dtype=np.float32)
+    masks = np.asarray(masks, dtype=np.uint16)
+    N = X.shape[0]
+    rng = np.random.default_rng(seed)
+    qs = np.sort(rng.choice(N, min(n_query_sample, N), replace=False))
+    if n_cand_sample is None or n_cand_sample >= N:
+        cs = qs
+    else:
+        cs = np.sort(rng.choice(N, n_cand_sample, replace=False))
+    Xs = np.ascontiguousarray(X[np.union1d(qs, cs)])
+    ids = np.union1d(qs, cs)
+    q_pos = np.searchsorted(ids, qs)
+    c_pos = np.searchsorted(ids, cs)
+    dims = np.array([bin(int(m)).count("1") for m in masks])
+    frac = target_neighbours / (N - 1)
+    eps = np.zeros(len(masks), dtype=np.float64)
+    for d in np.unique(dims):
+        sel = np.flatnonzero(dims == d)
+        pick = sel if len(sel) <= max_masks_per_dim else np.sort(
+            rng.permutation(sel)[:max_masks_per_dim])
+        pooled = []
+        for mi in pick:
+            for qp in q_pos:
+                row = dist_row(Xs, masks[mi], qp)[c_pos]
+                keep = c_pos != qp
+                pooled.append(row[keep])
+        pooled = np.concatenate(pooled)
+        eps[sel] = np.quantile(pooled, frac)
+    return eps

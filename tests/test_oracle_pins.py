@@ -1,0 +1,258 @@
+"""Pins for the fp64 oracle against what the paper and the mathematics fix
+(SURVEY.md 8(c) "What pins each part"): closed forms, a library routine,
+exhaustive enumeration, invariants.  None of these re-types the oracle's loop."""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.spatial import cKDTree
+from scipy.special import comb
+
+import workloads
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+# ---------------------------------------------------------------- Eq. 1
+def test_eq1_mask_count():
+    # PAPER.md:142 Eq. 1: sum_{i=2}^{15} C(15,i) = 32,752
+    m = workloads.all_masks(15)
+    assert len(m) == 32752 == (1 << 15) - 1 - 15
+    assert len(set(m.tolist())) == 32752
+    assert (workloads.popcount(m) >= 2).all()
+    assert len(workloads.all_masks(4)) == 11  # BASELINE.json configs[0]
+    assert len(workloads.pair_masks_plus_full(15)) == 106
+
+
+def test_table2_internal_consistency():
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "table2_paper.txt"))
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) == 10
+    assert sum(int(r[5]) for r in rows) == 30          # N*k directed edges
+    assert sum(int(r[1]) for r in rows) % 2 == 0       # symmetric eps-join
+    assert all(float(r[3]) <= 0.67 for r in rows)      # mean of distances <= eps
+    assert [r for r in rows if int(r[1]) == 0][0][3] == "0.0000"  # reading A6
+
+
+# ---------------------------------------------------------------- distance closed forms
+def test_one_feature_and_duplicated_column(oracle_mod):
+    rng = np.random.default_rng(5)
+    X = rng.random((40, 4)).astype(np.float32)
+    X[:, 2] = X[:, 1]                                   # column 2 := column 1
+    for i in (0, 7, 39):
+        d1 = oracle_mod.dist_row(X, 0b0010, i)
+        np.testing.assert_allclose(d1, np.abs(X[:, 1].astype(np.float64) - float(X[i, 1])), rtol=1e-15)
+        d2 = oracle_mod.dist_row(X, 0b0110, i)
+        np.testing.assert_allclose(d2, math.sqrt(2.0) * d1, rtol=1e-15)
+        # a transposed operand / wrong column would break this one
+        d3 = oracle_mod.dist_row(X, 0b1001, i)
+        ref = np.hypot(X[:, 0].astype(np.float64) - float(X[i, 0]), X[:, 3].astype(np.float64) - float(X[i, 3]))
+        np.testing.assert_allclose(d3, ref, rtol=1e-15)
+
+
+def test_power_of_two_scaling_is_exact(oracle_mod):
+    rng = np.random.default_rng(6)
+    X = rng.random((30, 3)).astype(np.float32)
+    idx_a, d_a = oracle_mod.knn_selfjoin(X, [0b111], 4)
+    idx_b, d_b = oracle_mod.knn_selfjoin(X * np.float32(0.25), [0b111], 4)
+    assert (idx_a == idx_b).all()
+    assert (d_b == 0.25 * d_a).all()
+
+
+# ---------------------------------------------------------------- 1-D lattice (closed form A)
+def test_lattice_closed_form(oracle_mod):
+    n, h, k = 64, 2.0 ** -7, 6
+    X = workloads.lattice_table(n, 3, h, seed=1)
+    idx, dist = oracle_mod.knn_selfjoin(X, [0b001], k)
+    kth, mean, indeg = oracle_mod.knn_scores(n, idx, dist)
+    for i in range(n):
+        # distances to the others are |i-j|*h; ties (i-r, i+r) go to the smaller id
+        others = sorted((abs(i - j) * h, j) for j in range(n) if j != i)[:k]
+        assert idx[0, i].tolist() == [j for _, j in others]
+        assert dist[0, i].tolist() == [d for d, _ in others]
+    interior = np.arange(k // 2, n - k // 2)
+    assert (kth[0, interior] == (k // 2) * h).all()
+    np.testing.assert_allclose(mean[0, interior], h * (k / 2 + 1) / 2, rtol=1e-15)
+    assert kth[0, 0] == k * h and mean[0, 0] == h * (k + 1) / 2          # boundary point
+    cnt, s, mu = oracle_mod.range_selfjoin(X, [0b001], [2.5 * h])
+    assert (cnt[0, 2:-2] == 4).all() and cnt[0, 0] == 2 and cnt[0, 1] == 3
+    np.testing.assert_allclose(s[0, 2:-2], 6 * h, rtol=1e-15)
+    # closed ball (reading A2): eps exactly on a lattice distance includes it
+    cnt2, _, _ = oracle_mod.range_selfjoin(X, [0b001], [2.0 * h])
+    assert (cnt2[0, 2:-2] == 4).all()
+
+
+# ---------------------------------------------------------------- hypercube (closed form B, ties)
+@pytest.mark.parametrize("nf", [6, 9])
+def test_hypercube_counts_and_order_statistics(oracle_mod, nf):
+    X = workloads.hypercube_table(nf)
+    n = 1 << nf
+    rng = np.random.default_rng(nf)
+    masks = rng.choice(workloads.all_masks(nf, 1), 6, replace=False)
+    for eps in (0.5, 1.0, 1.5, 2.01):
+        cnt, s, mu = oracle_mod.range_selfjoin(X, masks, np.full(len(masks), eps))
+        for mi, m in enumerate(masks):
+            d = bin(int(m)).count("1")
+            mult = 1 << (nf - d)
+            exp_cnt = sum(comb(d, r, exact=True) * mult for r in range(d + 1) if math.sqrt(r) <= eps) - 1
+            exp_sum = sum(comb(d, r, exact=True) * mult * math.sqrt(r) for r in range(d + 1) if math.sqrt(r) <= eps)
+            assert (cnt[mi] == exp_cnt).all()
+            np.testing.assert_allclose(s[mi], exp_sum, rtol=1e-12)
+            np.testing.assert_allclose(mu[mi], exp_sum / exp_cnt if exp_cnt else 0.0, rtol=1e-12)
+    k = 10
+    idx, dist = oracle_mod.knn_selfjoin(X, masks, k)
+    for mi, m in enumerate(masks):
+        d = bin(int(m)).count("1")
+        mult = 1 << (nf - d)
+        levels = []                                    # sorted distance multiset of any vertex
+        for r in range(d + 1):
+            levels += [math.sqrt(r)] * (comb(d, r, exact=True) * mult - (1 if r == 0 else 0))
+        assert (dist[mi] == np.array(levels[:k])).all()
+        assert (idx[mi] != np.arange(n)[:, None]).all()  # self excluded by index (A4)
+        # tie-break to smaller id (A3): zero-distance twins are listed first, ascending id
+        n_zero = min(k, mult - 1)
+        if n_zero:
+            twins = np.sort(idx[mi][:, :n_zero], axis=1)
+            assert (twins == idx[mi][:, :n_zero]).all()
+
+
+# ---------------------------------------------------------------- library routine (scipy cKDTree)
+@pytest.mark.parametrize("seed,n,nf", [(0, 300, 5), (1, 257, 15)])
+def test_against_ckdtree(oracle_mod, seed, n, nf):
+    X = workloads.make_table(n, seed, cols=list(range(nf)))
+    rng = np.random.default_rng(seed)
+    masks = rng.choice(workloads.all_masks(nf), 5, replace=False)
+    k = 7
+    idx, dist = oracle_mod.knn_selfjoin(X, masks, k)
+    eps = np.array([np.median(dist[mi, :, -1]) for mi in range(len(masks))])
+    cnt, s, mu = oracle_mod.range_selfjoin(X, masks, eps)
+    for mi, m in enumerate(masks):
+        cols = [f for f in range(nf) if (int(m) >> f) & 1]
+        sub = X[:, cols].astype(np.float64)
+        tree = cKDTree(sub)
+        dd, ii = tree.query(sub, k=k + 1)
+        # continuous data: no exact ties, self is the 0-distance hit in column 0
+        assert (ii[:, 0] == np.arange(n)).all()
+        assert (idx[mi] == ii[:, 1:]).all()
+        np.testing.assert_allclose(dist[mi], dd[:, 1:], rtol=1e-12)
+        balls = tree.query_ball_point(sub, eps[mi] * (1 + 1e-12))
+        lib_cnt = np.array([len(b) - 1 for b in balls])
+        assert (cnt[mi] == lib_cnt).all()
+        lib_sum = np.array([np.linalg.norm(sub[b] - sub[i], axis=1).sum() for i, b in enumerate(balls)])
+        np.testing.assert_allclose(s[mi], lib_sum, rtol=1e-10, atol=1e-14)
+
+
+# ---------------------------------------------------------------- exhaustive, tiny N
+def test_knn_exhaustive_enumeration(oracle_mod):
+    rng = np.random.default_rng(11)
+    for trial in range(5):
+        n = int(rng.integers(4, 9))
+        X = np.round(rng.random((n, 3)) * 4).astype(np.float32) / 4      # coarse grid => ties
+        for k in (1, 2, 3):
+            for m in (0b001, 0b011, 0b111, 0b110):
+                idx, dist = oracle_mod.knn_selfjoin(X, [m], k)
+                cols = [f for f in range(3) if (m >> f) & 1]
+                for i in range(n):
+                    others = [j for j in range(n) if j != i]
+                    best = None
+                    for sub in itertools.combinations(others, k):
+                        key = sorted((float(np.sqrt(((X[i, cols].astype(np.float64) - X[j, cols]) ** 2).sum())), j)
+                                     for j in sub)
+                        if best is None or key < best:
+                            best = key
+                    assert [j for _, j in best] == idx[0, i].tolist()
+                    np.testing.assert_allclose([d for d, _ in best], dist[0, i], rtol=1e-15)
+
+
+# ---------------------------------------------------------------- invariants
+def test_invariants_on_config1(oracle_mod):
+    cfg = workloads.get_config("c1_tiny")
+    X, masks, k = cfg.table(), cfg.masks(), cfg.k
+    n = len(X)
+    idx, dist = oracle_mod.knn_selfjoin(X, masks, k)
+    kth, mean, indeg = oracle_mod.knn_scores(n, idx, dist)
+    assert (indeg.sum(axis=1) == n * k).all()
+    assert (np.diff(dist, axis=2) >= 0).all()
+    assert (mean <= kth + 1e-15).all()
+    assert (idx != np.arange(n)[None, :, None]).all()
+    assert all(len(set(r)) == k for r in idx.reshape(-1, k).tolist())
+    # order statistics are monotone along lattice edges S -> S u {f}
+    pos = {int(m): i for i, m in enumerate(masks)}
+    for m in masks:
+        for f in range(4):
+            if not (int(m) >> f) & 1 and (int(m) | (1 << f)) in pos:
+                assert (dist[pos[int(m)]] <= dist[pos[int(m) | (1 << f)]] + 1e-15).all()
+    # eps-join: symmetric, nested in eps, consistent with kNN ranks
+    eps = np.array([np.median(kth[mi]) for mi in range(len(masks))])
+    cnt, s, mu = oracle_mod.range_selfjoin(X, masks, eps)
+    cnt_small, _, _ = oracle_mod.range_selfjoin(X, masks, 0.5 * eps)
+    assert (cnt.sum(axis=1) % 2 == 0).all()                          # pair (i,j) <=> (j,i)
+    assert (cnt_small <= cnt).all()                                  # PAPER.md:235 Fig. 3 nesting
+    for m in masks:
+        for f in range(4):
+            if not (int(m) >> f) & 1 and (int(m) | (1 << f)) in pos:
+                a, b = pos[int(m)], pos[int(m) | (1 << f)]
+                c_sup, _, _ = oracle_mod.range_selfjoin(X, [masks[b]], [eps[a]])
+                assert (c_sup[0] <= cnt[a]).all()
+    for mi in (0, 5, 10):
+        for i in (0, 17, 1999):
+            c_at, _, _ = oracle_mod.range_selfjoin(X, [masks[mi]], [kth[mi, i]], queries=[i])
+            assert c_at[0, 0] >= k
+            c_below, _, _ = oracle_mod.range_selfjoin(X, [masks[mi]], [kth[mi, i] * (1 - 1e-12)], queries=[i])
+            assert c_below[0, 0] <= k - 1 or kth[mi, i] == 0.0
+    assert (mu[cnt == 0] == 0).all() and (s[cnt == 0] == 0).all()
+
+
+def test_permutation_equivariance(oracle_mod):
+    X = workloads.make_table(200, 9, cols=[0, 1, 2, 3, 4])
+    masks = np.array([0b00110, 0b11001, 0b11111], dtype=np.uint16)
+    idx, dist = oracle_mod.knn_selfjoin(X, masks, 5)
+    rng = np.random.default_rng(3)
+    perm = rng.permutation(200)
+    idx_p, dist_p = oracle_mod.knn_selfjoin(X[perm], masks, 5)
+    np.testing.assert_array_equal(dist_p, dist[:, perm])
+    assert (perm[idx_p] == idx[:, perm]).all()
+    cperm = np.array([3, 0, 4, 1, 2])                     # new column c holds old column cperm[c]
+    masks_p = np.array([sum(1 << c for c in range(5) if (int(m) >> cperm[c]) & 1) for m in masks], dtype=np.uint16)
+    idx_c, dist_c = oracle_mod.knn_selfjoin(X[:, cperm], masks_p, 5)
+    assert (idx_c == idx).all()
+    np.testing.assert_allclose(dist_c, dist, rtol=1e-14)
+
+
+def test_sampled_queries_equal_full_rows(oracle_mod):
+    X = workloads.make_table(150, 2, cols=[0, 1, 2])
+    masks = workloads.all_masks(3)
+    idx, dist = oracle_mod.knn_selfjoin(X, masks, 4)
+    q = np.array([149, 3, 77])
+    idx_q, dist_q = oracle_mod.knn_selfjoin(X, masks, 4, queries=q)
+    assert (idx_q == idx[:, q]).all() and (dist_q == dist[:, q]).all()
+
+
+def test_duplicate_block_self_exclusion(oracle_mod):
+    # reading A4/A7: a different object at distance 0 is a neighbour; self never is
+    X = workloads.duplicate_block_table(400, 3, frac=0.3)
+    m = np.array([(1 << 13) | (1 << 14)], dtype=np.uint16)
+    idx, dist = oracle_mod.knn_selfjoin(X, m, 8)
+    vals, counts = np.unique(X[:, 13], return_counts=True)
+    block_val = vals[np.argmax(counts)]
+    block = np.flatnonzero((X[:, 13] == block_val) & (X[:, 14] == X[np.argmax(X[:, 13] == block_val), 14]))
+    assert len(block) >= 100
+    assert (dist[0, block] == 0).all()
+    assert (idx[0, block] != block[:, None]).all()
+    # smallest ids of the block, skipping self
+    for i in block[:5]:
+        assert idx[0, i].tolist() == [j for j in block.tolist() if j != i][:8]
+
+
+def test_oracle_rejects_bad_arguments(oracle_mod):
+    X = np.zeros((5, 3), dtype=np.float32)
+    with pytest.raises(ValueError):
+        oracle_mod.knn_selfjoin(X, [0b111], 5)            # k <= N-1 (A9)
+    with pytest.raises(ValueError):
+        oracle_mod.knn_selfjoin(X, [0], 2)                # empty mask
+    with pytest.raises(ValueError):
+        oracle_mod.knn_selfjoin(X, [0b1000], 2)           # bit >= n_feat
+    with pytest.raises(ValueError):
+        oracle_mod.range_selfjoin(X, [0b1], [0.0])        # eps > 0
