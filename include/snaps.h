@@ -1,0 +1,178 @@
+/*
+ * snaps.h -- C ABI of libsnaps: the data-parallel hot path of SNAPS population
+ * outlier detection (arXiv 2405.20176) on one B200 (sm_100a).
+ *
+ * Citations are lines of /root/reference/PAPER.md.  "Readings" A1..A19 are the
+ * interpretations listed in DESIGN.md.
+ *
+ * Conventions for every entry point
+ *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  Output
+ *     pointers named out_* are device pointers unless stated otherwise.
+ *   - The caller owns every buffer; the library allocates nothing that
+ *     outlives a call and never frees caller memory.  Scratch comes from
+ *     d_workspace (size from snaps_workspace_bytes with the same N, n_feat,
+ *     n_masks, k).
+ *   - All device work is enqueued on `stream` (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream).  The call returns when the
+ *     work is enqueued; host-side planning may block the calling thread but
+ *     never synchronises the device.  "stream complete" => all outputs final.
+ *   - Return value: SNAPS_OK or an error code; argument errors are detected
+ *     before any launch.  snaps_last_error() gives a thread-local message.
+ *   - X is row-major, N rows (objects), n_feat columns (features), row stride
+ *     ld floats, fp32, normalised to [0,1] by the caller.  NaN
+ *     in X is undefined behaviour (the paper removes NaNs first).
+ *   - A subspace ("feature space") is a uint16 bitmask: bit j
+ *     set <=> column j is used.  Masks must be non-zero with no bit >= n_feat.
+ *   - Distances are Euclidean on the masked columns (reading A1), computed in
+ *     fp32 by direct differences ("32-bit floating point").
+ *   - Results do not depend on batching, tile sizes or scheduling; kNN ties
+ *     are broken by the smaller object id (reading A3).
+ */
+#ifndef SNAPS_H
+#define SNAPS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef int snaps_status;
+#define SNAPS_OK 0
+#define SNAPS_INVALID_ARG 1
+#define SNAPS_CUDA_ERROR 2
+#define SNAPS_WORKSPACE_TOO_SMALL 3
+#define SNAPS_UNSUPPORTED 4
+
+#define SNAPS_MAX_FEATURES 15 /* PAPER.md:109 "We examine d <= 15" */
+#define SNAPS_MAX_K 32
+
+/* Message for the last non-OK status on this thread (static storage). */
+const char *snaps_last_error(void);
+
+/* Library version string (static storage). */
+const char *snaps_version(void);
+
+/*
+ * Bytes of device scratch the joins need for these sizes (table staged as
+ * 80-byte rows, per-query candidate seeds, batch descriptors).  k may be 0
+ * for the range join.  Returns 0 on invalid sizes.
+ */
+size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k);
+
+/*
+ * Number of (ordered query-candidate pair, mask) distance evaluations the
+ * join kernels perform for this mask list, INCLUDING the lattice slots the
+ * planner computes but does not output; the algorithmic count is
+ * N*(N)*n_masks.  Used by bench.py's roofline arithmetic.  h_masks: host.
+ */
+int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t *h_masks, int n_masks);
+
+/*
+ * kNN self-join, kNNSJ (section 3.6): for every mask S and
+ * every object i, the k objects j != i with the smallest (D(i,j;S), j).
+ * Self is excluded by index (reading A4): a different object at
+ * distance 0 is a neighbour.
+ *
+ *   d_X        device, [N][ld] fp32
+ *   h_masks    host, [n_masks] uint16
+ *   k          1 <= k <= min(N-1, SNAPS_MAX_K)
+ *   out_idx    device or pinned host, [n_masks][N][k] int32 neighbour ids,
+ *              ascending by (distance, id); may be NULL
+ *   out_dist   device or pinned host, [n_masks][N][k] fp32 distances D (not
+ *              D^2), ascending; may be NULL
+ *   out_kth    device, [n_masks][N] fp32, D_(k): k-th-neighbour distance
+ *              (BASELINE.json configs[0], reading A11); may be NULL
+ *   out_mean   device, [n_masks][N] fp32, (1/k) sum_r D_(r): the distance-aware
+ *              kNN metric (reading A5); may be NULL
+ *   out_indeg  device, [n_masks][N] int32, in-degree of the kNN graph: number
+ *              of objects that list i among their kNN, the distance-oblivious
+ *              metric; ZEROED by the call; may be NULL
+ *
+ * Scores-only operation (out_idx == out_dist == NULL) is supported because
+ * the lists of the all-subspace run are 83 GB.  Errors: SNAPS_INVALID_ARG for
+ * N < 2, n_feat outside 1..15, ld < n_feat, NULL d_X/h_masks, n_masks < 1, a
+ * zero mask or a mask bit >= n_feat, k outside its range, d_X not 4-byte
+ * aligned, all five outputs NULL; SNAPS_WORKSPACE_TOO_SMALL; SNAPS_CUDA_ERROR.
+ */
+snaps_status snaps_knn_selfjoin(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                const uint16_t *h_masks, int n_masks, int k,
+                                int32_t *out_idx, float *out_dist,
+                                float *out_kth, float *out_mean, int32_t *out_indeg,
+                                void *d_workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * eps range self-join, DSSJ (section 3.5): for
+ * every mask S and object i, the objects j != i with D(i,j;S) <= eps_S
+ * (closed ball, reading A2; pairs within 1e-6 relative of eps may fall on
+ * either side in fp32).
+ *
+ *   h_eps        host, [n_masks] fp32, each finite and > 0
+ *   out_count    device, [n_masks][N] uint32: number of neighbours within eps,
+ *                self excluded = the distance-oblivious DSSJ
+ *                metric; required
+ *   out_sumdist  device, [n_masks][N] fp32: sum of D over those neighbours
+ *                (numerator of the distance-aware metric); may be
+ *                NULL
+ *   out_mean     device, [n_masks][N] fp32: sumdist/count, 0 when count == 0
+ *                (reading A6); may be NULL
+ */
+snaps_status snaps_range_selfjoin(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                  const uint16_t *h_masks, int n_masks, const float *h_eps,
+                                  uint32_t *out_count, float *out_sumdist, float *out_mean,
+                                  void *d_workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Per-object outlier scores from join outputs already on the device
+ * (PAPER.md:164-165, 251-252).  Any input group and any output may be NULL.
+ *
+ *   knn_idx, knn_dist   [n_masks][N][k] as written by snaps_knn_selfjoin
+ *   eps_count, eps_sumdist  [n_masks][N] as written by snaps_range_selfjoin
+ *   out_kth, out_knn_mean   [n_masks][N] fp32 (need knn_dist)
+ *   out_indegree            [n_masks][N] int32 (needs knn_idx); zeroed here
+ *   out_eps_mean            [n_masks][N] fp32 = sumdist/count, 0 if count == 0
+ */
+snaps_status snaps_outlier_scores(int64_t N, int n_masks, int k,
+                                  const int32_t *knn_idx, const float *knn_dist,
+                                  const uint32_t *eps_count, const float *eps_sumdist,
+                                  float *out_kth, float *out_knn_mean, int32_t *out_indegree,
+                                  float *out_eps_mean, void *stream);
+
+/*
+ * Batched ("oversubscribed") kNN self-join for outputs that
+ * exceed device memory: masks are processed in groups of masks_per_batch; each
+ * group's lists and scores are produced into a device staging ring inside
+ * d_workspace and copied on a side stream into the caller's PINNED HOST
+ * buffers while the next group computes.
+ *
+ *   h_out_*   pinned host buffers with the shapes of snaps_knn_selfjoin's
+ *             outputs; any may be NULL (at least one non-NULL)
+ *   masks_per_batch  >= 1; workspace must hold snaps_workspace_bytes(...) +
+ *             snaps_stream_ring_bytes(N, k, masks_per_batch)
+ * `stream` completes only after the last host copy has landed.
+ */
+size_t snaps_stream_ring_bytes(int64_t N, int k, int masks_per_batch);
+
+snaps_status snaps_knn_selfjoin_streamed(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                         const uint16_t *h_masks, int n_masks, int k,
+                                         int masks_per_batch,
+                                         int32_t *h_out_idx, float *h_out_dist,
+                                         float *h_out_kth, float *h_out_mean,
+                                         int32_t *h_out_indeg,
+                                         void *d_workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Peak-rate probe used for the roofline denominator:
+ * runs an FP32 instruction-throughput microkernel on `stream` and returns the
+ * measured warp-instruction lane rate.  kind: 0 = FFMA (3-register), 1 = FADD,
+ * 2 = FADD + FSETP pairs (the join's inner-loop mix).  *h_lane_ops_per_s
+ * receives executed lane-ops per second (one FFMA counts as ONE lane-op).
+ * Synchronises `stream`.
+ */
+snaps_status snaps_probe_fp32_rate(int kind, double *h_lane_ops_per_s, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SNAPS_H */

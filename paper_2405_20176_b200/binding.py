@@ -1,0 +1,225 @@
+"""ctypes binding for libsnaps.so -- same names as include/snaps.h, marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+EXPORTED_SYMBOLS = [
+    "snaps_last_error", "snaps_version", "snaps_workspace_bytes", "snaps_planned_evals",
+    "snaps_knn_selfjoin", "snaps_range_selfjoin", "snaps_outlier_scores",
+    "snaps_stream_ring_bytes", "snaps_knn_selfjoin_streamed", "snaps_probe_fp32_rate",
+]
+
+_lib = None
+
+
+class SnapsError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"snaps status {status}: {message}")
+        self.status = status
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Load libsnaps.so (building it in-tree if missing).  Fails loudly if it cannot."""
+    global _lib
+    if _lib is None:
+        path = _build.build()
+        L = ctypes.CDLL(path)
+        i64, i32, vp, sz = ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_size_t
+        L.snaps_last_error.restype = ctypes.c_char_p
+        L.snaps_version.restype = ctypes.c_char_p
+        L.snaps_workspace_bytes.restype = sz
+        L.snaps_workspace_bytes.argtypes = [i64, i32, i32, i32]
+        L.snaps_planned_evals.restype = i64
+        L.snaps_planned_evals.argtypes = [i64, i32, vp, i32]
+        L.snaps_knn_selfjoin.restype = i32
+        L.snaps_knn_selfjoin.argtypes = [vp, i64, i32, i64, vp, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.snaps_range_selfjoin.restype = i32
+        L.snaps_range_selfjoin.argtypes = [vp, i64, i32, i64, vp, i32, vp, vp, vp, vp, vp, sz, vp]
+        L.snaps_outlier_scores.restype = i32
+        L.snaps_outlier_scores.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+        L.snaps_stream_ring_bytes.restype = sz
+        L.snaps_stream_ring_bytes.argtypes = [i64, i32, i32]
+        L.snaps_knn_selfjoin_streamed.restype = i32
+        L.snaps_knn_selfjoin_streamed.argtypes = [vp, i64, i32, i64, vp, i32, i32, i32,
+                                                  vp, vp, vp, vp, vp, vp, sz, vp]
+        L.snaps_probe_fp32_rate.restype = i32
+        L.snaps_probe_fp32_rate.argtypes = [i32, ctypes.POINTER(ctypes.c_double), vp]
+        _lib = L
+    return _lib
+
+
+def _check(status: int):
+    if status != 0:
+        raise SnapsError(status, lib().snaps_last_error().decode())
+
+
+def version() -> str:
+    return lib().snaps_version().decode()
+
+
+def _masks(masks) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(masks, dtype=np.uint16).ravel())
+
+
+def _dptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def workspace_bytes(N: int, n_feat: int, n_masks: int, k: int) -> int:
+    return int(lib().snaps_workspace_bytes(N, n_feat, n_masks, k))
+
+
+def stream_ring_bytes(N: int, k: int, masks_per_batch: int) -> int:
+    return int(lib().snaps_stream_ring_bytes(N, k, masks_per_batch))
+
+
+def planned_evals(N: int, n_feat: int, masks) -> int:
+    m = _masks(masks)
+    return int(lib().snaps_planned_evals(N, n_feat, m.ctypes.data_as(ctypes.c_void_p), len(m)))
+
+
+def _workspace(X, n_masks, k, extra=0):
+    import torch
+    nbytes = workspace_bytes(X.shape[0], X.shape[1], n_masks, k) + extra
+    if nbytes == 0:
+        raise SnapsError(1, "invalid sizes for workspace")
+    return torch.empty(nbytes, dtype=torch.uint8, device=X.device)
+
+
+def knn_selfjoin(X, masks, k, *, lists=True, scores=True, out=None, workspace=None, stream=None):
+    """snaps_knn_selfjoin on a CUDA fp32 tensor X [N, n_feat].
+
+    Returns a dict with idx/dist [n_masks, N, k] (if lists) and kth/mean/indeg [n_masks, N]
+    (if scores), all torch CUDA tensors.  `out` may supply preallocated tensors by those names."""
+    import torch
+    assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
+    m = _masks(masks)
+    N, n_feat = X.shape
+    out = dict(out or {})
+    dev = X.device
+    if lists:
+        out.setdefault("idx", torch.empty((len(m), N, k), dtype=torch.int32, device=dev))
+        out.setdefault("dist", torch.empty((len(m), N, k), dtype=torch.float32, device=dev))
+    if scores:
+        out.setdefault("kth", torch.empty((len(m), N), dtype=torch.float32, device=dev))
+        out.setdefault("mean", torch.empty((len(m), N), dtype=torch.float32, device=dev))
+        out.setdefault("indeg", torch.empty((len(m), N), dtype=torch.int32, device=dev))
+    ws = workspace if workspace is not None else _workspace(X, len(m), k)
+    _check(lib().snaps_knn_selfjoin(
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m), k,
+        _dptr(out.get("idx")), _dptr(out.get("dist")), _dptr(out.get("kth")),
+        _dptr(out.get("mean")), _dptr(out.get("indeg")), _dptr(ws), ws.numel(), _stream(stream)))
+    out["_workspace"] = ws
+    return out
+
+
+def range_selfjoin(X, masks, eps, *, sums=True, out=None, workspace=None, stream=None):
+    """snaps_range_selfjoin: returns dict count [n_masks, N] (int32 view of uint32) and, if
+    sums, sumdist / mean."""
+    import torch
+    assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
+    m = _masks(masks)
+    e = np.ascontiguousarray(np.asarray(eps, dtype=np.float32).ravel())
+    assert len(e) == len(m)
+    N, n_feat = X.shape
+    out = dict(out or {})
+    dev = X.device
+    out.setdefault("count", torch.empty((len(m), N), dtype=torch.int32, device=dev))
+    if sums:
+        out.setdefault("sumdist", torch.empty((len(m), N), dtype=torch.float32, device=dev))
+        out.setdefault("mean", torch.empty((len(m), N), dtype=torch.float32, device=dev))
+    ws = workspace if workspace is not None else _workspace(X, len(m), 0)
+    _check(lib().snaps_range_selfjoin(
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
+        e.ctypes.data_as(ctypes.c_void_p), _dptr(out["count"]), _dptr(out.get("sumdist")),
+        _dptr(out.get("mean")), _dptr(ws), ws.numel(), _stream(stream)))
+    out["_workspace"] = ws
+    return out
+
+
+def outlier_scores(N, n_masks, k, *, knn_idx=None, knn_dist=None, eps_count=None, eps_sumdist=None,
+                   stream=None):
+    """snaps_outlier_scores from join outputs on the device."""
+    import torch
+    ref = next(t for t in (knn_idx, knn_dist, eps_count, eps_sumdist) if t is not None)
+    dev = ref.device
+    out = {}
+    if knn_dist is not None:
+        out["kth"] = torch.empty((n_masks, N), dtype=torch.float32, device=dev)
+        out["mean"] = torch.empty((n_masks, N), dtype=torch.float32, device=dev)
+    if knn_idx is not None:
+        out["indeg"] = torch.empty((n_masks, N), dtype=torch.int32, device=dev)
+    if eps_count is not None and eps_sumdist is not None:
+        out["eps_mean"] = torch.empty((n_masks, N), dtype=torch.float32, device=dev)
+    _check(lib().snaps_outlier_scores(
+        N, n_masks, k, _dptr(knn_idx), _dptr(knn_dist), _dptr(eps_count), _dptr(eps_sumdist),
+        _dptr(out.get("kth")), _dptr(out.get("mean")), _dptr(out.get("indeg")),
+        _dptr(out.get("eps_mean")), _stream(stream)))
+    return out
+
+
+def knn_selfjoin_streamed(X, masks, k, masks_per_batch, *, lists=True, scores=True, out=None,
+                          workspace=None, stream=None):
+    """snaps_knn_selfjoin_streamed: outputs land in PINNED HOST tensors."""
+    import torch
+    assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
+    m = _masks(masks)
+    N, n_feat = X.shape
+    out = dict(out or {})
+
+    def pinned(shape, dtype):
+        return torch.empty(shape, dtype=dtype, pin_memory=True)
+
+    if lists:
+        out.setdefault("idx", pinned((len(m), N, k), torch.int32))
+        out.setdefault("dist", pinned((len(m), N, k), torch.float32))
+    if scores:
+        out.setdefault("kth", pinned((len(m), N), torch.float32))
+        out.setdefault("mean", pinned((len(m), N), torch.float32))
+        out.setdefault("indeg", pinned((len(m), N), torch.int32))
+    for t in out.values():
+        assert t.is_pinned()
+    ws = workspace if workspace is not None else _workspace(
+        X, len(m), k, extra=stream_ring_bytes(N, k, masks_per_batch))
+    _check(lib().snaps_knn_selfjoin_streamed(
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m), k,
+        masks_per_batch, _dptr(out.get("idx")), _dptr(out.get("dist")), _dptr(out.get("kth")),
+        _dptr(out.get("mean")), _dptr(out.get("indeg")), _dptr(ws), ws.numel(), _stream(stream)))
+    out["_workspace"] = ws
+    return out
+
+
+def knn_selfjoin_host(X_host, masks, k, masks_per_batch=None, *, lists=False, scores=True, stream=None):
+    """End-to-end call with HOST buffers: pinned X -> device, join, pinned host outputs.
+    Returns the dict of pinned host tensors after the stream is enqueued (caller synchronises)."""
+    import torch
+    Xh = torch.as_tensor(X_host)
+    if not Xh.is_pinned():
+        Xh = Xh.pin_memory()
+    Xd = Xh.to("cuda", non_blocking=True)
+    n_masks = len(_masks(masks))
+    mpb = masks_per_batch or max(1, min(n_masks, 2048))
+    out = knn_selfjoin_streamed(Xd, masks, k, mpb, lists=lists, scores=scores, stream=stream)
+    out["_X"] = Xd
+    return out
+
+
+def probe_fp32_rate(kind: int, stream=None) -> float:
+    v = ctypes.c_double(0.0)
+    _check(lib().snaps_probe_fp32_rate(kind, ctypes.byref(v), _stream(stream)))
+    return float(v.value)

@@ -1,0 +1,440 @@
+// api.cu -- C ABI of libsnaps (include/snaps.h): argument checks, the host-side mask-batch
+// planner (step a2), workspace carving, kernel launches and the pinned-host output ring (a8).
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <map>
+#include <vector>
+
+#include "../../include/snaps.h"
+#include "knn_lattice.cuh"
+#include "misc_kernels.cuh"
+#include "range_lattice.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+snaps_status fail(snaps_status code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                      \
+    do {                                                                                    \
+        cudaError_t e_ = (expr);                                                            \
+        if (e_ != cudaSuccess)                                                              \
+            return fail(SNAPS_CUDA_ERROR, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e_),  \
+                        __FILE__, __LINE__);                                                \
+    } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int n_tiles_for(int64_t N) { return static_cast<int>((N + snaps::kTileRows - 1) / snaps::kTileRows); }
+
+// Gray rank of the 9 high-feature bits: consecutive batches differ in one feature, which is
+// what makes the previous batch's neighbours good threshold seeds.
+uint32_t gray_rank(uint32_t gray) {
+    uint32_t b = gray;
+    for (uint32_t s = 1; s < 16; s <<= 1) b ^= b >> s;
+    return b;
+}
+
+// Step a2.  One batch per distinct set H of features 6..14; slot[T] = position of mask H|T.
+// A mask listed more than once gets a further batch with the same H.
+void plan_lattice(const uint16_t* masks, int n_masks, const float* thr,
+                  std::vector<snaps::BatchDesc>* out) {
+    std::map<uint32_t, std::vector<int>> by_h;  // gray rank of H -> batch indices
+    std::vector<snaps::BatchDesc>& B = *out;
+    B.clear();
+    for (int m = 0; m < n_masks; ++m) {
+        const uint32_t H = masks[m] & ~static_cast<uint32_t>(snaps::kLat - 1);
+        const int T = masks[m] & (snaps::kLat - 1);
+        std::vector<int>& lst = by_h[gray_rank(H >> snaps::kLow)];
+        int use = -1;
+        for (int bi : lst)
+            if (B[bi].slot[T] < 0) {
+                use = bi;
+                break;
+            }
+        if (use < 0) {
+            snaps::BatchDesc d;
+            d.hmask = H;
+            d.n_valid = 0;
+            for (int t = 0; t < snaps::kLat; ++t) {
+                d.slot[t] = -1;
+                d.thr[t] = -1.f;
+            }
+            B.push_back(d);
+            use = static_cast<int>(B.size()) - 1;
+            lst.push_back(use);
+        }
+        B[use].slot[T] = m;
+        B[use].n_valid += 1;
+        if (thr) B[use].thr[T] = thr[m];
+    }
+    std::vector<snaps::BatchDesc> ordered;
+    ordered.reserve(B.size());
+    for (auto& kv : by_h)
+        for (int bi : kv.second) ordered.push_back(B[bi]);
+    B.swap(ordered);
+}
+
+snaps_status check_common(const float* d_X, int64_t N, int n_feat, int64_t ld,
+                          const uint16_t* h_masks, int n_masks) {
+    if (!d_X) return fail(SNAPS_INVALID_ARG, "d_X is NULL");
+    if (reinterpret_cast<uintptr_t>(d_X) % 4 != 0) return fail(SNAPS_INVALID_ARG, "d_X not 4-byte aligned");
+    if (N < 2) return fail(SNAPS_INVALID_ARG, "N = %lld < 2", (long long)N);
+    if (N > (int64_t)1 << 30) return fail(SNAPS_UNSUPPORTED, "N = %lld > 2^30", (long long)N);
+    if (n_feat < 1 || n_feat > SNAPS_MAX_FEATURES)
+        return fail(SNAPS_INVALID_ARG, "n_feat = %d outside 1..15", n_feat);
+    if (ld < n_feat) return fail(SNAPS_INVALID_ARG, "ld = %lld < n_feat", (long long)ld);
+    if (!h_masks || n_masks < 1) return fail(SNAPS_INVALID_ARG, "no masks");
+    for (int m = 0; m < n_masks; ++m) {
+        if (h_masks[m] == 0) return fail(SNAPS_INVALID_ARG, "mask %d is zero", m);
+        if ((h_masks[m] >> n_feat) != 0)
+            return fail(SNAPS_INVALID_ARG, "mask %d (0x%x) has a bit >= n_feat", m, h_masks[m]);
+    }
+    return SNAPS_OK;
+}
+
+struct Workspace {
+    float* Xp;
+    int* counter;
+    snaps::BatchDesc* batches;
+    unsigned char* ring;   // rest
+    size_t ring_bytes;
+};
+
+size_t base_workspace_bytes(int64_t N, int n_masks) {
+    const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
+    const size_t batches = align_up(static_cast<size_t>(n_masks) * sizeof(snaps::BatchDesc), 256);
+    return table + 256 + batches;
+}
+
+snaps_status carve(void* d_ws, size_t bytes, int64_t N, int n_masks, Workspace* w) {
+    if (!d_ws) return fail(SNAPS_INVALID_ARG, "d_workspace is NULL");
+    if (reinterpret_cast<uintptr_t>(d_ws) % 256 != 0)
+        return fail(SNAPS_INVALID_ARG, "d_workspace not 256-byte aligned");
+    const size_t need = base_workspace_bytes(N, n_masks);
+    if (bytes < need)
+        return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", bytes, need);
+    unsigned char* p = static_cast<unsigned char*>(d_ws);
+    const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
+    w->Xp = reinterpret_cast<float*>(p);
+    w->counter = reinterpret_cast<int*>(p + table);
+    w->batches = reinterpret_cast<snaps::BatchDesc*>(p + table + 256);
+    w->ring = p + need;
+    w->ring_bytes = bytes - need;
+    return SNAPS_OK;
+}
+
+int sm_count() {
+    static int cached = 0;
+    if (!cached) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+            cached = n;
+        else
+            cached = 148;
+    }
+    return cached;
+}
+
+// Work decomposition: queries per CTA = consumer warps; batches are cut into chunks so that
+// there are enough (query block, chunk) items to balance the persistent CTAs, while chunks
+// stay long enough for threshold seeding from the previous batch to pay.
+void decompose(int64_t N, int n_batches, int warps, int grid, int* n_qblocks, int* bpi, int* n_bchunks) {
+    *n_qblocks = static_cast<int>((N + warps - 1) / warps);
+    int chunks = 1;
+    while (static_cast<int64_t>(*n_qblocks) * chunks < 24LL * grid && (n_batches + chunks) / (chunks + 1) >= 8)
+        ++chunks;
+    *bpi = (n_batches + chunks - 1) / chunks;
+    *n_bchunks = (n_batches + *bpi - 1) / *bpi;
+}
+
+int knn_warps_for(int k) {
+    // 227 KB of shared memory: tile ring + per-warp list state
+    const size_t budget = 227 * 1024;
+    int w = 15;
+    while (w > 1 && snaps::knn_lattice_smem_bytes(k, w) > budget) --w;
+    return w;
+}
+
+// Launch the kNN kernel over descriptors already uploaded at d_batches[0..nb).
+snaps_status knn_enqueue(const Workspace& w, const snaps::BatchDesc* d_batches, int nb, int64_t N, int k,
+                         int32_t* out_idx, float* out_dist, float* out_kth, float* out_mean,
+                         int32_t* out_indeg, cudaStream_t st) {
+    CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
+    snaps::KnnParams p;
+    p.Xp = w.Xp;
+    p.N = static_cast<int>(N);
+    p.n_tiles = n_tiles_for(N);
+    p.k = k;
+    p.batches = d_batches;
+    p.n_batches = nb;
+    p.warps = knn_warps_for(k);
+    const int grid_max = sm_count();
+    decompose(N, nb, p.warps, grid_max, &p.n_qblocks, &p.batches_per_item, &p.n_bchunks);
+    p.work_counter = w.counter;
+    p.out_idx = out_idx;
+    p.out_dist = out_dist;
+    p.out_kth = out_kth;
+    p.out_mean = out_mean;
+    p.out_indeg = out_indeg;
+    const int64_t items = static_cast<int64_t>(p.n_qblocks) * p.n_bchunks;
+    const int grid = static_cast<int>(std::min<int64_t>(items, grid_max));
+    CUDA_TRY(snaps::knn_lattice_launch(p, grid, st));
+    return SNAPS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* snaps_last_error(void) { return g_err; }
+
+const char* snaps_version(void) { return "snaps-b200 0.1 (sm_100a)"; }
+
+size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k) {
+    if (N < 2 || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES || n_masks < 1 || k < 0 || k > SNAPS_MAX_K)
+        return 0;
+    return base_workspace_bytes(N, n_masks);
+}
+
+int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t* h_masks, int n_masks) {
+    if (!h_masks || n_masks < 1 || N < 2 || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES) return -1;
+    std::vector<snaps::BatchDesc> b;
+    plan_lattice(h_masks, n_masks, nullptr, &b);
+    return static_cast<int64_t>(b.size()) * snaps::kLat * N * N;
+}
+
+snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t ld,
+                                const uint16_t* h_masks, int n_masks, int k, int32_t* out_idx,
+                                float* out_dist, float* out_kth, float* out_mean,
+                                int32_t* out_indeg, void* d_workspace, size_t workspace_bytes,
+                                void* stream) {
+    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    if (rc) return rc;
+    if (k < 1 || k > SNAPS_MAX_K || k > N - 1)
+        return fail(SNAPS_INVALID_ARG, "k = %d outside 1..min(N-1, %d)", k, SNAPS_MAX_K);
+    if (!out_idx && !out_dist && !out_kth && !out_mean && !out_indeg)
+        return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
+    Workspace w;
+    rc = carve(d_workspace, workspace_bytes, N, n_masks, &w);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::vector<snaps::BatchDesc> batches;
+    plan_lattice(h_masks, n_masks, nullptr, &batches);
+    const int n_tiles = n_tiles_for(N);
+    CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
+                                       n_tiles * snaps::kTileRows, st));
+    if (out_indeg)
+        CUDA_TRY(cudaMemsetAsync(out_indeg, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, st));
+    CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
+                             cudaMemcpyHostToDevice, st));
+    return knn_enqueue(w, w.batches, static_cast<int>(batches.size()), N, k, out_idx, out_dist, out_kth,
+                       out_mean, out_indeg, st);
+}
+
+snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t ld,
+                                  const uint16_t* h_masks, int n_masks, const float* h_eps,
+                                  uint32_t* out_count, float* out_sumdist, float* out_mean,
+                                  void* d_workspace, size_t workspace_bytes, void* stream) {
+    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    if (rc) return rc;
+    if (!h_eps) return fail(SNAPS_INVALID_ARG, "h_eps is NULL");
+    if (!out_count) return fail(SNAPS_INVALID_ARG, "out_count is NULL");
+    std::vector<float> thr(n_masks);
+    for (int m = 0; m < n_masks; ++m) {
+        if (!(h_eps[m] > 0.f) || !isfinite(h_eps[m]))
+            return fail(SNAPS_INVALID_ARG, "eps[%d] = %g is not finite and > 0", m, (double)h_eps[m]);
+        // D <= eps  <=>  D^2 <= eps^2: compare d^2 < nextafter(fl(eps^2)) (closed ball, reading A2)
+        const float e2 = static_cast<float>(static_cast<double>(h_eps[m]) * static_cast<double>(h_eps[m]));
+        thr[m] = nextafterf(e2, INFINITY);
+    }
+    Workspace w;
+    rc = carve(d_workspace, workspace_bytes, N, n_masks, &w);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::vector<snaps::BatchDesc> batches;
+    plan_lattice(h_masks, n_masks, thr.data(), &batches);
+    const int nb = static_cast<int>(batches.size());
+    const int n_tiles = n_tiles_for(N);
+    CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
+                                       n_tiles * snaps::kTileRows, st));
+    CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * nb,
+                             cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
+    snaps::RangeParams p;
+    p.Xp = w.Xp;
+    p.N = static_cast<int>(N);
+    p.n_tiles = n_tiles;
+    p.batches = w.batches;
+    p.n_batches = nb;
+    p.warps = 15;
+    const int grid_max = sm_count();
+    decompose(N, nb, p.warps, grid_max, &p.n_qblocks, &p.batches_per_item, &p.n_bchunks);
+    p.work_counter = w.counter;
+    p.out_count = out_count;
+    p.out_sum = out_sumdist;
+    p.out_mean = out_mean;
+    const int64_t items = static_cast<int64_t>(p.n_qblocks) * p.n_bchunks;
+    const int grid = static_cast<int>(std::min<int64_t>(items, grid_max));
+    CUDA_TRY(snaps::range_lattice_launch(p, grid, st));
+    return SNAPS_OK;
+}
+
+snaps_status snaps_outlier_scores(int64_t N, int n_masks, int k, const int32_t* knn_idx,
+                                  const float* knn_dist, const uint32_t* eps_count,
+                                  const float* eps_sumdist, float* out_kth, float* out_knn_mean,
+                                  int32_t* out_indegree, float* out_eps_mean, void* stream) {
+    if (N < 2 || n_masks < 1) return fail(SNAPS_INVALID_ARG, "bad sizes");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const bool want_knn = out_kth || out_knn_mean || out_indegree;
+    if (want_knn) {
+        if (k < 1 || k > SNAPS_MAX_K) return fail(SNAPS_INVALID_ARG, "k = %d outside 1..%d", k, SNAPS_MAX_K);
+        if ((out_kth || out_knn_mean) && !knn_dist) return fail(SNAPS_INVALID_ARG, "knn_dist is NULL");
+        if (out_indegree && !knn_idx) return fail(SNAPS_INVALID_ARG, "knn_idx is NULL");
+        if (out_indegree)
+            CUDA_TRY(cudaMemsetAsync(out_indegree, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, st));
+        CUDA_TRY(snaps::knn_scores_launch(N, n_masks, k, knn_idx, knn_dist, out_kth, out_knn_mean,
+                                          out_indegree, st));
+    }
+    if (out_eps_mean) {
+        if (!eps_count || !eps_sumdist) return fail(SNAPS_INVALID_ARG, "eps inputs are NULL");
+        CUDA_TRY(snaps::eps_mean_launch(N * n_masks, eps_count, eps_sumdist, out_eps_mean, st));
+    }
+    if (!want_knn && !out_eps_mean) return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
+    return SNAPS_OK;
+}
+
+size_t snaps_stream_ring_bytes(int64_t N, int k, int masks_per_batch) {
+    if (N < 2 || k < 1 || masks_per_batch < 1) return 0;
+    // two staging slots, each: idx + dist lists and three score arrays for one mask group
+    const size_t per_mask = align_up(static_cast<size_t>(N) * (2 * static_cast<size_t>(k) + 3) * 4, 256) + 5 * 256;
+    return 2 * per_mask * static_cast<size_t>(masks_per_batch);
+}
+
+snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat, int64_t ld,
+                                         const uint16_t* h_masks, int n_masks, int k,
+                                         int masks_per_batch, int32_t* h_out_idx, float* h_out_dist,
+                                         float* h_out_kth, float* h_out_mean, int32_t* h_out_indeg,
+                                         void* d_workspace, size_t workspace_bytes, void* stream) {
+    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    if (rc) return rc;
+    if (k < 1 || k > SNAPS_MAX_K || k > N - 1)
+        return fail(SNAPS_INVALID_ARG, "k = %d outside 1..min(N-1, %d)", k, SNAPS_MAX_K);
+    if (masks_per_batch < 1) return fail(SNAPS_INVALID_ARG, "masks_per_batch < 1");
+    if (!h_out_idx && !h_out_dist && !h_out_kth && !h_out_mean && !h_out_indeg)
+        return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
+    Workspace w;
+    rc = carve(d_workspace, workspace_bytes, N, n_masks, &w);
+    if (rc) return rc;
+    const size_t ring_need = snaps_stream_ring_bytes(N, k, masks_per_batch);
+    if (w.ring_bytes < ring_need)
+        return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace ring %zu < %zu bytes", w.ring_bytes, ring_need);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int n_tiles = n_tiles_for(N);
+    CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
+                                       n_tiles * snaps::kTileRows, st));
+
+    const size_t mpb = static_cast<size_t>(masks_per_batch);
+    const size_t n_list = align_up(mpb * N * k * 4, 256);
+    const size_t n_score = align_up(mpb * N * 4, 256);
+    struct Slot {
+        int32_t* idx;
+        float* dist;
+        float* kth;
+        float* mean;
+        int32_t* indeg;
+    } slots[2];
+    unsigned char* r = w.ring;
+    for (int s = 0; s < 2; ++s) {
+        slots[s].idx = reinterpret_cast<int32_t*>(r); r += n_list;
+        slots[s].dist = reinterpret_cast<float*>(r); r += n_list;
+        slots[s].kth = reinterpret_cast<float*>(r); r += n_score;
+        slots[s].mean = reinterpret_cast<float*>(r); r += n_score;
+        slots[s].indeg = reinterpret_cast<int32_t*>(r); r += n_score;
+    }
+    // Plan every mask group up front and upload all descriptors with one copy, so that the
+    // loop below only enqueues (no host<->device synchronisation between groups).
+    std::vector<snaps::BatchDesc> all_batches;
+    std::vector<size_t> group_off;
+    for (int m0 = 0; m0 < n_masks; m0 += masks_per_batch) {
+        std::vector<snaps::BatchDesc> b;
+        plan_lattice(h_masks + m0, std::min(masks_per_batch, n_masks - m0), nullptr, &b);
+        group_off.push_back(all_batches.size());
+        all_batches.insert(all_batches.end(), b.begin(), b.end());
+    }
+    group_off.push_back(all_batches.size());
+    CUDA_TRY(cudaMemcpyAsync(w.batches, all_batches.data(), sizeof(snaps::BatchDesc) * all_batches.size(),
+                             cudaMemcpyHostToDevice, st));
+    cudaStream_t side;
+    CUDA_TRY(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
+    cudaEvent_t computed[2], copied[2];
+    for (int s = 0; s < 2; ++s) {
+        CUDA_TRY(cudaEventCreateWithFlags(&computed[s], cudaEventDisableTiming));
+        CUDA_TRY(cudaEventCreateWithFlags(&copied[s], cudaEventDisableTiming));
+    }
+    snaps_status result = SNAPS_OK;
+    int group = 0;
+    for (int m0 = 0; m0 < n_masks && result == SNAPS_OK; m0 += masks_per_batch, ++group) {
+        const int nm = std::min(masks_per_batch, n_masks - m0);
+        const int s = group & 1;
+        if (group >= 2) {
+            // staging slot s is free once its previous copy-out has finished
+            cudaError_t e = cudaStreamWaitEvent(st, copied[s], 0);
+            if (e != cudaSuccess) { result = fail(SNAPS_CUDA_ERROR, "cudaStreamWaitEvent: %s", cudaGetErrorString(e)); break; }
+        }
+        if (h_out_indeg) {
+            cudaError_t e = cudaMemsetAsync(slots[s].indeg, 0, sizeof(int32_t) * static_cast<size_t>(nm) * N, st);
+            if (e != cudaSuccess) { result = fail(SNAPS_CUDA_ERROR, "cudaMemsetAsync: %s", cudaGetErrorString(e)); break; }
+        }
+        result = knn_enqueue(w, w.batches + group_off[group],
+                             static_cast<int>(group_off[group + 1] - group_off[group]), N, k,
+                             h_out_idx ? slots[s].idx : nullptr,
+                             h_out_dist ? slots[s].dist : nullptr, h_out_kth ? slots[s].kth : nullptr,
+                             h_out_mean ? slots[s].mean : nullptr, h_out_indeg ? slots[s].indeg : nullptr, st);
+        if (result != SNAPS_OK) break;
+        cudaEventRecord(computed[s], st);
+        cudaStreamWaitEvent(side, computed[s], 0);
+        const size_t off_list = static_cast<size_t>(m0) * N * k, off_score = static_cast<size_t>(m0) * N;
+        const size_t b_list = static_cast<size_t>(nm) * N * k * 4, b_score = static_cast<size_t>(nm) * N * 4;
+        cudaError_t e = cudaSuccess;
+        if (h_out_idx && e == cudaSuccess) e = cudaMemcpyAsync(h_out_idx + off_list, slots[s].idx, b_list, cudaMemcpyDeviceToHost, side);
+        if (h_out_dist && e == cudaSuccess) e = cudaMemcpyAsync(h_out_dist + off_list, slots[s].dist, b_list, cudaMemcpyDeviceToHost, side);
+        if (h_out_kth && e == cudaSuccess) e = cudaMemcpyAsync(h_out_kth + off_score, slots[s].kth, b_score, cudaMemcpyDeviceToHost, side);
+        if (h_out_mean && e == cudaSuccess) e = cudaMemcpyAsync(h_out_mean + off_score, slots[s].mean, b_score, cudaMemcpyDeviceToHost, side);
+        if (h_out_indeg && e == cudaSuccess) e = cudaMemcpyAsync(h_out_indeg + off_score, slots[s].indeg, b_score, cudaMemcpyDeviceToHost, side);
+        if (e != cudaSuccess) { result = fail(SNAPS_CUDA_ERROR, "cudaMemcpyAsync D2H: %s", cudaGetErrorString(e)); break; }
+        cudaEventRecord(copied[s], side);
+    }
+    // the caller's stream completes only after the last copies have landed
+    for (int s = 0; s < 2 && s < group; ++s) cudaStreamWaitEvent(st, copied[s], 0);
+    for (int s = 0; s < 2; ++s) {
+        cudaEventDestroy(computed[s]);
+        cudaEventDestroy(copied[s]);
+    }
+    cudaStreamDestroy(side);
+    return result;
+}
+
+snaps_status snaps_probe_fp32_rate(int kind, double* h_lane_ops_per_s, void* stream) {
+    if (kind < 0 || kind > 2 || !h_lane_ops_per_s) return fail(SNAPS_INVALID_ARG, "bad probe arguments");
+    double ops = 0.0;
+    float ms = 0.f;
+    CUDA_TRY(snaps::probe_fp32_launch(kind, &ops, &ms, static_cast<cudaStream_t>(stream)));
+    *h_lane_ops_per_s = ops / (static_cast<double>(ms) * 1e-3);
+    return SNAPS_OK;
+}
+
+}  // extern "C"

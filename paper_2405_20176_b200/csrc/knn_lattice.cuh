@@ -1,0 +1,31 @@
+// knn_lattice.cuh -- launch interface of the sub-lattice kNN self-join kernel.
+#pragma once
+#include "snaps_device.cuh"
+
+namespace snaps {
+
+constexpr int kKnnMaxThreads = 512;  // (consumer warps + 1 producer warp) * 32
+
+struct KnnParams {
+    const float* Xp;            // staged table, n_tiles*128 rows of 20 floats
+    int N;
+    int n_tiles;
+    int k;
+    const BatchDesc* batches;   // device
+    int n_batches;
+    int batches_per_item;       // consecutive batches one warp keeps its query for
+    int n_bchunks;              // ceil(n_batches / batches_per_item)
+    int n_qblocks;              // ceil(N / warps)
+    int warps;                  // consumer warps per CTA (= queries per CTA)
+    int* work_counter;          // device, zeroed before launch
+    int32_t* out_idx;
+    float* out_dist;
+    float* out_kth;
+    float* out_mean;
+    int32_t* out_indeg;
+};
+
+size_t knn_lattice_smem_bytes(int k, int warps);
+cudaError_t knn_lattice_launch(const KnnParams& p, int grid, cudaStream_t stream);
+
+}  // namespace snaps

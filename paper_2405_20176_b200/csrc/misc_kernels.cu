@@ -1,0 +1,134 @@
+// misc_kernels.cu -- small kernels around the joins.
+#include "misc_kernels.cuh"
+#include "snaps_device.cuh"
+#include <algorithm>
+
+namespace snaps {
+
+// a1: N x n_feat (row stride ld) -> n_rows_padded x 20 floats, zero padded.
+__global__ void stage_table_kernel(const float* __restrict__ X, int64_t ld, int N, int n_feat,
+                                   float* __restrict__ Xp, int n_rows_padded) {
+    const int64_t total = static_cast<int64_t>(n_rows_padded) * kRowFloats;
+    for (int64_t i = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; i < total;
+         i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+        const int64_t r = i / kRowFloats;
+        const int j = static_cast<int>(i - r * kRowFloats);
+        Xp[i] = (r < N && j < n_feat) ? X[r * ld + j] : 0.f;
+    }
+}
+
+cudaError_t stage_table_launch(const float* X, int64_t ld, int N, int n_feat, float* Xp,
+                               int n_rows_padded, cudaStream_t stream) {
+    const int64_t total = static_cast<int64_t>(n_rows_padded) * kRowFloats;
+    const int grid = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 16));
+    stage_table_kernel<<<grid, 256, 0, stream>>>(X, ld, N, n_feat, Xp, n_rows_padded);
+    return cudaGetLastError();
+}
+
+// k-th and mean kNN distance, in-degree of the kNN graph.
+__global__ void knn_scores_kernel(int64_t N, int n_masks, int k, const int32_t* __restrict__ idx,
+                                  const float* __restrict__ dist, float* __restrict__ out_kth,
+                                  float* __restrict__ out_mean, int32_t* __restrict__ out_indeg) {
+    const int64_t total = N * n_masks;
+    for (int64_t o = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; o < total;
+         o += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+        const int64_t m = o / N;
+        if (dist) {
+            float sum = 0.f, dk = 0.f;
+            for (int e = 0; e < k; ++e) {
+                dk = dist[o * k + e];
+                sum += dk;
+            }
+            if (out_kth) out_kth[o] = dk;
+            if (out_mean) out_mean[o] = sum / static_cast<float>(k);
+        }
+        if (idx && out_indeg)
+            for (int e = 0; e < k; ++e) atomicAdd(&out_indeg[m * N + idx[o * k + e]], 1);
+    }
+}
+
+cudaError_t knn_scores_launch(int64_t N, int n_masks, int k, const int32_t* idx, const float* dist,
+                              float* out_kth, float* out_mean, int32_t* out_indeg,
+                              cudaStream_t stream) {
+    const int64_t total = N * n_masks;
+    const int grid = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 32));
+    knn_scores_kernel<<<grid, 256, 0, stream>>>(N, n_masks, k, idx, dist, out_kth, out_mean,
+                                                out_indeg);
+    return cudaGetLastError();
+}
+
+// mean distance to the eps-neighbours, 0 when there are none.
+__global__ void eps_mean_kernel(int64_t total, const uint32_t* __restrict__ cnt,
+                                const float* __restrict__ sum, float* __restrict__ out_mean) {
+    for (int64_t o = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; o < total;
+         o += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+        const uint32_t c = cnt[o];
+        out_mean[o] = c > 0 ? sum[o] / static_cast<float>(c) : 0.f;
+    }
+}
+
+cudaError_t eps_mean_launch(int64_t total, const uint32_t* cnt, const float* sum, float* out_mean,
+                            cudaStream_t stream) {
+    const int grid = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 32));
+    eps_mean_kernel<<<grid, 256, 0, stream>>>(total, cnt, sum, out_mean);
+    return cudaGetLastError();
+}
+
+// ---- FP32 instruction-rate probes (roofline denominator) ----
+constexpr int kProbeIters = 4096;
+constexpr int kProbeIlp = 16;
+
+template <int KIND>
+__global__ void __launch_bounds__(512, 1) probe_kernel(float* out, float a, float b) {
+    float v[kProbeIlp];
+#pragma unroll
+    for (int i = 0; i < kProbeIlp; ++i) v[i] = a * static_cast<float>(threadIdx.x + i);
+    int hits = 0;
+#pragma unroll 1
+    for (int it = 0; it < kProbeIters; ++it) {
+#pragma unroll
+        for (int i = 0; i < kProbeIlp; ++i) {
+            if (KIND == 0) {
+                v[i] = __fmaf_rn(v[i], a, b);
+            } else if (KIND == 1) {
+                v[i] = __fadd_rn(v[i], b);
+            } else {
+                v[i] = __fadd_rn(v[i], b);
+                // one compare per add, OR-chained into a predicate like the join's filter
+                hits |= (v[i] < a) ? 1 : 0;
+            }
+        }
+    }
+    float s = static_cast<float>(hits);
+#pragma unroll
+    for (int i = 0; i < kProbeIlp; ++i) s += v[i];
+    if (s == 123.456f) out[0] = s;
+}
+
+cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, cudaStream_t stream) {
+    float* d_out = nullptr;
+    cudaError_t e = cudaMalloc(&d_out, 64);
+    if (e != cudaSuccess) return e;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int grid = 148 * 4, block = 512;
+    for (int rep = 0; rep < 3; ++rep) {
+        if (rep == 2) cudaEventRecord(e0, stream);
+        if (kind == 0) probe_kernel<0><<<grid, block, 0, stream>>>(d_out, 1.0000001f, 1e-7f);
+        else if (kind == 1) probe_kernel<1><<<grid, block, 0, stream>>>(d_out, 1.0000001f, 1e-7f);
+        else probe_kernel<2><<<grid, block, 0, stream>>>(d_out, -1.0f, 1e-7f);
+    }
+    cudaEventRecord(e1, stream);
+    e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaEventElapsedTime(ms, e0, e1);
+    const double per_thread = static_cast<double>(kProbeIters) * kProbeIlp * (kind == 2 ? 2.0 : 1.0);
+    *lane_ops = per_thread * grid * block;
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d_out);
+    return e;
+}
+
+}  // namespace snaps

@@ -1,0 +1,28 @@
+// range_lattice.cuh -- launch interface of the sub-lattice eps range self-join kernel.
+#pragma once
+#include "snaps_device.cuh"
+
+namespace snaps {
+
+constexpr int kRangeMaxThreads = 512;
+
+struct RangeParams {
+    const float* Xp;
+    int N;
+    int n_tiles;
+    const BatchDesc* batches;   // thr[] = nextafter(eps^2) per slot, -1 for unused slots
+    int n_batches;
+    int batches_per_item;
+    int n_bchunks;
+    int n_qblocks;
+    int warps;
+    int* work_counter;
+    uint32_t* out_count;
+    float* out_sum;
+    float* out_mean;
+};
+
+size_t range_lattice_smem_bytes(int warps, bool with_sum);
+cudaError_t range_lattice_launch(const RangeParams& p, int grid, cudaStream_t stream);
+
+}  // namespace snaps
