@@ -26,12 +26,14 @@ constexpr unsigned kFull = 0xffffffffu;
 // set H of features 6..14 (all feature subsets are wanted, so
 // complete sub-lattices are the common case).  slot[T] is the index of mask
 // H|T in the caller's list, or -1 if that mask was not asked for.
-struct BatchDesc {
+struct alignas(16) BatchDesc {
+    float thr[kLat];           // range join: nextafter(eps^2) per slot (unused for kNN); read as float4
+    int32_t slot[kLat];
     uint32_t hmask;            // bits 6..14
     int32_t n_valid;
-    int32_t slot[kLat];
-    float thr[kLat];           // range join: nextafter(eps^2) per slot (unused for kNN)
+    int32_t pad_[2];
 };
+static_assert(sizeof(BatchDesc) % 16 == 0, "BatchDesc rows are read with 128-bit loads");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));

@@ -130,7 +130,9 @@ def test_range_join(snaps, oracle_mod, n, nf, seed, sums):
     masks = rng.choice(allm, min(len(allm), 48), replace=False)
     kq = min(10, n - 1)
     _, od = oracle_mod.knn_selfjoin(X, masks, kq)
-    eps = np.array([max(np.median(od[m, :, -1]), 1e-3) for m in range(len(masks))], dtype=np.float32)
+    # 1.003x: keep eps off the realised pair distance the median sits on (tiny n would put that
+    # pair inside the 1e-6 band of reading A2)
+    eps = np.array([max(1.003 * np.median(od[m, :, -1]), 1e-3) for m in range(len(masks))], dtype=np.float32)
     out = snaps.range_selfjoin(_dev(X), masks, eps, sums=sums)
     torch.cuda.synchronize()
     cnt = out["count"].cpu().numpy()
