@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- all-subspace kNN self-join (BASELINE.json configs[1]) on N GPUs of one node.
+
+A step = one pass of the whole hot path over one synthetic
+SNAPShot1-shaped table: stage the N x 15 fp32 table, plan the 32,752 subspace masks into
+sub-lattice batches, per-pair squared differences, add-only subset sums, per-(query, subspace)
+top-k selection, and the fused per-object outlier scores (k-th distance, mean kNN distance,
+kNN-graph in-degree).  `value` is timed with inputs resident in HBM; `e2e` goes through the
+public host-buffer call with the H2D of the table and the D2H of the scores inside the timed
+region.  Multi-GPU: every rank joins its own catalogue (seed 1 + rank) -- the path has no
+exchange step, so scaling is "weak" and there is no collective on the data path.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config NAME]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads  # noqa: E402
+
+METRIC = "subspaces/sec and pair-distance evals/sec (kNNSJ N=31,693,k=10); % FP32 peak"
+UNIT = "subspaces/s"
+
+# Roofline denominator: the path is bound by plain FP32/ALU issue, so the
+# peak is derived from unit counts and clocks: 148 SMs x 128 FP32 lanes x 1.965 GHz lane-ops/s
+# (one FADD, FMUL, FSUB, FFMA or FP32 compare = one lane-op; an FMA-counts-2 "FP32 peak" is twice
+# this number in FLOP/s, which an add-and-compare workload cannot reach by construction).
+N_SM, LANES_PER_SM = 148, 128
+
+
+def peaks():
+    sm_max_mhz = 1965.0
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            sm_max_mhz = float(json.load(f).get("sm_max_mhz", sm_max_mhz))
+    except OSError:
+        pass
+    return N_SM * LANES_PER_SM * sm_max_mhz * 1e6, sm_max_mhz
+
+
+def stratified_masks(masks, per_dim, seed):
+    pc = workloads.popcount(masks)
+    rng = np.random.default_rng(seed)
+    sel = [rng.choice(np.flatnonzero(pc == d), min(per_dim, int((pc == d).sum())), replace=False)
+           for d in np.unique(pc)]
+    return masks[np.sort(np.concatenate(sel))]
+
+
+def oracle_sample(cfg, X, masks, n_queries, seed=0):
+    """The T1 oracle on a bounded sample: ~2 masks per dimension x n_queries sampled queries,
+    each against all N candidates.  -> (seconds, evals, cores, description)."""
+    import oracle
+    oracle.build()
+    sm = stratified_masks(masks, 2, seed)
+    rng = np.random.default_rng(seed + 1)
+    q = np.sort(rng.choice(len(X), min(n_queries, len(X)), replace=False))
+    t0 = time.perf_counter()
+    oracle.knn_selfjoin(X, sm, cfg.k, queries=q)
+    dt = time.perf_counter() - t0
+    evals = float(len(sm)) * len(q) * len(X)
+    what = (f"{len(sm)} subspaces (2 per dimension d=2..15) x {len(q)} sampled queries x all "
+            f"{len(X)} candidates, k={cfg.k}, fp64 brute force; subspaces/s = evals/s / N^2")
+    return dt, evals, oracle.num_threads(), what
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle as it stands on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    cfg = workloads.get_config(args.config)
+    X, masks = cfg.table(), cfg.masks()
+    n2 = float(len(X)) ** 2
+    for _ in range(args.warmup):
+        oracle_sample(cfg, X, masks, 64)
+    tot_t, tot_e, cores, what = 0.0, 0.0, 0, ""
+    for s in range(args.steps):
+        dt, ev, cores, what = oracle_sample(cfg, X, masks, args.ref_queries, seed=s)
+        tot_t += dt
+        tot_e += ev
+    evals_per_s = tot_e / tot_t
+    value = evals_per_s / n2
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "evals_per_s": evals_per_s,
+        "config": {"workload": workload_name(cfg, len(masks)), "sampled": True},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": "each step: " + what},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg, n_masks):
+    return (f"{cfg.name}: kNNSJ k={cfg.k} over N={cfg.n} x {cfg.n_feat} fp32 (SNAPShot1-shaped, "
+            f"seed {cfg.seed}+rank), all {n_masks} subspaces of 2-15 features, scores kth/mean/indeg")
+
+
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
+                 "-lms", "200", "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.p.terminate()
+        self.p.wait()
+        self.f.flush()
+        self.f.seek(0)
+        rows = [[c.strip() for c in ln.split(",")] for ln in self.f if ln.strip()]
+        self.f.close()
+        os.unlink(self.f.name)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        sm, reasons, smax, pw = [], set(), None, []
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                smax = float(r[1])
+                pw.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="snaps", choices=["snaps", "reference"])
+    ap.add_argument("--config", default="c2_snapshot1_knn")
+    ap.add_argument("--ref-queries", type=int, default=1024,
+                    help="sampled queries per step of --impl reference")
+    ap.add_argument("--cpu-queries", type=int, default=4096,
+                    help="sampled queries of the cpu_baseline leg (0 = skip)")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_2405_20176_b200 as snaps
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback exists)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    snaps.lib()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    cfg = workloads.get_config(args.config)
+    assert "knn" in cfg.join
+    X = workloads.make_table(cfg.n, cfg.seed + rank, cols=list(range(cfg.n_feat)),
+                             outlier_frac=0.01 if cfg.n < 100000 else 0.001)
+    masks = cfg.masks()
+    N, n_feat, k, n_masks = len(X), X.shape[1], cfg.k, len(masks)
+    evals = float(N) * N * n_masks                 # algorithmic (pair, subspace) evaluations
+    planned = float(snaps.planned_evals(N, n_feat, masks))
+
+    Xd = torch.from_numpy(X).to(dev)
+    ws = torch.empty(snaps.workspace_bytes(N, n_feat, n_masks, k), dtype=torch.uint8, device=dev)
+    out = {"kth": torch.empty((n_masks, N), dtype=torch.float32, device=dev),
+           "mean": torch.empty((n_masks, N), dtype=torch.float32, device=dev),
+           "indeg": torch.empty((n_masks, N), dtype=torch.int32, device=dev)}
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    snaps.profile_enable(True)
+
+    def step():
+        flush.zero_()
+        snaps.knn_selfjoin(Xd, masks, k, lists=False, out=out, workspace=ws)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    kernel_ms, launches = [], 0
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+        ms, n = snaps.profile_last_kernel_ms()     # waits for this step's join kernel
+        kernel_ms.append(ms)
+        launches += n + 2                          # + stage_table kernel + the L2 flush fill
+    ev1.record()
+    torch.cuda.synchronize()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    ms_per_step = max_over_ranks(ev0.elapsed_time(ev1) / args.steps)
+    value = world * n_masks / (ms_per_step * 1e-3)
+    evals_per_s = world * evals / (ms_per_step * 1e-3)
+
+    # sanity on the last step's result: every object has in-degree sum N*k
+    chk = int(out["indeg"][n_masks // 2].sum().item())
+    assert chk == N * k, f"in-degree sum {chk} != N*k = {N * k}"
+
+    # ---- roofline of the dominant kernel (knn_lattice_kernel): ALU/FP32-issue bound
+    peak_lane_ops, sm_max = peaks()
+    k_ms = float(np.mean(kernel_ms))
+    n_batches = planned / (64.0 * N * N)
+    lane_ops = 2.0 * evals + 30.0 * float(N) * N * n_batches   # per launch, algorithmic
+    achieved = lane_ops / (k_ms * 1e-3)
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get("knn_lattice_kernel_dram_bytes_per_launch")
+    except OSError:
+        pass
+    roofline = {
+        "bound": "alu", "kernel": "knn_lattice_kernel", "achieved": achieved / 1e12,
+        "peak": peak_lane_ops / 1e12, "unit": "TFLOP/s", "frac": achieved / peak_lane_ops,
+        "traffic": traffic, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
+        "peak_source": f"derived: {N_SM} SMs x {LANES_PER_SM} FP32 lanes x {sm_max:.0f} MHz "
+                       "(FADD/FMUL/compare = 1 flop, no FMA in the path; FMA-counts-2 peak is 2x)",
+        "frac_of_fma2_peak": achieved / (2 * peak_lane_ops),
+        "algorithmic_lane_ops_per_launch": lane_ops,
+        "evals_per_s_kernel": evals / (k_ms * 1e-3),
+        "evals_performed_over_algorithmic": planned / evals,
+    }
+    if rank == 0:
+        try:
+            roofline["probe_lane_ops_per_s"] = {
+                "ffma": snaps.probe_fp32_rate(0), "fadd": snaps.probe_fp32_rate(1),
+                "fadd+fsetp": snaps.probe_fp32_rate(2)}
+        except snaps.SnapsError as e:                      # pragma: no cover
+            roofline["probe_lane_ops_per_s"] = str(e)
+
+    # ---- end to end through the host-buffer API: pinned X -> device, join, scores -> pinned host
+    e2e = None
+    if not args.no_e2e:
+        import psutil
+        score_bytes = 3 * 4 * n_masks * N
+        if psutil.virtual_memory().available > 3 * score_bytes:
+            del out
+            torch.cuda.empty_cache()
+            Xh = torch.from_numpy(X).pin_memory()
+            mpb = 2048
+            hws = torch.empty(snaps.workspace_bytes(N, n_feat, n_masks, k) +
+                              snaps.stream_ring_bytes(N, k, mpb), dtype=torch.uint8, device=dev)
+            hout = {"kth": torch.empty((n_masks, N), dtype=torch.float32, pin_memory=True),
+                    "mean": torch.empty((n_masks, N), dtype=torch.float32, pin_memory=True),
+                    "indeg": torch.empty((n_masks, N), dtype=torch.int32, pin_memory=True)}
+            xdev = torch.empty_like(Xd)
+
+            def host_step():
+                snaps.knn_selfjoin_host(Xh, masks, k, mpb, lists=False, out=hout, workspace=hws,
+                                        x_device=xdev)
+                torch.cuda.current_stream().synchronize()
+                return float(hout["kth"][-1, -1])          # the host reads the result
+
+            host_step()
+            barrier()
+            t0 = time.perf_counter()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record()
+            n_e2e = max(1, min(args.steps, 2))
+            for _ in range(n_e2e):
+                host_step()
+            g1.record()
+            torch.cuda.synchronize()
+            wall = (time.perf_counter() - t0) / n_e2e
+            e_ms = max_over_ranks(max(g0.elapsed_time(g1) / n_e2e, wall * 1e3))
+            assert int(hout["indeg"][n_masks // 2].sum().item()) == N * k
+            e2e = {"value": world * n_masks / (e_ms * 1e-3), "unit": UNIT,
+                   "h2d_bytes_per_step": int(X.nbytes + masks.nbytes),
+                   "d2h_bytes_per_step": int(score_bytes), "ms_per_step": e_ms, "steps": n_e2e,
+                   "api": "knn_selfjoin_host -> snaps_knn_selfjoin_streamed (pinned host in/out)"}
+        else:
+            e2e = {"value": None, "unit": UNIT, "skipped": "host RAM too small for pinned scores"}
+
+    cpu = None
+    if rank == 0 and world == 1 and args.cpu_queries > 0:
+        dt, ev, cores, what = oracle_sample(cfg, X, masks, args.cpu_queries)
+        cpu = {"value": ev / dt / (float(N) * N), "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": what, "evals_per_s": ev / dt, "seconds": dt}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, n_masks),
+                       "l2": "256 MB flush fill before every step; each step also writes 12.5 GB of scores",
+                       "outputs": "scores only (lists of this config are 83 GB)"},
+            "evals_per_s": evals_per_s, "fp32_peak_frac": roofline["frac"],
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
+            "clocks": clocks,
+            "paper_context": "paper: DSSJ all 32,752 spaces 2.64 h on 1xA100 (o=8) incl. CPU "
+                             "post-processing; LSST5M kNNSJ ~100 s/feature space (PAPER.md:394, Table 4)",
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -172,6 +172,17 @@ snaps_status snaps_knn_selfjoin_streamed(const float *d_X, int64_t N, int n_feat
  */
 snaps_status snaps_probe_fp32_rate(int kind, double *h_lane_ops_per_s, void *stream);
 
+/*
+ * Kernel timing for roofline reports.  While enabled,
+ * every join call records a CUDA event pair on `stream` around each launch of
+ * its dominant (join) kernel; the pairs of the most recent call are kept.
+ * snaps_profile_last_kernel_ms synchronises on them and returns the summed
+ * device time in milliseconds and the number of launches (either pointer may
+ * be NULL).  Disabled by default; enabling costs two event records per launch.
+ */
+snaps_status snaps_profile_enable(int on);
+snaps_status snaps_profile_last_kernel_ms(float *h_ms, int *h_launches);
+
 #ifdef __cplusplus
 }
 #endif

@@ -12,6 +12,7 @@ EXPORTED_SYMBOLS = [
     "snaps_last_error", "snaps_version", "snaps_workspace_bytes", "snaps_planned_evals",
     "snaps_knn_selfjoin", "snaps_range_selfjoin", "snaps_outlier_scores",
     "snaps_stream_ring_bytes", "snaps_knn_selfjoin_streamed", "snaps_probe_fp32_rate",
+    "snaps_profile_enable", "snaps_profile_last_kernel_ms",
 ]
 
 _lib = None
@@ -53,6 +54,11 @@ def lib():
                                                   vp, vp, vp, vp, vp, vp, sz, vp]
         L.snaps_probe_fp32_rate.restype = i32
         L.snaps_probe_fp32_rate.argtypes = [i32, ctypes.POINTER(ctypes.c_double), vp]
+        L.snaps_profile_enable.restype = i32
+        L.snaps_profile_enable.argtypes = [i32]
+        L.snaps_profile_last_kernel_ms.restype = i32
+        L.snaps_profile_last_kernel_ms.argtypes = [ctypes.POINTER(ctypes.c_float),
+                                                   ctypes.POINTER(ctypes.c_int)]
         _lib = L
     return _lib
 
@@ -192,8 +198,8 @@ def knn_selfjoin_streamed(X, masks, k, masks_per_batch, *, lists=True, scores=Tr
         out.setdefault("kth", pinned((len(m), N), torch.float32))
         out.setdefault("mean", pinned((len(m), N), torch.float32))
         out.setdefault("indeg", pinned((len(m), N), torch.int32))
-    for t in out.values():
-        assert t.is_pinned()
+    for n, t in out.items():
+        assert n.startswith("_") or t.is_pinned(), n
     ws = workspace if workspace is not None else _workspace(
         X, len(m), k, extra=stream_ring_bytes(N, k, masks_per_batch))
     _check(lib().snaps_knn_selfjoin_streamed(
@@ -204,17 +210,26 @@ def knn_selfjoin_streamed(X, masks, k, masks_per_batch, *, lists=True, scores=Tr
     return out
 
 
-def knn_selfjoin_host(X_host, masks, k, masks_per_batch=None, *, lists=False, scores=True, stream=None):
+def knn_selfjoin_host(X_host, masks, k, masks_per_batch=None, *, lists=False, scores=True, out=None,
+                      workspace=None, x_device=None, stream=None):
     """End-to-end call with HOST buffers: pinned X -> device, join, pinned host outputs.
-    Returns the dict of pinned host tensors after the stream is enqueued (caller synchronises)."""
+    Returns the dict of pinned host tensors after the work is enqueued (caller synchronises).
+    `out`, `workspace` and `x_device` may supply preallocated buffers for repeated calls."""
     import torch
     Xh = torch.as_tensor(X_host)
     if not Xh.is_pinned():
         Xh = Xh.pin_memory()
-    Xd = Xh.to("cuda", non_blocking=True)
+    s = torch.cuda.current_stream() if stream is None else stream
+    with torch.cuda.stream(s):
+        if x_device is None:
+            Xd = Xh.to("cuda", non_blocking=True)
+        else:
+            Xd = x_device
+            Xd.copy_(Xh, non_blocking=True)
     n_masks = len(_masks(masks))
     mpb = masks_per_batch or max(1, min(n_masks, 2048))
-    out = knn_selfjoin_streamed(Xd, masks, k, mpb, lists=lists, scores=scores, stream=stream)
+    out = knn_selfjoin_streamed(Xd, masks, k, mpb, lists=lists, scores=scores, out=out,
+                                workspace=workspace, stream=s)
     out["_X"] = Xd
     return out
 
@@ -223,3 +238,14 @@ def probe_fp32_rate(kind: int, stream=None) -> float:
     v = ctypes.c_double(0.0)
     _check(lib().snaps_probe_fp32_rate(kind, ctypes.byref(v), _stream(stream)))
     return float(v.value)
+
+
+def profile_enable(on: bool = True) -> None:
+    _check(lib().snaps_profile_enable(1 if on else 0))
+
+
+def profile_last_kernel_ms():
+    """-> (summed device ms of the last call's join-kernel launches, number of launches)."""
+    ms, n = ctypes.c_float(0.0), ctypes.c_int(0)
+    _check(lib().snaps_profile_last_kernel_ms(ctypes.byref(ms), ctypes.byref(n)))
+    return float(ms.value), int(n.value)

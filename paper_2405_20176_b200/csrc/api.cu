@@ -8,6 +8,7 @@
 
 #include <algorithm>
 #include <map>
+#include <utility>
 #include <vector>
 
 #include "../../include/snaps.h"
@@ -36,6 +37,30 @@ snaps_status fail(snaps_status code, const char* fmt, ...) {
     } while (0)
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- optional event pairs around the join kernels (snaps_profile_*) ----
+bool g_prof_on = false;
+std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_prof_pool;  // created once, reused
+size_t g_prof_used = 0;
+
+void prof_reset() { g_prof_used = 0; }
+
+bool prof_begin(cudaStream_t st) {
+    if (!g_prof_on) return false;
+    if (g_prof_used == g_prof_pool.size()) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return false;
+        g_prof_pool.emplace_back(a, b);
+    }
+    cudaEventRecord(g_prof_pool[g_prof_used].first, st);
+    return true;
+}
+
+void prof_end(bool began, cudaStream_t st) {
+    if (!began) return;
+    cudaEventRecord(g_prof_pool[g_prof_used].second, st);
+    ++g_prof_used;
+}
 
 int n_tiles_for(int64_t N) { return static_cast<int>((N + snaps::kTileRows - 1) / snaps::kTileRows); }
 
@@ -192,7 +217,9 @@ snaps_status knn_enqueue(const Workspace& w, const snaps::BatchDesc* d_batches, 
     p.out_indeg = out_indeg;
     const int64_t items = static_cast<int64_t>(p.n_qblocks) * p.n_bchunks;
     const int grid = static_cast<int>(std::min<int64_t>(items, grid_max));
+    const bool prof = prof_begin(st);
     CUDA_TRY(snaps::knn_lattice_launch(p, grid, st));
+    prof_end(prof, st);
     return SNAPS_OK;
 }
 
@@ -222,6 +249,7 @@ snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t
                                 float* out_dist, float* out_kth, float* out_mean,
                                 int32_t* out_indeg, void* d_workspace, size_t workspace_bytes,
                                 void* stream) {
+    prof_reset();
     snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
     if (rc) return rc;
     if (k < 1 || k > SNAPS_MAX_K || k > N - 1)
@@ -249,6 +277,7 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
                                   const uint16_t* h_masks, int n_masks, const float* h_eps,
                                   uint32_t* out_count, float* out_sumdist, float* out_mean,
                                   void* d_workspace, size_t workspace_bytes, void* stream) {
+    prof_reset();
     snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
     if (rc) return rc;
     if (!h_eps) return fail(SNAPS_INVALID_ARG, "h_eps is NULL");
@@ -289,7 +318,9 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
     p.out_mean = out_mean;
     const int64_t items = static_cast<int64_t>(p.n_qblocks) * p.n_bchunks;
     const int grid = static_cast<int>(std::min<int64_t>(items, grid_max));
+    const bool prof = prof_begin(st);
     CUDA_TRY(snaps::range_lattice_launch(p, grid, st));
+    prof_end(prof, st);
     return SNAPS_OK;
 }
 
@@ -329,6 +360,7 @@ snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat
                                          int masks_per_batch, int32_t* h_out_idx, float* h_out_dist,
                                          float* h_out_kth, float* h_out_mean, int32_t* h_out_indeg,
                                          void* d_workspace, size_t workspace_bytes, void* stream) {
+    prof_reset();
     snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
     if (rc) return rc;
     if (k < 1 || k > SNAPS_MAX_K || k > N - 1)
@@ -426,6 +458,25 @@ snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat
     }
     cudaStreamDestroy(side);
     return result;
+}
+
+snaps_status snaps_profile_enable(int on) {
+    g_prof_on = on != 0;
+    prof_reset();
+    return SNAPS_OK;
+}
+
+snaps_status snaps_profile_last_kernel_ms(float* h_ms, int* h_launches) {
+    float total = 0.f;
+    for (size_t i = 0; i < g_prof_used; ++i) {
+        CUDA_TRY(cudaEventSynchronize(g_prof_pool[i].second));
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, g_prof_pool[i].first, g_prof_pool[i].second));
+        total += ms;
+    }
+    if (h_ms) *h_ms = total;
+    if (h_launches) *h_launches = static_cast<int>(g_prof_used);
+    return SNAPS_OK;
 }
 
 snaps_status snaps_probe_fp32_rate(int kind, double* h_lane_ops_per_s, void* stream) {
