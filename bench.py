@@ -165,6 +165,9 @@ def main():
     ap.add_argument("--cpu-queries", type=int, default=4096,
                     help="sampled queries of the cpu_baseline leg (0 = skip)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--profile-masks", type=int, default=0,
+                    help="profiling aid (ncu --set full replays every launch ~40x): keep only the "
+                         "first M masks; the JSON line is then marked profile_only and is NOT a bench value")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -202,6 +205,8 @@ def main():
     X = workloads.make_table(cfg.n, cfg.seed + rank, cols=list(range(cfg.n_feat)),
                              outlier_frac=0.01 if cfg.n < 100000 else 0.001)
     masks = cfg.masks()
+    if args.profile_masks > 0:
+        masks = masks[:args.profile_masks]
     N, n_feat, k, n_masks = len(X), X.shape[1], cfg.k, len(masks)
     evals = float(N) * N * n_masks                 # algorithmic (pair, subspace) evaluations
     planned = float(snaps.planned_evals(N, n_feat, masks))
@@ -326,6 +331,7 @@ def main():
 
     if rank == 0:
         line = {
+            **({"profile_only": f"first {n_masks} masks"} if args.profile_masks > 0 else {}),
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
