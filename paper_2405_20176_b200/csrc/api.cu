@@ -132,16 +132,20 @@ snaps_status check_common(const float* d_X, int64_t N, int n_feat, int64_t ld,
 
 struct Workspace {
     float* Xp;
+    float4* Xb;
     int* counter;
     snaps::BatchDesc* batches;
     unsigned char* ring;   // rest
     size_t ring_bytes;
 };
 
+int n_blocks_for(int64_t N) { return static_cast<int>((N + 31) / 32); }
+
 size_t base_workspace_bytes(int64_t N, int n_masks) {
     const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
+    const size_t blocked = align_up(static_cast<size_t>(n_blocks_for(N)) * 2048, 256);
     const size_t batches = align_up(static_cast<size_t>(n_masks) * sizeof(snaps::BatchDesc), 256);
-    return table + 256 + batches;
+    return table + blocked + 256 + batches;
 }
 
 snaps_status carve(void* d_ws, size_t bytes, int64_t N, int n_masks, Workspace* w) {
@@ -153,9 +157,11 @@ snaps_status carve(void* d_ws, size_t bytes, int64_t N, int n_masks, Workspace* 
         return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", bytes, need);
     unsigned char* p = static_cast<unsigned char*>(d_ws);
     const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
+    const size_t blocked = align_up(static_cast<size_t>(n_blocks_for(N)) * 2048, 256);
     w->Xp = reinterpret_cast<float*>(p);
-    w->counter = reinterpret_cast<int*>(p + table);
-    w->batches = reinterpret_cast<snaps::BatchDesc*>(p + table + 256);
+    w->Xb = reinterpret_cast<float4*>(p + table);
+    w->counter = reinterpret_cast<int*>(p + table + blocked);
+    w->batches = reinterpret_cast<snaps::BatchDesc*>(p + table + blocked + 256);
     w->ring = p + need;
     w->ring_bytes = bytes - need;
     return SNAPS_OK;
@@ -187,9 +193,10 @@ void decompose(int64_t N, int n_batches, int warps, int grid, int* n_qblocks, in
 }
 
 int knn_warps_for(int k) {
-    // 227 KB of shared memory: tile ring + per-warp list state
-    const size_t budget = 227 * 1024;
-    int w = 15;
+    // per-warp list state in shared memory; what is left of the 256 KB array stays L1 for the
+    // table stream
+    const size_t budget = 164 * 1024;
+    int w = 16;
     while (w > 1 && snaps::knn_lattice_smem_bytes(k, w) > budget) --w;
     return w;
 }
@@ -201,6 +208,8 @@ snaps_status knn_enqueue(const Workspace& w, const snaps::BatchDesc* d_batches, 
     CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
     snaps::KnnParams p;
     p.Xp = w.Xp;
+    p.Xb = w.Xb;
+    p.n_blocks = n_blocks_for(N);
     p.N = static_cast<int>(N);
     p.n_tiles = n_tiles_for(N);
     p.k = k;
@@ -265,6 +274,7 @@ snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t
     const int n_tiles = n_tiles_for(N);
     CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
                                        n_tiles * snaps::kTileRows, st));
+    CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
     if (out_indeg)
         CUDA_TRY(cudaMemsetAsync(out_indeg, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, st));
     CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
@@ -378,6 +388,7 @@ snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat
     const int n_tiles = n_tiles_for(N);
     CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
                                        n_tiles * snaps::kTileRows, st));
+    CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
 
     const size_t mpb = static_cast<size_t>(masks_per_batch);
     const size_t n_list = align_up(mpb * N * k * 4, 256);

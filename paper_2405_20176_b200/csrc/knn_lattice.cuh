@@ -4,10 +4,12 @@
 
 namespace snaps {
 
-constexpr int kKnnMaxThreads = 512;  // (consumer warps + 1 producer warp) * 32
+constexpr int kKnnMaxThreads = 512;  // warps * 32
 
 struct KnnParams {
-    const float* Xp;            // staged table, n_tiles*128 rows of 20 floats
+    const float* Xp;            // staged table, row-major, n_tiles*128 rows of 20 floats (seeds, query rows)
+    const float4* Xb;           // staged table, blocked: [n_blocks][4 feature groups][32 rows] float4
+    int n_blocks;               // ceil(N / 32)
     int N;
     int n_tiles;
     int k;

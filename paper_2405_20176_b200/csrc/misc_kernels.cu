@@ -13,7 +13,9 @@ __global__ void stage_table_kernel(const float* __restrict__ X, int64_t ld, int 
          i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
         const int64_t r = i / kRowFloats;
         const int j = static_cast<int>(i - r * kRowFloats);
-        Xp[i] = (r < N && j < n_feat) ? X[r * ld + j] : 0.f;
+        // padding rows sit far away in every feature, so that no sum that includes one of their
+        // features can pass a threshold (ids are still checked where entries are merged, A19)
+        Xp[i] = (j < n_feat) ? (r < N ? X[r * ld + j] : kPadCoord) : 0.f;
     }
 }
 
@@ -22,6 +24,34 @@ cudaError_t stage_table_launch(const float* X, int64_t ld, int N, int n_feat, fl
     const int64_t total = static_cast<int64_t>(n_rows_padded) * kRowFloats;
     const int grid = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 16));
     stage_table_kernel<<<grid, 256, 0, stream>>>(X, ld, N, n_feat, Xp, n_rows_padded);
+    return cudaGetLastError();
+}
+
+// a1, second layout for the kNN kernel: blocks of 32 rows, within a block four feature groups of
+// 32 float4 (lane-major), so that a warp reads a block with four fully coalesced 128-bit loads.
+__global__ void stage_blocked_kernel(const float* __restrict__ X, int64_t ld, int N, int n_feat,
+                                     float4* __restrict__ Xb, int n_blocks) {
+    const int64_t total = static_cast<int64_t>(n_blocks) * 128;
+    for (int64_t i = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; i < total;
+         i += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+        const int64_t blk = i >> 7;
+        const int g = static_cast<int>((i >> 5) & 3), ln = static_cast<int>(i & 31);
+        const int64_t r = blk * 32 + ln;
+        float v[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = 4 * g + u;
+            v[u] = (j < n_feat) ? (r < N ? X[r * ld + j] : kPadCoord) : 0.f;
+        }
+        Xb[i] = make_float4(v[0], v[1], v[2], v[3]);
+    }
+}
+
+cudaError_t stage_blocked_launch(const float* X, int64_t ld, int N, int n_feat, float4* Xb,
+                                 int n_blocks, cudaStream_t stream) {
+    const int64_t total = static_cast<int64_t>(n_blocks) * 128;
+    const int grid = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 16));
+    stage_blocked_kernel<<<grid, 256, 0, stream>>>(X, ld, N, n_feat, Xb, n_blocks);
     return cudaGetLastError();
 }
 

@@ -8,6 +8,9 @@ namespace snaps {
 cudaError_t stage_table_launch(const float* X, int64_t ld, int N, int n_feat, float* Xp,
                                int n_rows_padded, cudaStream_t stream);
 
+cudaError_t stage_blocked_launch(const float* X, int64_t ld, int N, int n_feat, float4* Xb,
+                                 int n_blocks, cudaStream_t stream);
+
 cudaError_t knn_scores_launch(int64_t N, int n_masks, int k, const int32_t* idx, const float* dist,
                               float* out_kth, float* out_mean, int32_t* out_indeg,
                               cudaStream_t stream);

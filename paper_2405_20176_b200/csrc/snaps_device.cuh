@@ -19,8 +19,9 @@ constexpr int kTileBytes = kTileRows * kRowBytes;  // 10240
 constexpr int kStages = 3;                     // tile ring depth
 constexpr int kLow = 6;                        // lattice features per batch
 constexpr int kLat = 1 << kLow;                // 64 subset sums per (pair, batch)
-constexpr int kPend = 8;                       // pending-append slots per list
+constexpr int kRing = 128;                     // kNN: per-warp ring of (list, id, d^2) triples awaiting merge
 constexpr unsigned kFull = 0xffffffffu;
+constexpr float kPadCoord = 1e18f;             // coordinate of padding rows (squares stay finite: 15e36)
 
 // One batch = the sub-lattice { H u T : T subset of features 0..5 } for a fixed
 // set H of features 6..14 (all feature subsets are wanted, so
