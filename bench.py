@@ -168,6 +168,8 @@ def main():
     ap.add_argument("--profile-masks", type=int, default=0,
                     help="profiling aid (ncu --set full replays every launch ~40x): keep only the "
                          "first M masks; the JSON line is then marked profile_only and is NOT a bench value")
+    ap.add_argument("--profile-offset", type=int, default=0,
+                    help="with --profile-masks: index of the first mask kept")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -206,7 +208,7 @@ def main():
                              outlier_frac=0.01 if cfg.n < 100000 else 0.001)
     masks = cfg.masks()
     if args.profile_masks > 0:
-        masks = masks[:args.profile_masks]
+        masks = masks[args.profile_offset:args.profile_offset + args.profile_masks]
     N, n_feat, k, n_masks = len(X), X.shape[1], cfg.k, len(masks)
     evals = float(N) * N * n_masks                 # algorithmic (pair, subspace) evaluations
     planned = float(snaps.planned_evals(N, n_feat, masks))
@@ -331,7 +333,7 @@ def main():
 
     if rank == 0:
         line = {
-            **({"profile_only": f"first {n_masks} masks"} if args.profile_masks > 0 else {}),
+            **({"profile_only": f"{n_masks} masks from index {args.profile_offset}"} if args.profile_masks > 0 else {}),
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",

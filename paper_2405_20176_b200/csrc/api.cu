@@ -4,6 +4,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -195,8 +196,12 @@ void decompose(int64_t N, int n_batches, int warps, int grid, int* n_qblocks, in
 int knn_warps_for(int k) {
     // per-warp list state in shared memory; what is left of the 256 KB array stays L1 for the
     // table stream
-    const size_t budget = 164 * 1024;
-    int w = 16;
+    const size_t budget = 200 * 1024;
+    int w = snaps::kKnnMaxThreads / 32;
+    if (const char* e = getenv("SNAPS_KNN_WARPS")) {   // tuning knob: warps (queries) per CTA
+        const int v = atoi(e);
+        if (v >= 1 && v <= snaps::kKnnMaxThreads / 32 && snaps::knn_lattice_smem_bytes(k, v) <= 227 * 1024) return v;
+    }
     while (w > 1 && snaps::knn_lattice_smem_bytes(k, w) > budget) --w;
     return w;
 }
@@ -216,16 +221,18 @@ snaps_status knn_enqueue(const Workspace& w, const snaps::BatchDesc* d_batches, 
     p.batches = d_batches;
     p.n_batches = nb;
     p.warps = knn_warps_for(k);
-    const int grid_max = sm_count();
-    decompose(N, nb, p.warps, grid_max, &p.n_qblocks, &p.batches_per_item, &p.n_bchunks);
-    p.work_counter = w.counter;
+    // runs of up to 32 consecutive batches keep a query's lists warm for seeding; items are
+    // plentiful (N per run), so the dynamic per-warp scheduler balances the tail
+    p.batches_per_item = std::min(nb, 32);
+    p.n_bchunks = (nb + p.batches_per_item - 1) / p.batches_per_item;
+    p.work_counter = reinterpret_cast<unsigned long long*>(w.counter);
     p.out_idx = out_idx;
     p.out_dist = out_dist;
     p.out_kth = out_kth;
     p.out_mean = out_mean;
     p.out_indeg = out_indeg;
-    const int64_t items = static_cast<int64_t>(p.n_qblocks) * p.n_bchunks;
-    const int grid = static_cast<int>(std::min<int64_t>(items, grid_max));
+    const int64_t items = N * p.n_bchunks;
+    const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
     const bool prof = prof_begin(st);
     CUDA_TRY(snaps::knn_lattice_launch(p, grid, st));
     prof_end(prof, st);

@@ -2,24 +2,26 @@
 //
 // What it computes: PAPER.md:112, 122 (kNNSJ) for every mask of a sub-lattice batch;
 // scores of PAPER.md:251-252 fused into the tail.  How:
-//   * one consumer warp = one query object x the 64 masks {H u T : T subset of
-//     features 0..5}; the 32 lanes hold 32 different candidates per step;
-//   * candidate tiles (128 rows x 80 B) arrive in a 3-stage shared-memory ring via
-//     cp.async.bulk + mbarrier from a dedicated producer warp (no __syncthreads in
-//     the steady state);
+//   * one warp = one query object x the 64 masks {H u T : T subset of features 0..5};
+//     the 32 lanes hold 32 different candidates per step;
+//   * candidates stream from the blocked copy of the table (2.5 MB at N=31,693: L2 resident,
+//     four coalesced 128-bit loads per step, next block prefetched into registers); the warps
+//     of a CTA scan in a loose convoy and share the lines through L1 -- no barrier couples them;
 //   * FILTER (every candidate): 15 squared differences once, then the 16 partial sums
 //     X[u] over features 2..5 (add-only).  X[u] is a lower bound of the four sums
 //     X[u] (+sq0) (+sq1) of "group" u (adding non-negative terms never rounds below the
 //     addend), so a candidate can enter one of the group's lists only if X[u] < G[u],
 //     G[u] = max of the group's four current thresholds (register-held);
 //   * COMPACT: lanes that pass any group test push (id, base, sq0..5) into a per-warp
-//     shared-memory queue (ballot + popc); with running thresholds ~2-4% of candidates pass;
+//     shared-memory queue (ballot + popc); with running thresholds a few % of candidates pass;
 //   * REFINE (every 32 queued candidates, all lanes busy): the 64 subset sums by add-only
 //     enumeration in a fixed order, each compared with its list's current threshold
-//     (k-th squared distance so far); passing (list, id, d^2) triples go to a per-warp ring;
+//     (k-th squared distance so far), branch-free into a 64-bit pass mask per lane; passing
+//     (list, id, d^2) triples go to a per-warp ring at positions from a warp prefix sum;
 //   * DRAIN: ring entries are merged into the sorted lists entry-parallel (one lane per
-//     entry, lanes that target the same list take turns), thresholds and G
-//     are refreshed;
+//     entry, lanes that target the same list take turns); a list is 12/20/28/36 words apart
+//     from the next so that whole lists move with conflict-free 128-bit accesses and the
+//     insert is a rank computation in registers; thresholds and G are refreshed;
 //   * thresholds start from an upper bound seeded by evaluating k known objects
 //     (the first k ids and the previous batch's neighbours: consecutive batches
 //     differ in one feature), tightened by min over supersets (the k-th distance
@@ -38,111 +40,43 @@ __device__ unsigned long long g_stats[16];
 #define STAT_CLK() 0ll
 #endif
 
-// ---- per-warp shared-memory state (32-bit words) ----------------------------------
-// rows of 64 words (one word per list), element-major so that lane l touching
-// list l is conflict-free:
-//   rows [0,k)     list d^2 (ascending by (d^2,id))     rows [k,2k)   list ids
-//   row 2k   list count     row 2k+1  threshold     row 2k+2  seed bound     row 2k+3  output slot
-//   row 2k+4 words 0..15: G (group maxima), words 16..30: the query's 15 features
-//   then the ring (3 arrays of kRing words) and the queue (64 entries of 8 words)
-#define L_D2(e, L) ws[((e)) * 64 + (L)]
-#define L_ID(e, L) wsi[(k + (e)) * 64 + (L)]
-#define L_CNT(L) wsi[(2 * k) * 64 + (L)]
-#define THR(L) ws[(2 * k + 1) * 64 + (L)]
-#define SEED(L) ws[(2 * k + 2) * 64 + (L)]
-#define SLOT(L) wsi[(2 * k + 3) * 64 + (L)]
-#define GMAX(u) ws[(2 * k + 4) * 64 + (u)]
-#define QROW(j) ws[(2 * k + 4) * 64 + 16 + (j)]
-#define RG_T(i) wsi[(2 * k + 5) * 64 + (i)]
-#define RG_ID(i) wsi[(2 * k + 5) * 64 + kRing + (i)]
-#define RG_D2(i) ws[(2 * k + 5) * 64 + 2 * kRing + (i)]
-#define QUEUE4(e) (reinterpret_cast<float4*>(ws + (2 * k + 5) * 64 + 3 * kRing) + 2 * (e))
+// ---- per-warp shared-memory state (32-bit words); S = list stride (template parameter) ----
+//   [0, 64*S)        list d^2, list L at L*S, ascending by (d^2, id)
+//   [64*S, 128*S)    list ids
+//   then rows of 64 words: list count, threshold, seed bound, output slot,
+//   one row: words 0..15 G (group maxima), words 16..30 the query's 15 features
+//   then the ring (3 arrays of kRing words) and the queue (kQueue entries of 8 words)
+#define L_D2(e, L) ws[(L) * S + (e)]
+#define L_ID(e, L) wsi[64 * S + (L) * S + (e)]
+#define ROWS(r) (128 * S + (r) * 64)
+#define L_CNT(L) wsi[ROWS(0) + (L)]
+#define THR(L) ws[ROWS(1) + (L)]
+#define SEED(L) ws[ROWS(2) + (L)]
+#define SLOT(L) wsi[ROWS(3) + (L)]
+#define GMAX(u) ws[ROWS(4) + (u)]
+#define QROW(j) ws[ROWS(4) + 16 + (j)]
+#define MT(T, j) ws[ROWS(5) + (T) * 36 + (j)]
+#define CANDID(j) wsi[ROWS(5) + 32 * 36 + (j)]
+#define QUEUE4(e) (reinterpret_cast<float4*>(ws + ROWS(5) + 32 * 36 + 32) + 2 * (e))
 constexpr int kQueue = 64;   // queue entries (8 words each); refine as soon as 32 are waiting
 
-__host__ __device__ constexpr int knn_warp_words(int k) { return (2 * k + 5) * 64 + 3 * kRing + kQueue * 8; }
-
-// Merge ring entries [0, cnt) into the sorted lists.  One lane per entry; lanes whose
-// entries target the same list take turns; the (d^2, id) key decides, not arrival order.
-// The insert is rank based: all loads of a list are independent (no pointer-chasing shift loop).
-template <int KCAP>
-__device__ __noinline__ void knn_drain(float* ws, int k, int lane, int q, int N, int cnt) {
-    int* wsi = reinterpret_cast<int*>(ws);
-    __syncwarp();
-    const long long t0_ = STAT_CLK();
-    STAT_ADD(4, 1);
-    STAT_ADD(5, cnt);
-#pragma unroll 1
-    for (int e0 = 0; e0 < cnt; e0 += 32) {
-        const int i = e0 + lane;
-        bool valid = i < cnt;
-        int T = 0, id = 0;
-        float d = 0.f;
-        if (valid) {
-            T = RG_T(i);
-            id = RG_ID(i);
-            d = RG_D2(i);
-            // self by index (reading A4), padding rows (A19), and entries that a tighter
-            // threshold has overtaken since they were appended (ties are settled by the
-            // (d^2, id) key below: ring order is not id order)
-            if (id == q || id >= N || d > THR(T)) valid = false;
-        }
-        const unsigned peers = __match_any_sync(kFull, valid ? T : 64 + lane);
-        const int rank = __popc(peers & ((1u << lane) - 1u));
-        const int rounds = __reduce_max_sync(kFull, valid ? rank + 1 : 0);
-        STAT_ADD(6, rounds);
-#pragma unroll 1
-        for (int r = 0; r < rounds; ++r) {
-            if (valid && rank == r) {
-                const int c = L_CNT(T);
-                float v[KCAP];
-                int w[KCAP];
-#pragma unroll
-                for (int e = 0; e < KCAP; ++e) {
-                    v[e] = (e < c) ? L_D2(e, T) : __int_as_float(0x7f800000);
-                    w[e] = (e < c) ? L_ID(e, T) : 0x7fffffff;
-                }
-                int pos = 0;  // number of list entries whose key precedes (d, id)
-#pragma unroll
-                for (int e = 0; e < KCAP; ++e) pos += (v[e] < d || (v[e] == d && w[e] < id)) ? 1 : 0;
-                if (pos < k) {
-                    const int cn = c < k ? c + 1 : k;
-#pragma unroll
-                    for (int e = KCAP - 1; e >= 1; --e) {
-                        if (e > pos && e < cn) {
-                            L_D2(e, T) = v[e - 1];
-                            L_ID(e, T) = w[e - 1];
-                        }
-                    }
-#pragma unroll
-                    for (int e = 0; e < KCAP; ++e) {
-                        if (e == pos) {
-                            L_D2(e, T) = d;
-                            L_ID(e, T) = id;
-                        }
-                    }
-                    L_CNT(T) = cn;
-                    if (cn == k) THR(T) = L_D2(k - 1, T);
-                }
-            }
-            __syncwarp();
-        }
-    }
-    if (lane < 16) {
-        const float4 t = *reinterpret_cast<const float4*>(&THR(4 * lane));
-        GMAX(lane) = fmaxf(fmaxf(t.x, t.y), fmaxf(t.z, t.w));
-    }
-    __syncwarp();
-    STAT_ADD(1, STAT_CLK() - t0_);
+__host__ __device__ constexpr int knn_list_stride(int k) { return k <= 12 ? 12 : k <= 20 ? 20 : k <= 28 ? 28 : 36; }
+__host__ __device__ constexpr int knn_warp_words(int k) {
+    return 128 * knn_list_stride(k) + 5 * 64 + 32 * 36 + 32 + kQueue * 8;
 }
 
-// REFINE: lanes 0..n-1 take the n oldest queue entries; the 64 subset sums of each are
-// compared with their lists' thresholds (branch-free, a 64-bit pass mask per lane); passing
-// (list, id, d^2) triples are appended to the ring at positions from a warp prefix sum (at
-// most kRing/32 per lane and round, so the ring cannot overflow) and merged.
+// REFINE: lanes 0..n-1 take the n oldest queue entries and form their 64 subset sums
+// (lane = candidate); the sums cross to the list owners through a 32 x 32 shared-memory
+// transpose (row stride 36 words: conflict-free both ways), 32 lists at a time; then
+// lane = list: the owner compares its list's 32 new sums with its threshold and merges the
+// passing ones into the sorted list held in registers (rank computation, no shift loop).
+// Candidates come in increasing id order, so among equal d^2 the earlier one stays first:
+// ties are broken by the smaller id (reading A3).
 // The add order (high features by FMA in feature order -> features 2,3,4,5 -> 0 -> 1) is the
 // same wherever a squared distance is formed, so a value never depends on scheduling.
-template <int KCAP>
+template <int S>
 __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N, int head, int n) {
+    constexpr int NE = S > 32 ? 32 : S;   // list elements held (S = 36 carries 4 words of padding)
     int* wsi = reinterpret_cast<int*>(ws);
     __syncwarp();
     const long long t0_ = STAT_CLK();
@@ -157,73 +91,107 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N
         cand = __float_as_int(a.x);
         base = a.y; sq[0] = a.z; sq[1] = a.w;
         sq[2] = b.x; sq[3] = b.y; sq[4] = b.z; sq[5] = b.w;
+        // self by index (reading A4) and padding rows (A19) never reach a list
+        if (cand == q || cand >= N) base = __int_as_float(0x7f800000);
     }
-    unsigned mlo = 0u, mhi = 0u;
-    {
-        float X[16];
-        X[0] = base;
+    CANDID(lane) = cand;
+    float X8[8];   // partial sums over features 2,3,4; feature 5 is added per half (same order as X[16])
+    X8[0] = base;
 #pragma unroll
-        for (int u = 1; u < 16; ++u) {
-            const int hb = 31 - __clz(u);
-            X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);
-        }
+    for (int u = 1; u < 8; ++u) {
+        const int hb = 31 - __clz(u);
+        X8[u] = __fadd_rn(X8[u & ~(1 << hb)], sq[2 + hb]);
+    }
 #pragma unroll
-        for (int u = 0; u < 16; ++u) {
-            const float s0 = X[u];
+    for (int half = 0; half < 2; ++half) {
+#pragma unroll
+        for (int uu = 0; uu < 8; ++uu) {
+            const float s0 = half ? __fadd_rn(X8[uu], sq[5]) : X8[uu];
             const float s1 = __fadd_rn(s0, sq[0]);
             const float s2 = __fadd_rn(s0, sq[1]);
             const float s3 = __fadd_rn(s1, sq[1]);
-            const float4 th = *reinterpret_cast<const float4*>(&THR(4 * u));
-            const unsigned bits = (s0 < th.x ? 1u : 0u) | (s1 < th.y ? 2u : 0u) |
-                                  (s2 < th.z ? 4u : 0u) | (s3 < th.w ? 8u : 0u);
-            if (u < 8) mlo |= bits << (4 * u);
-            else mhi |= bits << (4 * (u - 8));
+            MT(4 * uu + 0, lane) = s0;
+            MT(4 * uu + 1, lane) = s1;
+            MT(4 * uu + 2, lane) = s2;
+            MT(4 * uu + 3, lane) = s3;
         }
-    }
-    constexpr int kPerLane = kRing / 32;
-#pragma unroll 1
-    while (__any_sync(kFull, (mlo | mhi) != 0u)) {
-        const int have = __popc(mlo) + __popc(mhi);
-        // everything at once if it fits the ring, else a bounded share per lane and round
-        const int mine = (__reduce_add_sync(kFull, have) <= kRing) ? have
-                                                                   : (have < kPerLane ? have : kPerLane);
-        int incl = mine;  // inclusive prefix sum over lanes
+        __syncwarp();
+        // ---- lane = list T.  The k entries are right aligned in the NE slots (ascending; unused
+        // bottom slots hold -inf, not yet filled top slots +inf), so the k-th is always slot NE-1.
+        const int T = 32 * half + lane;
+        const float seed = SEED(T);
+        float thr = THR(T);
+        bool changed = false;
+        float v[NE];
+        int w[NE];
+        {
+            const float4* pv = reinterpret_cast<const float4*>(&L_D2(0, T));
+            const int4* pw = reinterpret_cast<const int4*>(&L_ID(0, T));
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int v = __shfl_up_sync(kFull, incl, o);
-            if (lane >= o) incl += v;
-        }
-        const int total = __shfl_sync(kFull, incl, 31);
-        int pos = incl - mine;
-#pragma unroll 1
-        for (int j = 0; j < mine; ++j, ++pos) {
-            int T;
-            if (mlo) {
-                T = __ffs(mlo) - 1;
-                mlo &= mlo - 1u;
-            } else {
-                T = 32 + __ffs(mhi) - 1;
-                mhi &= mhi - 1u;
+            for (int e4 = 0; e4 < NE / 4; ++e4) {
+                const float4 a = pv[e4];
+                const int4 b = pw[e4];
+                v[4 * e4 + 0] = a.x; v[4 * e4 + 1] = a.y; v[4 * e4 + 2] = a.z; v[4 * e4 + 3] = a.w;
+                w[4 * e4 + 0] = b.x; w[4 * e4 + 1] = b.y; w[4 * e4 + 2] = b.z; w[4 * e4 + 3] = b.w;
             }
-            float x = base;
-            if (T & 4) x = __fadd_rn(x, sq[2]);
-            if (T & 8) x = __fadd_rn(x, sq[3]);
-            if (T & 16) x = __fadd_rn(x, sq[4]);
-            if (T & 32) x = __fadd_rn(x, sq[5]);
-            if (T & 1) x = __fadd_rn(x, sq[0]);
-            if (T & 2) x = __fadd_rn(x, sq[1]);
-            RG_T(pos) = T;
-            RG_ID(pos) = cand;
-            RG_D2(pos) = x;
         }
-        knn_drain<KCAP>(ws, k, lane, q, N, total);
+#pragma unroll 1
+        for (int j4 = 0; j4 < 8; ++j4) {
+            const float4 m = *reinterpret_cast<const float4*>(&MT(lane, 4 * j4));
+            if (fminf(fminf(m.x, m.y), fminf(m.z, m.w)) < thr) {
+                changed = true;
+                const int4 ids = *reinterpret_cast<const int4*>(&CANDID(4 * j4));
+#define MERGE_ONE(dval, idval)                                                        \
+                if ((dval) < thr) {                                                   \
+                    const float d = (dval);                                           \
+                    const int id = (idval);                                           \
+                    int pos = 0;                                                      \
+                    _Pragma("unroll") for (int e = 0; e < NE; ++e)                    \
+                        pos += static_cast<int>((v[e] < d) | ((v[e] == d) & (w[e] < id))); \
+                    _Pragma("unroll") for (int e = NE - 1; e >= 1; --e) {             \
+                        const bool up = e > pos;                                      \
+                        v[e] = up ? v[e - 1] : v[e];                                  \
+                        w[e] = up ? w[e - 1] : w[e];                                  \
+                    }                                                                 \
+                    _Pragma("unroll") for (int e = 0; e < NE; ++e) {                  \
+                        const bool here = e == pos;                                   \
+                        v[e] = here ? d : v[e];                                       \
+                        w[e] = here ? id : w[e];                                      \
+                    }                                                                 \
+                    thr = fminf(seed, v[NE - 1]);                                     \
+                }
+                MERGE_ONE(m.x, ids.x)
+                MERGE_ONE(m.y, ids.y)
+                MERGE_ONE(m.z, ids.z)
+                MERGE_ONE(m.w, ids.w)
+#undef MERGE_ONE
+            }
+        }
+        if (changed) {
+            float4* qv = reinterpret_cast<float4*>(&L_D2(0, T));
+            int4* qw = reinterpret_cast<int4*>(&L_ID(0, T));
+#pragma unroll
+            for (int e4 = 0; e4 < NE / 4; ++e4) {
+                qv[e4] = make_float4(v[4 * e4], v[4 * e4 + 1], v[4 * e4 + 2], v[4 * e4 + 3]);
+                qw[e4] = make_int4(w[4 * e4], w[4 * e4 + 1], w[4 * e4 + 2], w[4 * e4 + 3]);
+            }
+            THR(T) = thr;
+        }
+        __syncwarp();
     }
+    if (lane < 16) {
+        const float4 t = *reinterpret_cast<const float4*>(&THR(4 * lane));
+        GMAX(lane) = fmaxf(fmaxf(t.x, t.y), fmaxf(t.z, t.w));
+    }
+    __syncwarp();
     STAT_ADD(0, STAT_CLK() - t0_);
 }
 
 // Upper bounds on the final k-th squared distance of every list of the new batch.
+template <int S>
 __device__ __noinline__ void knn_seed(float* ws, const float* __restrict__ Xp, int q, int k,
                                       uint32_t H, bool has_prev, int lane) {
+    constexpr int NE = S > 32 ? 32 : S;
     int* wsi = reinterpret_cast<int*>(ws);
     __syncwarp();
     float qrow[15];
@@ -242,10 +210,10 @@ __device__ __noinline__ void knn_seed(float* ws, const float* __restrict__ Xp, i
                 b1 = fmaxf(b1, masked_d2(Xp + static_cast<size_t>(c) * kRowFloats, qrow, mask));
             }
             bound = b1;
-            if (has_prev && L_CNT(L) == k) {
+            if (has_prev && L_D2(NE - 1, L) < __int_as_float(0x7f800000)) {   // previous list is full
                 float b2 = 0.f;
 #pragma unroll 1
-                for (int e = 0; e < k; ++e) {
+                for (int e = NE - k; e < NE; ++e) {
                     const int c = L_ID(e, L);
                     b2 = fmaxf(b2, masked_d2(Xp + static_cast<size_t>(c) * kRowFloats, qrow, mask));
                 }
@@ -274,7 +242,9 @@ __device__ __noinline__ void knn_seed(float* ws, const float* __restrict__ Xp, i
 #pragma unroll 1
     for (int h = 0; h < 2; ++h) {
         const int L = lane + 32 * h;
-        L_CNT(L) = 0;
+        // empty list: k right-aligned slots at +inf above NE-k slots at -inf
+        for (int e = 0; e < NE; ++e)
+            L_D2(e, L) = __int_as_float(e < NE - k ? 0xff800000 : 0x7f800000);
         THR(L) = SEED(L);
     }
     __syncwarp();
@@ -286,7 +256,9 @@ __device__ __noinline__ void knn_seed(float* ws, const float* __restrict__ Xp, i
 }
 
 // Step a7: sqrt, scores, in-degree, lists.
+template <int S>
 __device__ __noinline__ void knn_emit(float* ws, const KnnParams& p, int q, int lane) {
+    constexpr int NE = S > 32 ? 32 : S;
     int* wsi = reinterpret_cast<int*>(ws);
     const int k = p.k;
     __syncwarp();
@@ -299,8 +271,8 @@ __device__ __noinline__ void knn_emit(float* ws, const KnnParams& p, int q, int 
         float sum = 0.f, dk = 0.f;
 #pragma unroll 1
         for (int e = 0; e < k; ++e) {
-            const float d = sqrtf(L_D2(e, L));
-            const int id = L_ID(e, L);
+            const float d = sqrtf(L_D2(NE - k + e, L));
+            const int id = L_ID(NE - k + e, L);
             sum += d;
             dk = d;
             if (p.out_idx) p.out_idx[o * k + e] = id;
@@ -326,31 +298,27 @@ __device__ __noinline__ void knn_emit(float* ws, const KnnParams& p, int q, int 
         }                                                                     \
     } while (0)
 
-template <int KCAP>
+template <int S>
 __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const KnnParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
-    int* s_item = reinterpret_cast<int*>(smem);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int W = p.warps;
     const int k = p.k;
     float* ws = reinterpret_cast<float*>(smem + 128) + static_cast<size_t>(warp) * knn_warp_words(k);
     int* wsi = reinterpret_cast<int*>(ws);
 
-    const int n_items = p.n_qblocks * p.n_bchunks;
+    // one item = one query x a run of consecutive batches, fetched per warp: no block-level
+    // synchronisation anywhere in the kernel (a warp never waits for a slower query)
+    const long long n_items = static_cast<long long>(p.N) * p.n_bchunks;
     const unsigned lt = (1u << lane) - 1u;
     for (;;) {
-        // one item = W queries x a run of consecutive batches; the warps of a CTA start an item
-        // together so that their scans of the table stay close and share L1 lines
-        if (threadIdx.x == 0) s_item[0] = atomicAdd(p.work_counter, 1);
-        __syncthreads();
-        const int item = s_item[0];
-        __syncthreads();
+        long long item = 0;
+        if (lane == 0) item = atomicAdd(p.work_counter, 1ull);
+        item = __shfl_sync(kFull, item, 0);
         if (item >= n_items) break;
-        const int qb = item % p.n_qblocks, bc = item / p.n_qblocks;
+        const int q = static_cast<int>(item % p.N);
+        const int bc = static_cast<int>(item / p.N);
         const int b0 = bc * p.batches_per_item;
         const int b1 = min(b0 + p.batches_per_item, p.n_batches);
-        const int q = qb * W + warp;
-        if (q >= p.N) continue;
 
         float qlo[kLow];
         float qhi[9];
@@ -370,7 +338,7 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             const long long tb_ = STAT_CLK();
             SLOT(lane) = bd->slot[lane];
             SLOT(lane + 32) = bd->slot[lane + 32];
-            knn_seed(ws, p.Xp, q, k, H, has_prev, lane);
+            knn_seed<S>(ws, p.Xp, q, k, H, has_prev, lane);
             STAT_ADD(9, STAT_CLK() - tb_);
             float G[16];
             RELOAD_G();
@@ -426,15 +394,15 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
                     }
                     qtail += __popc(bal);
                     if (qtail - qhead >= 32) {
-                        knn_refine<KCAP>(ws, k, lane, q, p.N, qhead, 32);
+                        knn_refine<S>(ws, k, lane, q, p.N, qhead, 32);
                         qhead += 32;
                         RELOAD_G();
                     }
                 }
             }
             const long long te_ = STAT_CLK();
-            if (qtail > qhead) knn_refine<KCAP>(ws, k, lane, q, p.N, qhead, qtail - qhead);
-            knn_emit(ws, p, q, lane);
+            if (qtail > qhead) knn_refine<S>(ws, k, lane, q, p.N, qhead, qtail - qhead);
+            knn_emit<S>(ws, p, q, lane);
             STAT_ADD(10, STAT_CLK() - te_);
             STAT_ADD(3, STAT_CLK() - tb_);
             STAT_ADD(11, 1);
@@ -460,7 +428,9 @@ extern "C" int snaps_debug_stats(unsigned long long* out16, int reset) {
 
 cudaError_t knn_lattice_launch(const KnnParams& p, int grid, cudaStream_t stream) {
     const size_t smem = knn_lattice_smem_bytes(p.k, p.warps);
-    auto kernel = p.k <= 16 ? knn_lattice_kernel<16> : knn_lattice_kernel<32>;
+    const int stride = knn_list_stride(p.k);
+    auto kernel = stride == 12 ? knn_lattice_kernel<12> : stride == 20 ? knn_lattice_kernel<20>
+                : stride == 28 ? knn_lattice_kernel<28> : knn_lattice_kernel<36>;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kernel<<<grid, p.warps * 32, smem, stream>>>(p);

@@ -4,7 +4,7 @@
 
 namespace snaps {
 
-constexpr int kKnnMaxThreads = 512;  // warps * 32
+constexpr int kKnnMaxThreads = 448;  // 14 warps: 144 registers per thread
 
 struct KnnParams {
     const float* Xp;            // staged table, row-major, n_tiles*128 rows of 20 floats (seeds, query rows)
@@ -17,9 +17,8 @@ struct KnnParams {
     int n_batches;
     int batches_per_item;       // consecutive batches one warp keeps its query for
     int n_bchunks;              // ceil(n_batches / batches_per_item)
-    int n_qblocks;              // ceil(N / warps)
-    int warps;                  // consumer warps per CTA (= queries per CTA)
-    int* work_counter;          // device, zeroed before launch
+    int warps;                  // warps per CTA (each works on its own query)
+    unsigned long long* work_counter;  // device, zeroed before launch
     int32_t* out_idx;
     float* out_dist;
     float* out_kth;
