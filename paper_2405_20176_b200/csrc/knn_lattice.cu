@@ -135,36 +135,38 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N
                 w[4 * e4 + 0] = b.x; w[4 * e4 + 1] = b.y; w[4 * e4 + 2] = b.z; w[4 * e4 + 3] = b.w;
             }
         }
-#pragma unroll 1
+        // which of the 32 new sums can enter (against the threshold as it stands now) ...
+        unsigned mask = 0u;
+#pragma unroll
         for (int j4 = 0; j4 < 8; ++j4) {
             const float4 m = *reinterpret_cast<const float4*>(&MT(lane, 4 * j4));
-            if (fminf(fminf(m.x, m.y), fminf(m.z, m.w)) < thr) {
+            mask |= (m.x < thr ? 1u : 0u) << (4 * j4);
+            mask |= (m.y < thr ? 1u : 0u) << (4 * j4 + 1);
+            mask |= (m.z < thr ? 1u : 0u) << (4 * j4 + 2);
+            mask |= (m.w < thr ? 1u : 0u) << (4 * j4 + 3);
+        }
+        // ... merged in candidate order (= increasing id).  Every id already in the list is
+        // smaller than the new one, so "list entry e precedes (d, id)" is v[e] <= d, and the
+        // new sorted array is v'[e] = v[e] if v[e] <= d, else d if v[e-1] <= d, else v[e-1].
+#pragma unroll 1
+        while (mask) {
+            const int j = __ffs(mask) - 1;
+            mask &= mask - 1u;
+            const float d = MT(lane, j);
+            if (d < thr) {
+                const int id = CANDID(j);
                 changed = true;
-                const int4 ids = *reinterpret_cast<const int4*>(&CANDID(4 * j4));
-#define MERGE_ONE(dval, idval)                                                        \
-                if ((dval) < thr) {                                                   \
-                    const float d = (dval);                                           \
-                    const int id = (idval);                                           \
-                    int pos = 0;                                                      \
-                    _Pragma("unroll") for (int e = 0; e < NE; ++e)                    \
-                        pos += static_cast<int>((v[e] < d) | ((v[e] == d) & (w[e] < id))); \
-                    _Pragma("unroll") for (int e = NE - 1; e >= 1; --e) {             \
-                        const bool up = e > pos;                                      \
-                        v[e] = up ? v[e - 1] : v[e];                                  \
-                        w[e] = up ? w[e - 1] : w[e];                                  \
-                    }                                                                 \
-                    _Pragma("unroll") for (int e = 0; e < NE; ++e) {                  \
-                        const bool here = e == pos;                                   \
-                        v[e] = here ? d : v[e];                                       \
-                        w[e] = here ? id : w[e];                                      \
-                    }                                                                 \
-                    thr = fminf(seed, v[NE - 1]);                                     \
+                bool below[NE];
+#pragma unroll
+                for (int e = 0; e < NE; ++e) below[e] = v[e] <= d;
+#pragma unroll
+                for (int e = NE - 1; e >= 1; --e) {
+                    v[e] = below[e] ? v[e] : (below[e - 1] ? d : v[e - 1]);
+                    w[e] = below[e] ? w[e] : (below[e - 1] ? id : w[e - 1]);
                 }
-                MERGE_ONE(m.x, ids.x)
-                MERGE_ONE(m.y, ids.y)
-                MERGE_ONE(m.z, ids.z)
-                MERGE_ONE(m.w, ids.w)
-#undef MERGE_ONE
+                v[0] = below[0] ? v[0] : d;
+                w[0] = below[0] ? w[0] : id;
+                thr = fminf(seed, v[NE - 1]);
             }
         }
         if (changed) {
@@ -310,6 +312,7 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
     // synchronisation anywhere in the kernel (a warp never waits for a slower query)
     const long long n_items = static_cast<long long>(p.N) * p.n_bchunks;
     const unsigned lt = (1u << lane) - 1u;
+    const int n_blocks = p.n_blocks;
     for (;;) {
         long long item = 0;
         if (lane == 0) item = atomicAdd(p.work_counter, 1ull);
@@ -349,57 +352,73 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
                 wq[j] = w[j] * qhi[j];
             }
             int qhead = 0, qtail = 0;  // queue positions (warp-uniform, monotone)
-            // candidates: block t = rows 32t..32t+31, lane = row, four coalesced 128-bit loads
-            const float4* blk = p.Xb + lane;
-            float4 n0 = __ldg(blk), n1 = __ldg(blk + 32), n2 = __ldg(blk + 64), n3 = __ldg(blk + 96);
+            // candidates: block t = rows 32t..32t+31, lane = row, four coalesced 128-bit loads;
+            // two register sets alternate (one in use, one in flight) -- no register moves
+#define LOAD_BLOCK(dst, t_)                                                                   \
+    {                                                                                         \
+        const float4* b_ = p.Xb + static_cast<size_t>(t_) * 128 + lane;                        \
+        dst.v0 = __ldg(b_); dst.v1 = __ldg(b_ + 32); dst.v2 = __ldg(b_ + 64); dst.v3 = __ldg(b_ + 96); \
+    }
+#define FILTER_BLOCK(r, t_)                                                                   \
+    {                                                                                         \
+        const float c[15] = {r.v0.x, r.v0.y, r.v0.z, r.v0.w, r.v1.x, r.v1.y, r.v1.z, r.v1.w,   \
+                             r.v2.x, r.v2.y, r.v2.z, r.v2.w, r.v3.x, r.v3.y, r.v3.z};          \
+        /* keep the padding word of the fourth load live until here: otherwise its register is  \
+           handed out as scratch while the prefetch is still in flight and the warp stalls on it */ \
+        asm volatile("" ::"f"(r.v3.w));                                                        \
+        float sq[kLow];                                                                       \
+        _Pragma("unroll") for (int j = 0; j < kLow; ++j) {                                    \
+            const float diff = c[j] - qlo[j];                                                 \
+            sq[j] = __fmul_rn(diff, diff);                                                    \
+        }                                                                                     \
+        float base = 0.f;                                                                     \
+        _Pragma("unroll") for (int j = 0; j < 9; ++j) {                                       \
+            const float diff = __fmaf_rn(c[kLow + j], w[j], -wq[j]);                          \
+            base = __fmaf_rn(diff, diff, base);                                               \
+        }                                                                                     \
+        /* FILTER: group lower bounds against group maxima */                                 \
+        float X[16];                                                                          \
+        X[0] = base;                                                                          \
+        _Pragma("unroll") for (int u = 1; u < 16; ++u) {                                      \
+            const int hb = 31 - __clz(u);                                                     \
+            X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);                                  \
+        }                                                                                     \
+        bool pa = false, pb = false;                                                          \
+        _Pragma("unroll") for (int u = 0; u < 16; u += 2) {                                   \
+            pa |= (X[u] < G[u]);                                                              \
+            pb |= (X[u + 1] < G[u + 1]);                                                      \
+        }                                                                                     \
+        const bool pass = pa | pb;                                                            \
+        const unsigned bal = __ballot_sync(kFull, pass);                                      \
+        if (bal) {                                                                            \
+            /* COMPACT */                                                                     \
+            if (pass) {                                                                       \
+                float4* e = QUEUE4((qtail + __popc(bal & lt)) % kQueue);                      \
+                e[0] = make_float4(__int_as_float((t_) * 32 + lane), base, sq[0], sq[1]);     \
+                e[1] = make_float4(sq[2], sq[3], sq[4], sq[5]);                               \
+            }                                                                                 \
+            qtail += __popc(bal);                                                             \
+            if (qtail - qhead >= 32) {                                                        \
+                knn_refine<S>(ws, k, lane, q, p.N, qhead, 32);                                \
+                qhead += 32;                                                                  \
+                RELOAD_G();                                                                   \
+            }                                                                                 \
+        }                                                                                     \
+    }
+            struct Blk { float4 v0, v1, v2, v3; } ra, rb;
+            LOAD_BLOCK(ra, 0)
+            rb = ra;
 #pragma unroll 1
-            for (int t = 0; t < p.n_blocks; ++t) {
-                const float4 r0 = n0, r1 = n1, r2 = n2, r3 = n3;
-                if (t + 1 < p.n_blocks) {   // software prefetch of the next block
-                    blk += 128;
-                    n0 = __ldg(blk); n1 = __ldg(blk + 32); n2 = __ldg(blk + 64); n3 = __ldg(blk + 96);
-                }
-                const float c[15] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w,
-                                     r2.x, r2.y, r2.z, r2.w, r3.x, r3.y, r3.z};
-                float sq[kLow];
-#pragma unroll
-                for (int j = 0; j < kLow; ++j) {
-                    const float diff = c[j] - qlo[j];
-                    sq[j] = __fmul_rn(diff, diff);
-                }
-                float base = 0.f;
-#pragma unroll
-                for (int j = 0; j < 9; ++j) {
-                    const float diff = __fmaf_rn(c[kLow + j], w[j], -wq[j]);
-                    base = __fmaf_rn(diff, diff, base);
-                }
-                // FILTER: group lower bounds against group maxima
-                float X[16];
-                X[0] = base;
-#pragma unroll
-                for (int u = 1; u < 16; ++u) {
-                    const int hb = 31 - __clz(u);
-                    X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);
-                }
-                bool pass = false;
-#pragma unroll
-                for (int u = 0; u < 16; ++u) pass |= (X[u] < G[u]);
-                const unsigned bal = __ballot_sync(kFull, pass);
-                if (bal) {
-                    // COMPACT
-                    if (pass) {
-                        float4* e = QUEUE4((qtail + __popc(bal & lt)) % kQueue);
-                        e[0] = make_float4(__int_as_float(t * 32 + lane), base, sq[0], sq[1]);
-                        e[1] = make_float4(sq[2], sq[3], sq[4], sq[5]);
-                    }
-                    qtail += __popc(bal);
-                    if (qtail - qhead >= 32) {
-                        knn_refine<S>(ws, k, lane, q, p.N, qhead, 32);
-                        qhead += 32;
-                        RELOAD_G();
-                    }
+            for (int t = 0; t < n_blocks; t += 2) {
+                if (t + 1 < n_blocks) LOAD_BLOCK(rb, t + 1)
+                FILTER_BLOCK(ra, t)
+                if (t + 1 < n_blocks) {
+                    if (t + 2 < n_blocks) LOAD_BLOCK(ra, t + 2)
+                    FILTER_BLOCK(rb, t + 1)
                 }
             }
+#undef LOAD_BLOCK
+#undef FILTER_BLOCK
             const long long te_ = STAT_CLK();
             if (qtail > qhead) knn_refine<S>(ws, k, lane, q, p.N, qhead, qtail - qhead);
             knn_emit<S>(ws, p, q, lane);
