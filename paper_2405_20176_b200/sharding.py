@@ -1,0 +1,42 @@
+"""Multi-GPU sharding of one catalogue's mask list (host logic, no device work).
+
+The method has no exchange step (feature spaces are independent and are dealt to the
+least loaded GPU), so ranks share nothing but the replicated table.  Masks are dealt by *batch*
+(all masks with the same features 6..14 stay together, so each rank still enumerates complete
+sub-lattices and the per-pair squared differences are reused as on one GPU); batches are dealt
+round-robin in Gray order so that every rank gets the same mix of subspace dimensions.
+Outputs of the ranks concatenate; `unshard` gives the permutation back to the caller's order.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+LOW_BITS = 6  # lattice features of a batch (csrc/snaps_device.cuh: kLow)
+
+
+def _gray_rank(g: np.ndarray) -> np.ndarray:
+    b = g.copy()
+    s = 1
+    while s < 16:
+        b ^= b >> s
+        s <<= 1
+    return b
+
+
+def shard_masks(masks, rank: int, world: int):
+    """-> (indices into `masks` owned by `rank`, ascending).  Disjoint over ranks, covers all."""
+    m = np.asarray(masks, dtype=np.uint16).astype(np.int64)
+    assert 0 <= rank < world
+    high = m >> LOW_BITS
+    keys = np.unique(high)
+    order = keys[np.argsort(_gray_rank(keys), kind="stable")]        # batches in Gray order
+    owner = {int(h): i % world for i, h in enumerate(order)}
+    mine = np.fromiter((owner[int(h)] == rank for h in high), dtype=bool, count=len(m))
+    return np.flatnonzero(mine)
+
+
+def unshard(index_lists, n_masks: int) -> np.ndarray:
+    """Given every rank's index list, the permutation p with concat(outputs)[p] in caller order."""
+    cat = np.concatenate(index_lists)
+    assert len(cat) == n_masks and len(np.unique(cat)) == n_masks
+    return np.argsort(cat, kind="stable")
