@@ -196,7 +196,7 @@ void decompose(int64_t N, int n_batches, int warps, int grid, int* n_qblocks, in
 int knn_warps_for(int k) {
     // per-warp list state in shared memory; what is left of the 256 KB array stays L1 for the
     // table stream
-    const size_t budget = 200 * 1024;
+    const size_t budget = 227 * 1024;
     int w = snaps::kKnnMaxThreads / 32;
     if (const char* e = getenv("SNAPS_KNN_WARPS")) {   // tuning knob: warps (queries) per CTA
         const int v = atoi(e);
@@ -221,9 +221,15 @@ snaps_status knn_enqueue(const Workspace& w, const snaps::BatchDesc* d_batches, 
     p.batches = d_batches;
     p.n_batches = nb;
     p.warps = knn_warps_for(k);
-    // runs of up to 32 consecutive batches keep a query's lists warm for seeding; items are
-    // plentiful (N per run), so the dynamic per-warp scheduler balances the tail
-    p.batches_per_item = std::min(nb, 32);
+    // runs of 8 consecutive batches: long enough for the previous batch's neighbours to seed the
+    // next one, short enough that the in-degree rows of the batches in flight (8 x 64 x 4N bytes)
+    // stay in L2; items are plentiful (N per run), so the per-warp scheduler balances the tail
+    int run = 8;
+    if (const char* e = getenv("SNAPS_KNN_RUN")) {      // tuning knob: batches per work item
+        const int v = atoi(e);
+        if (v >= 1) run = v;
+    }
+    p.batches_per_item = std::min(nb, run);
     p.n_bchunks = (nb + p.batches_per_item - 1) / p.batches_per_item;
     p.work_counter = reinterpret_cast<unsigned long long*>(w.counter);
     p.out_idx = out_idx;

@@ -4,7 +4,7 @@
 
 namespace snaps {
 
-constexpr int kKnnMaxThreads = 448;  // 14 warps: 144 registers per thread
+constexpr int kKnnMaxThreads = 512;  // 16 warps x 128 registers
 
 struct KnnParams {
     const float* Xp;            // staged table, row-major, n_tiles*128 rows of 20 floats (seeds, query rows)

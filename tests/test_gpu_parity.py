@@ -212,3 +212,98 @@ def test_argument_errors(snaps):
     assert e.value.status == 3
     with pytest.raises(snaps.SnapsError):
         snaps.knn_selfjoin(X, [0b11], 3, lists=False, scores=False)
+
+
+# ---------------------------------------------------------------- full-size configs, sampled outputs
+def _sampled_knn_check(snaps, oracle_mod, cfg, out, X, masks, n_masks_s, n_queries_s, seed):
+    """Compare kth/mean of a scores-only full-size run with the oracle on sampled (mask, query)
+    rows (a kNN row does not depend on other queries, so per-row sampling is exact)."""
+    rng = np.random.default_rng(seed)
+    pc = workloads.popcount(masks)
+    ms = np.sort(np.concatenate([rng.choice(np.flatnonzero(pc == d), min(2, int((pc == d).sum())), replace=False)
+                                 for d in np.unique(pc)]))[:n_masks_s]
+    qs = np.sort(rng.choice(len(X), n_queries_s, replace=False))
+    oi, od = oracle_mod.knn_selfjoin(X, masks[ms], cfg.k, queries=qs)
+    kth = out["kth"][ms][:, qs].cpu().numpy().astype(np.float64)
+    mean = out["mean"][ms][:, qs].cpu().numpy().astype(np.float64)
+    assert (np.abs(kth - od[:, :, -1]) <= 1e-4 * od[:, :, -1] + 1e-7).all()
+    assert (np.abs(mean - od.mean(axis=2)) <= 1e-4 * od.mean(axis=2) + 1e-7).all()
+    return ms, qs
+
+
+def test_config2_full_size_sampled(snaps, oracle_mod):
+    """BASELINE.json configs[1] exactly as bench.py launches it (N=31,693, 32,752 masks, k=10,
+    scores only): sampled rows against the oracle, whole-output invariants, and the in-degree of
+    two complete masks against a full oracle join of those masks."""
+    import torch
+    cfg = workloads.get_config("c2_snapshot1_knn")
+    X, masks = cfg.table(), cfg.masks()
+    N = len(X)
+    out = snaps.knn_selfjoin(_dev(X), masks, cfg.k, lists=False)
+    torch.cuda.synchronize()
+    ms, qs = _sampled_knn_check(snaps, oracle_mod, cfg, out, X, masks, 28, 48, seed=5)
+    # invariants over the whole output (PAPER.md:136; mean <= kth; monotone along lattice edges)
+    assert bool((out["indeg"].sum(dim=1) == N * cfg.k).all())
+    assert bool((out["mean"] <= out["kth"] * (1 + 1e-6)).all()) and bool((out["kth"] > 0).all())
+    pos = {int(m): i for i, m in enumerate(masks)}
+    rng = np.random.default_rng(6)
+    for m in rng.choice(masks, 40, replace=False):
+        for f in range(15):
+            sup = int(m) | (1 << f)
+            if sup != int(m):
+                a, b = out["kth"][pos[int(m)]], out["kth"][pos[sup]]
+                assert bool((a <= b * (1 + 1e-5) + 1e-7).all())      # D_(k)(S) <= D_(k)(S u {f})
+    # in-degree: two complete masks, full oracle join
+    for mi in (ms[0], ms[-1]):
+        oi, od = oracle_mod.knn_selfjoin(X, masks[mi:mi + 1], cfg.k + 1)
+        unamb = (od[0, :, cfg.k] - od[0, :, cfg.k - 1]) > 1e-5 * od[0, :, cfg.k]
+        hist = np.bincount(oi[0, :, :cfg.k].ravel(), minlength=N)
+        got = out["indeg"][mi].cpu().numpy()
+        if unamb.all():
+            assert (got == hist).all()
+        else:   # only ambiguous queries' k-th neighbours may differ
+            assert np.abs(got - hist).sum() <= 2 * (~unamb).sum()
+
+
+def test_config3_full_size_sampled(snaps, oracle_mod):
+    """BASELINE.json configs[2]: DSSJ over all 32,752 masks at N=31,693 with per-dimension eps_d for
+    ~50 neighbours (calibrated by the oracle on a 1,000-point sample); sampled rows + invariants."""
+    import torch
+    from oracle.calibrate import eps_per_dimension
+    cfg = workloads.get_config("c3_snapshot1_dssj")
+    X, masks = cfg.table(), cfg.masks()
+    N = len(X)
+    eps = eps_per_dimension(X, masks, cfg.target_neighbours, seed=cfg.seed, max_masks_per_dim=4,
+                            n_query_sample=300).astype(np.float32)
+    out = snaps.range_selfjoin(_dev(X), masks, eps)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(7)
+    pc = workloads.popcount(masks)
+    ms = np.sort(np.concatenate([rng.choice(np.flatnonzero(pc == d), min(2, int((pc == d).sum())), replace=False)
+                                 for d in np.unique(pc)]))
+    qs = np.sort(rng.choice(N, 48, replace=False))
+    cnt = out["count"][ms][:, qs].cpu().numpy()
+    check_range(cnt, out["sumdist"][ms][:, qs].cpu().numpy(), out["mean"][ms][:, qs].cpu().numpy(),
+                oracle_mod, X, masks[ms], eps[ms], queries=qs)
+    mean_cnt = out["count"].float().mean().item()
+    assert 10 < mean_cnt < 250, mean_cnt                     # calibrated for ~50 (sample noise allowed)
+    # no self-pairs, counts bounded by N-1; the mean is 0 exactly where the count is 0 (A6)
+    assert int(out["count"].max().item()) <= N - 1
+    assert bool((out["mean"][out["count"] == 0] == 0).all())
+
+
+def test_streamed_large_table_reduced_configs_4_5(snaps, oracle_mod):
+    """Configs 4-5 in shape (pair masks + full set; 256 sampled masks, k=16) on a reduced N, through
+    the pinned-host streaming call; sampled rows against the oracle."""
+    import torch
+    for name, n, k, masks in (("c4", 60_000, 10, workloads.pair_masks_plus_full(15)),
+                              ("c5", 40_000, 16, workloads.sample_masks(256, 4)[::4])):
+        X = workloads.make_table(n, 3, outlier_frac=0.001)
+        st = snaps.knn_selfjoin_streamed(_dev(X), masks, k, masks_per_batch=16, lists=True)
+        torch.cuda.synchronize()
+        rng = np.random.default_rng(8)
+        qs = np.sort(rng.choice(n, 24, replace=False))
+        sel = np.arange(len(masks))[:: max(1, len(masks) // 12)]
+        oi, od = oracle_mod.knn_selfjoin(X, masks[sel], k + 1, queries=qs)
+        check_knn(st["idx"][sel][:, qs].numpy(), st["dist"][sel][:, qs].numpy(), oi, od, queries=qs)
+        assert bool((st["indeg"].sum(dim=1) == n * k).all())
