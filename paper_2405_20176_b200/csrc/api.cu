@@ -181,18 +181,6 @@ int sm_count() {
     return cached;
 }
 
-// Work decomposition: queries per CTA = consumer warps; batches are cut into chunks so that
-// there are enough (query block, chunk) items to balance the persistent CTAs, while chunks
-// stay long enough for threshold seeding from the previous batch to pay.
-void decompose(int64_t N, int n_batches, int warps, int grid, int* n_qblocks, int* bpi, int* n_bchunks) {
-    *n_qblocks = static_cast<int>((N + warps - 1) / warps);
-    int chunks = 1;
-    while (static_cast<int64_t>(*n_qblocks) * chunks < 24LL * grid && (n_batches + chunks) / (chunks + 1) >= 8)
-        ++chunks;
-    *bpi = (n_batches + chunks - 1) / chunks;
-    *n_bchunks = (n_batches + *bpi - 1) / *bpi;
-}
-
 int knn_warps_for(int k) {
     // per-warp list state in shared memory; what is left of the 256 KB array stays L1 for the
     // table stream
@@ -326,21 +314,23 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
     CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * nb,
                              cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
+    CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
     snaps::RangeParams p;
     p.Xp = w.Xp;
+    p.Xb = w.Xb;
+    p.n_blocks = n_blocks_for(N);
     p.N = static_cast<int>(N);
-    p.n_tiles = n_tiles;
     p.batches = w.batches;
     p.n_batches = nb;
-    p.warps = 15;
-    const int grid_max = sm_count();
-    decompose(N, nb, p.warps, grid_max, &p.n_qblocks, &p.batches_per_item, &p.n_bchunks);
-    p.work_counter = w.counter;
+    p.warps = snaps::kRangeMaxThreads / 32;
+    p.batches_per_item = std::min(nb, 8);
+    p.n_bchunks = (nb + p.batches_per_item - 1) / p.batches_per_item;
+    p.work_counter = reinterpret_cast<unsigned long long*>(w.counter);
     p.out_count = out_count;
     p.out_sum = out_sumdist;
     p.out_mean = out_mean;
-    const int64_t items = static_cast<int64_t>(p.n_qblocks) * p.n_bchunks;
-    const int grid = static_cast<int>(std::min<int64_t>(items, grid_max));
+    const int64_t items = N * p.n_bchunks;
+    const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
     const bool prof = prof_begin(st);
     CUDA_TRY(snaps::range_lattice_launch(p, grid, st));
     prof_end(prof, st);

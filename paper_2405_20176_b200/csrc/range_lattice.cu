@@ -3,90 +3,122 @@
 //
 // What it computes: PAPER.md:111, 154-156: for every object i and mask S the number of
 // objects j != i with D(i,j;S) <= eps_S and the sum of those D
-// (PAPER.md:165).  Same pair staging and add-only subset sums as knn_lattice.cu; the
-// thresholds are the per-mask constants eps_S^2 (held in registers, one per lattice slot),
-// so no list state exists: a warp vote per group of 4 sums gates the counting path, where
-// a ballot's popcount is added to the list's counter by lane 0 (the warp-aggregated form
-// of an atomic increment) and each lane adds sqrt(d^2) to its own partial sum, reduced in
-// lane order at the end of the batch (deterministic).
+// (PAPER.md:165).  Same structure as knn_lattice.cu:
+//   * one warp = one query x the 64 masks {H u T : T subset of features 0..5}; lanes = candidates
+//     streamed from the blocked table (L2 resident, coalesced 128-bit loads, register prefetch);
+//   * FILTER: the 16 partial sums X[u] over features 2..5 are lower bounds of their group's four
+//     sums, so a candidate can be an eps-neighbour in group u only if X[u] < G[u] = the group's
+//     largest eps^2 (constants per batch, register-held);
+//   * COMPACT passing candidates into a per-warp queue; REFINE every 32 of them: lane = candidate
+//     forms the 64 subset sums (add-only, fixed order), a 32 x 32 shared-memory transpose hands
+//     them to the list owners (lane = list), which count the sums below eps^2 with one popcount
+//     and add sqrt(d^2) of the hits to the list's running sum in candidate order (deterministic;
+//     each list is touched by one lane only -- no atomics are needed at all).
 #include "range_lattice.cuh"
 
 namespace snaps {
 
-#define R_CNT(L) wsi[(L)]
-#define R_SLOT(L) wsi[64 + (L)]
-#define R_SUM(L, ln) ws[128 + (L) * 33 + (ln)]
+constexpr int kRQueue = 64;  // queue entries of 8 words; refine as soon as 32 are waiting
+constexpr float kRInf = __builtin_huge_valf();
 
-#define COUNT_ONE(sval, Lidx)                                                 \
-    {                                                                         \
-        const bool in_ = (sval) < thr[Lidx];                                  \
-        const unsigned bal_ = __ballot_sync(kFull, in_);                      \
-        if (bal_) {                                                           \
-            if (lane == 0) R_CNT(Lidx) += __popc(bal_);                       \
-            if (WITH_SUM && in_) R_SUM(Lidx, lane) += sqrtf(sval);            \
-        }                                                                     \
+// per-warp shared-memory words
+#define R_THR(L) ws[(L)]
+#define R_SLOT(L) wsi[64 + (L)]
+#define R_CNT(L) wsi[128 + (L)]
+#define R_SUM(L) ws[192 + (L)]
+#define R_QROW(j) ws[256 + (j)]
+#define R_MT(T, j) ws[272 + (T) * 36 + (j)]
+#define R_QUEUE4(e) (reinterpret_cast<float4*>(ws + 272 + 32 * 36) + 2 * (e))
+
+__host__ __device__ constexpr int range_warp_words() { return 272 + 32 * 36 + kRQueue * 8; }
+
+template <bool WITH_SUM>
+__device__ __noinline__ void range_refine(float* ws, int lane, int q, int N, int head, int n) {
+    int* wsi = reinterpret_cast<int*>(ws);
+    __syncwarp();
+    float base = kRInf;
+    float sq[kLow] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    if (lane < n) {
+        const float4* e = R_QUEUE4((head + lane) % kRQueue);
+        const float4 a = e[0], b = e[1];
+        const int cand = __float_as_int(a.x);
+        base = a.y; sq[0] = a.z; sq[1] = a.w;
+        sq[2] = b.x; sq[3] = b.y; sq[4] = b.z; sq[5] = b.w;
+        // self by index (reading A4) and padding rows (A19) are never counted
+        if (cand == q || cand >= N) base = kRInf;
     }
+    float X8[8];   // partial sums over features 2,3,4; feature 5 is added per half
+    X8[0] = base;
+#pragma unroll
+    for (int u = 1; u < 8; ++u) {
+        const int hb = 31 - __clz(u);
+        X8[u] = __fadd_rn(X8[u & ~(1 << hb)], sq[2 + hb]);
+    }
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+#pragma unroll
+        for (int uu = 0; uu < 8; ++uu) {
+            const float s0 = half ? __fadd_rn(X8[uu], sq[5]) : X8[uu];
+            const float s1 = __fadd_rn(s0, sq[0]);
+            const float s2 = __fadd_rn(s0, sq[1]);
+            const float s3 = __fadd_rn(s1, sq[1]);
+            R_MT(4 * uu + 0, lane) = s0;
+            R_MT(4 * uu + 1, lane) = s1;
+            R_MT(4 * uu + 2, lane) = s2;
+            R_MT(4 * uu + 3, lane) = s3;
+        }
+        __syncwarp();
+        // ---- lane = list T: d^2 < nextafter(eps^2)  <=>  D <= eps (closed ball, reading A2)
+        const int T = 32 * half + lane;
+        const float thr = R_THR(T);
+        unsigned mask = 0u;
+#pragma unroll
+        for (int j4 = 0; j4 < 8; ++j4) {
+            const float4 m = *reinterpret_cast<const float4*>(&R_MT(lane, 4 * j4));
+            mask |= (m.x < thr ? 1u : 0u) << (4 * j4);
+            mask |= (m.y < thr ? 1u : 0u) << (4 * j4 + 1);
+            mask |= (m.z < thr ? 1u : 0u) << (4 * j4 + 2);
+            mask |= (m.w < thr ? 1u : 0u) << (4 * j4 + 3);
+        }
+        if (mask) {
+            R_CNT(T) += __popc(mask);
+            if (WITH_SUM) {
+                float s = R_SUM(T);
+#pragma unroll 1
+                while (mask) {
+                    const int j = __ffs(mask) - 1;
+                    mask &= mask - 1u;
+                    s += sqrtf(R_MT(lane, j));
+                }
+                R_SUM(T) = s;
+            }
+        }
+        __syncwarp();
+    }
+}
 
 template <bool WITH_SUM>
 __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(const RangeParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
-    float* tiles = reinterpret_cast<float*>(smem);
-    uint64_t* full = reinterpret_cast<uint64_t*>(smem + kStages * kTileBytes);
-    uint64_t* empty = full + kStages;
-    int* s_item = reinterpret_cast<int*>(empty + kStages);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int W = p.warps;
-    const int ws_floats = 128 + (WITH_SUM ? 64 * 33 : 0);
-    float* ws = reinterpret_cast<float*>(smem + kStages * kTileBytes + 128) +
-                static_cast<size_t>(warp < W ? warp : 0) * ws_floats;
+    float* ws = reinterpret_cast<float*>(smem) + static_cast<size_t>(warp) * range_warp_words();
     int* wsi = reinterpret_cast<int*>(ws);
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < kStages; ++s) {
-            mbar_init(&full[s], 1);
-            mbar_init(&empty[s], W);
-        }
-        mbar_fence_init();
-    }
-    __syncthreads();
-
-    uint32_t g = 0;
-    const int n_items = p.n_qblocks * p.n_bchunks;
+    const long long n_items = static_cast<long long>(p.N) * p.n_bchunks;
+    const unsigned lt = (1u << lane) - 1u;
+    const int n_blocks = p.n_blocks;
     for (;;) {
-        if (threadIdx.x == 0) s_item[0] = atomicAdd(p.work_counter, 1);
-        __syncthreads();
-        const int item = s_item[0];
-        __syncthreads();
+        long long item = 0;
+        if (lane == 0) item = atomicAdd(p.work_counter, 1ull);
+        item = __shfl_sync(kFull, item, 0);
         if (item >= n_items) break;
-        const int qb = item % p.n_qblocks, bc = item / p.n_qblocks;
+        const int q = static_cast<int>(item % p.N);
+        const int bc = static_cast<int>(item / p.N);
         const int b0 = bc * p.batches_per_item;
         const int b1 = min(b0 + p.batches_per_item, p.n_batches);
-        const uint32_t ntile_total = static_cast<uint32_t>(b1 - b0) * p.n_tiles;
-
-        if (warp == W) {
-            if (lane == 0) {
-                for (uint32_t t = 0; t < ntile_total; ++t) {
-                    const uint32_t gg = g + t;
-                    const int s = gg % kStages;
-                    const uint32_t ph = (gg / kStages) & 1u;
-                    mbar_wait(&empty[s], ph ^ 1u);
-                    mbar_arrive_expect_tx(&full[s], kTileBytes);
-                    bulk_g2s(tiles + static_cast<size_t>(s) * kTileRows * kRowFloats,
-                             p.Xp + static_cast<size_t>(t % p.n_tiles) * kTileRows * kRowFloats,
-                             kTileBytes, &full[s]);
-                }
-            }
-            g += ntile_total;
-            __syncwarp();
-            continue;
-        }
-
-        const int q = qb * W + warp;
-        const bool active = q < p.N;
         float qlo[kLow];
         float qhi[9];
         {
-            const float* qr = p.Xp + static_cast<size_t>(active ? q : 0) * kRowFloats;
+            const float* qr = p.Xp + static_cast<size_t>(q) * kRowFloats;
 #pragma unroll
             for (int j = 0; j < kLow; ++j) qlo[j] = qr[j];
 #pragma unroll
@@ -96,129 +128,118 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
         for (int b = b0; b < b1; ++b) {
             const BatchDesc* bd = &p.batches[b];
             const uint32_t H = bd->hmask;
-            float thr[kLat];
-            {
-                const float4* t4 = reinterpret_cast<const float4*>(bd->thr);
-#pragma unroll
-                for (int i4 = 0; i4 < 16; ++i4) {
-                    const float4 v = t4[i4];
-                    thr[4 * i4 + 0] = v.x;
-                    thr[4 * i4 + 1] = v.y;
-                    thr[4 * i4 + 2] = v.z;
-                    thr[4 * i4 + 3] = v.w;
-                }
-            }
             __syncwarp();
+#pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const int L = lane + 32 * h;
-                R_CNT(L) = 0;
+                R_THR(L) = bd->thr[L];
                 R_SLOT(L) = bd->slot[L];
+                R_CNT(L) = 0;
+                R_SUM(L) = 0.f;
             }
-            if (WITH_SUM)
-                for (int L = 0; L < kLat; ++L) R_SUM(L, lane) = 0.f;
             __syncwarp();
-            float wq[9], w[9];
+            float G[16];   // group maxima of the (constant) thresholds
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                const float4 t = *reinterpret_cast<const float4*>(&R_THR(4 * u));
+                G[u] = fmaxf(fmaxf(t.x, t.y), fmaxf(t.z, t.w));
+            }
+            float wq[9], w[9];  // high features: diff = c*w - q*w, w in {0,1}
 #pragma unroll
             for (int j = 0; j < 9; ++j) {
                 w[j] = ((H >> (kLow + j)) & 1u) ? 1.f : 0.f;
                 wq[j] = w[j] * qhi[j];
             }
+            int qhead = 0, qtail = 0;
+#define LOAD_BLOCK(dst, t_)                                                                   \
+    {                                                                                         \
+        const float4* b_ = p.Xb + static_cast<size_t>(t_) * 128 + lane;                        \
+        dst.v0 = __ldg(b_); dst.v1 = __ldg(b_ + 32); dst.v2 = __ldg(b_ + 64); dst.v3 = __ldg(b_ + 96); \
+    }
+#define FILTER_BLOCK(r, t_)                                                                   \
+    {                                                                                         \
+        const float c[15] = {r.v0.x, r.v0.y, r.v0.z, r.v0.w, r.v1.x, r.v1.y, r.v1.z, r.v1.w,   \
+                             r.v2.x, r.v2.y, r.v2.z, r.v2.w, r.v3.x, r.v3.y, r.v3.z};          \
+        float sq[kLow];                                                                       \
+        _Pragma("unroll") for (int j = 0; j < kLow; ++j) {                                    \
+            const float diff = c[j] - qlo[j];                                                 \
+            sq[j] = __fmul_rn(diff, diff);                                                    \
+        }                                                                                     \
+        float base = 0.f;                                                                     \
+        _Pragma("unroll") for (int j = 0; j < 9; ++j) {                                       \
+            const float diff = __fmaf_rn(c[kLow + j], w[j], -wq[j]);                          \
+            base = __fmaf_rn(diff, diff, base);                                               \
+        }                                                                                     \
+        float X[16];                                                                          \
+        X[0] = base;                                                                          \
+        _Pragma("unroll") for (int u = 1; u < 16; ++u) {                                      \
+            const int hb = 31 - __clz(u);                                                     \
+            X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);                                  \
+        }                                                                                     \
+        bool pa = false, pb = false;                                                          \
+        _Pragma("unroll") for (int u = 0; u < 16; u += 2) {                                   \
+            pa |= (X[u] < G[u]);                                                              \
+            pb |= (X[u + 1] < G[u + 1]);                                                      \
+        }                                                                                     \
+        const bool pass = pa | pb;                                                            \
+        const unsigned bal = __ballot_sync(kFull, pass);                                      \
+        if (bal) {                                                                            \
+            if (pass) {                                                                       \
+                float4* e = R_QUEUE4((qtail + __popc(bal & lt)) % kRQueue);                   \
+                e[0] = make_float4(__int_as_float((t_) * 32 + lane), base, sq[0], sq[1]);     \
+                e[1] = make_float4(sq[2], sq[3], sq[4], sq[5]);                               \
+            }                                                                                 \
+            qtail += __popc(bal);                                                             \
+            if (qtail - qhead >= 32) {                                                        \
+                range_refine<WITH_SUM>(ws, lane, q, p.N, qhead, 32);                          \
+                qhead += 32;                                                                  \
+            }                                                                                 \
+        }                                                                                     \
+    }
+            struct Blk { float4 v0, v1, v2, v3; } ra, rb;
+            LOAD_BLOCK(ra, 0)
+            rb = ra;
 #pragma unroll 1
-            for (int t = 0; t < p.n_tiles; ++t, ++g) {
-                const int s = g % kStages;
-                mbar_wait(&full[s], (g / kStages) & 1u);
-                if (active) {
-                    const float* tile = tiles + static_cast<size_t>(s) * kTileRows * kRowFloats;
-#pragma unroll 1
-                    for (int it = 0; it < kTileRows / 32; ++it) {
-                        const int cand = t * kTileRows + it * 32 + lane;
-                        const float4* row =
-                            reinterpret_cast<const float4*>(tile + (it * 32 + lane) * kRowFloats);
-                        const float4 r0 = row[0], r1 = row[1], r2 = row[2], r3 = row[3];
-                        const float c[15] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w,
-                                             r2.x, r2.y, r2.z, r2.w, r3.x, r3.y, r3.z};
-                        float sq[kLow];
-#pragma unroll
-                        for (int j = 0; j < kLow; ++j) {
-                            const float diff = c[j] - qlo[j];
-                            sq[j] = __fmul_rn(diff, diff);
-                        }
-                        float base = 0.f;
-#pragma unroll
-                        for (int j = 0; j < 9; ++j) {
-                            const float diff = __fmaf_rn(c[kLow + j], w[j], -wq[j]);
-                            base = __fmaf_rn(diff, diff, base);
-                        }
-                        if (cand >= p.N || cand == q) base = __int_as_float(0x7f800000);
-                        float X[16];
-                        X[0] = base;
-#pragma unroll
-                        for (int u = 1; u < 16; ++u) {
-                            const int hb = 31 - __clz(u);
-                            X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);
-                        }
-#pragma unroll
-                        for (int u = 0; u < 16; ++u) {
-                            const float s0 = X[u];
-                            const float s1 = __fadd_rn(s0, sq[0]);
-                            const float s2 = __fadd_rn(s0, sq[1]);
-                            const float s3 = __fadd_rn(s1, sq[1]);
-                            const bool hit = (s0 < thr[4 * u]) | (s1 < thr[4 * u + 1]) |
-                                             (s2 < thr[4 * u + 2]) | (s3 < thr[4 * u + 3]);
-                            if (__any_sync(kFull, hit)) {
-                                COUNT_ONE(s0, 4 * u + 0)
-                                COUNT_ONE(s1, 4 * u + 1)
-                                COUNT_ONE(s2, 4 * u + 2)
-                                COUNT_ONE(s3, 4 * u + 3)
-                            }
-                        }
-                    }
+            for (int t = 0; t < n_blocks; t += 2) {
+                if (t + 1 < n_blocks) LOAD_BLOCK(rb, t + 1)
+                FILTER_BLOCK(ra, t)
+                if (t + 1 < n_blocks) {
+                    if (t + 2 < n_blocks) LOAD_BLOCK(ra, t + 2)
+                    FILTER_BLOCK(rb, t + 1)
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&empty[s]);
             }
-            if (active) {
-                __syncwarp();
-                for (int h = 0; h < 2; ++h) {
-                    const int L = lane + 32 * h;
-                    const int sl = R_SLOT(L);
-                    if (sl < 0) continue;
-                    const size_t o = static_cast<size_t>(sl) * static_cast<size_t>(p.N) + q;
-                    const int cnt = R_CNT(L);
-                    p.out_count[o] = static_cast<uint32_t>(cnt);
-                    if (WITH_SUM) {
-                        float tot = 0.f;
-                        for (int ln = 0; ln < 32; ++ln) tot += R_SUM(L, ln);
-                        if (p.out_sum) p.out_sum[o] = tot;
-                        if (p.out_mean) p.out_mean[o] = cnt > 0 ? tot / static_cast<float>(cnt) : 0.f;
-                    }
+#undef LOAD_BLOCK
+#undef FILTER_BLOCK
+            if (qtail > qhead) range_refine<WITH_SUM>(ws, lane, q, p.N, qhead, qtail - qhead);
+            // ---- a7: counts, sums, means (0 when there is no neighbour: PAPER.md:266, reading A6)
+            __syncwarp();
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int L = lane + 32 * h;
+                const int sl = R_SLOT(L);
+                if (sl < 0) continue;
+                const size_t o = static_cast<size_t>(sl) * static_cast<size_t>(p.N) + q;
+                const int cnt = R_CNT(L);
+                p.out_count[o] = static_cast<uint32_t>(cnt);
+                if (WITH_SUM) {
+                    const float tot = R_SUM(L);
+                    if (p.out_sum) p.out_sum[o] = tot;
+                    if (p.out_mean) p.out_mean[o] = cnt > 0 ? tot / static_cast<float>(cnt) : 0.f;
                 }
-                __syncwarp();
             }
         }
     }
 }
 
-size_t range_lattice_smem_bytes(int warps, bool with_sum) {
-    return static_cast<size_t>(kStages) * kTileBytes + 128 +
-           static_cast<size_t>(warps) * (128 + (with_sum ? 64 * 33 : 0)) * 4;
-}
+size_t range_lattice_smem_bytes(int warps) { return static_cast<size_t>(warps) * range_warp_words() * 4; }
 
 cudaError_t range_lattice_launch(const RangeParams& p, int grid, cudaStream_t stream) {
     const bool with_sum = p.out_sum != nullptr || p.out_mean != nullptr;
-    const size_t smem = range_lattice_smem_bytes(p.warps, with_sum);
-    cudaError_t e;
-    if (with_sum) {
-        e = cudaFuncSetAttribute(range_lattice_kernel<true>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        range_lattice_kernel<true><<<grid, (p.warps + 1) * 32, smem, stream>>>(p);
-    } else {
-        e = cudaFuncSetAttribute(range_lattice_kernel<false>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        range_lattice_kernel<false><<<grid, (p.warps + 1) * 32, smem, stream>>>(p);
-    }
+    const size_t smem = range_lattice_smem_bytes(p.warps);
+    auto kernel = with_sum ? range_lattice_kernel<true> : range_lattice_kernel<false>;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kernel<<<grid, p.warps * 32, smem, stream>>>(p);
     return cudaGetLastError();
 }
 

@@ -7,22 +7,22 @@ namespace snaps {
 constexpr int kRangeMaxThreads = 512;
 
 struct RangeParams {
-    const float* Xp;
+    const float* Xp;            // staged table, row-major (query rows)
+    const float4* Xb;           // staged table, blocked (candidate stream)
+    int n_blocks;               // ceil(N / 32)
     int N;
-    int n_tiles;
     const BatchDesc* batches;   // thr[] = nextafter(eps^2) per slot, -1 for unused slots
     int n_batches;
     int batches_per_item;
     int n_bchunks;
-    int n_qblocks;
-    int warps;
-    int* work_counter;
+    int warps;                  // warps per CTA (each works on its own query)
+    unsigned long long* work_counter;  // device, zeroed before launch
     uint32_t* out_count;
     float* out_sum;
     float* out_mean;
 };
 
-size_t range_lattice_smem_bytes(int warps, bool with_sum);
+size_t range_lattice_smem_bytes(int warps);
 cudaError_t range_lattice_launch(const RangeParams& p, int grid, cudaStream_t stream);
 
 }  // namespace snaps
