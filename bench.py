@@ -153,6 +153,57 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
+def run_range(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks):
+    """Extra line for the DSSJ config (BASELINE.json configs[2]): one pass of snaps_range_selfjoin
+    over all masks with the oracle-calibrated eps_d (calibration outside the timed region).
+    Not the headline metric; printed with the same keys so that the numbers in DESIGN.md can be
+    reproduced with `python bench.py --config c3_snapshot1_dssj`."""
+    from oracle.calibrate import eps_per_dimension     # input preparation, as in the parity test
+    X = workloads.make_table(cfg.n, cfg.seed + rank, cols=list(range(cfg.n_feat)), outlier_frac=0.01)
+    masks = cfg.masks()
+    eps = eps_per_dimension(X, masks, cfg.target_neighbours, seed=cfg.seed, max_masks_per_dim=4,
+                            n_query_sample=300).astype(np.float32)
+    N, n_masks = len(X), len(masks)
+    Xd = torch.from_numpy(X).to(dev)
+    out = snaps.range_selfjoin(Xd, masks, eps)
+    ws = out.pop("_workspace")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    snaps.profile_enable(True)
+
+    def step():
+        flush.zero_()
+        snaps.range_selfjoin(Xd, masks, eps, out=out, workspace=ws)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kernel_ms = []
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+        kernel_ms.append(snaps.profile_last_kernel_ms()[0])
+    ev1.record()
+    torch.cuda.synchronize()
+    barrier()
+    ms = max_over_ranks(ev0.elapsed_time(ev1) / args.steps)
+    if rank == 0:
+        evals = float(N) * N * n_masks
+        peak, _ = peaks()
+        lane_ops = 2.0 * evals + 30.0 * float(N) * N * 512
+        print(json.dumps({
+            "metric": "subspaces/sec (DSSJ N=31,693, eps_d for ~50 neighbours)", "value": world * n_masks / (ms * 1e-3),
+            "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: DSSJ over N={N} x 15, all {n_masks} subspaces, counts + sums + means"},
+            "evals_per_s": world * evals / (ms * 1e-3), "mean_neighbours": float(out["count"].float().mean().item()),
+            "roofline": {"bound": "alu", "kernel": "range_lattice_kernel", "achieved": lane_ops / (np.mean(kernel_ms) * 1e-3) / 1e12,
+                         "peak": peak / 1e12, "unit": "TFLOP/s", "frac": lane_ops / (np.mean(kernel_ms) * 1e-3) / peak,
+                         "traffic": None, "kernel_ms": float(np.mean(kernel_ms))},
+            "gpu_launches": 4 * args.steps}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -203,7 +254,11 @@ def main():
         return float(t.item())
 
     cfg = workloads.get_config(args.config)
-    assert "knn" in cfg.join
+    if cfg.join == "range":
+        run_range(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks)
+        if world > 1:
+            dist.destroy_process_group()
+        return
     X = workloads.make_table(cfg.n, cfg.seed + rank, cols=list(range(cfg.n_feat)),
                              outlier_frac=0.01 if cfg.n < 100000 else 0.001)
     masks = cfg.masks()
@@ -238,7 +293,7 @@ def main():
         step()
         ms, n = snaps.profile_last_kernel_ms()     # waits for this step's join kernel
         kernel_ms.append(ms)
-        launches += n + 2                          # + stage_table kernel + the L2 flush fill
+        launches += n + 3                          # + the two staging kernels + the L2 flush fill
     ev1.record()
     torch.cuda.synchronize()
     barrier()
