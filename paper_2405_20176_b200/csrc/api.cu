@@ -15,6 +15,7 @@
 #include "../../include/snaps.h"
 #include "knn_lattice.cuh"
 #include "misc_kernels.cuh"
+#include "pivot_sort.cuh"
 #include "range_lattice.cuh"
 
 namespace {
@@ -131,7 +132,14 @@ snaps_status check_common(const float* d_X, int64_t N, int n_feat, int64_t ld,
     return SNAPS_OK;
 }
 
+// Large tables take the pivot sweep (pivot_sort.cuh); SNAPS_KNN_SWEEP=0/1 overrides the size rule.
+bool use_sweep(int64_t N) {
+    if (const char* e = getenv("SNAPS_KNN_SWEEP")) return atoi(e) != 0;
+    return N >= (1 << 18);
+}
+
 struct Workspace {
+    unsigned char* pivot;   // 9 pivot sets + sort scratch (only when use_sweep(N))
     float* Xp;
     float4* Xb;
     int* counter;
@@ -142,29 +150,83 @@ struct Workspace {
 
 int n_blocks_for(int64_t N) { return static_cast<int>((N + 31) / 32); }
 
-size_t base_workspace_bytes(int64_t N, int n_masks) {
+
+
+// one pivot set: sorted blocked table, sorted values, position -> id, id -> position
+size_t pivot_set_bytes(int64_t N) {
+    const size_t n_pad = static_cast<size_t>(n_blocks_for(N)) * 32;
+    return align_up(n_pad * 64, 256) + 2 * align_up(n_pad * 4, 256) + align_up(static_cast<size_t>(N) * 4, 256);
+}
+
+size_t pivot_region_bytes(int64_t N) {
+    return 9 * pivot_set_bytes(N) + align_up(snaps::pivot_sort_temp_bytes(n_blocks_for(N) * 32), 256);
+}
+
+size_t base_workspace_bytes(int64_t N, int n_masks, int k) {
     const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
     const size_t blocked = align_up(static_cast<size_t>(n_blocks_for(N)) * 2048, 256);
     const size_t batches = align_up(static_cast<size_t>(n_masks) * sizeof(snaps::BatchDesc), 256);
-    return table + blocked + 256 + batches;
+    const size_t pivot = (k > 0 && use_sweep(N)) ? pivot_region_bytes(N) : 0;
+    return table + blocked + 256 + batches + pivot;
 }
 
-snaps_status carve(void* d_ws, size_t bytes, int64_t N, int n_masks, Workspace* w) {
+snaps_status carve(void* d_ws, size_t bytes, int64_t N, int n_masks, int k, Workspace* w) {
     if (!d_ws) return fail(SNAPS_INVALID_ARG, "d_workspace is NULL");
     if (reinterpret_cast<uintptr_t>(d_ws) % 256 != 0)
         return fail(SNAPS_INVALID_ARG, "d_workspace not 256-byte aligned");
-    const size_t need = base_workspace_bytes(N, n_masks);
+    const size_t need = base_workspace_bytes(N, n_masks, k);
     if (bytes < need)
         return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", bytes, need);
     unsigned char* p = static_cast<unsigned char*>(d_ws);
     const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
     const size_t blocked = align_up(static_cast<size_t>(n_blocks_for(N)) * 2048, 256);
+    const size_t batches = align_up(static_cast<size_t>(n_masks) * sizeof(snaps::BatchDesc), 256);
     w->Xp = reinterpret_cast<float*>(p);
     w->Xb = reinterpret_cast<float4*>(p + table);
     w->counter = reinterpret_cast<int*>(p + table + blocked);
     w->batches = reinterpret_cast<snaps::BatchDesc*>(p + table + blocked + 256);
+    w->pivot = p + table + blocked + 256 + batches;
     w->ring = p + need;
     w->ring_bytes = bytes - need;
+    return SNAPS_OK;
+}
+
+// Pointers of pivot set j (feature kLow + j) inside the pivot region.
+struct PivotSet {
+    float4* Xs;
+    float* piv;
+    int* idmap;
+    int* pos;
+};
+
+PivotSet pivot_set(const Workspace& w, int64_t N, int j) {
+    const size_t n_pad = static_cast<size_t>(n_blocks_for(N)) * 32;
+    unsigned char* b = w.pivot + static_cast<size_t>(j) * pivot_set_bytes(N);
+    PivotSet s;
+    s.Xs = reinterpret_cast<float4*>(b);
+    s.piv = reinterpret_cast<float*>(b + align_up(n_pad * 64, 256));
+    s.idmap = reinterpret_cast<int*>(b + align_up(n_pad * 64, 256) + align_up(n_pad * 4, 256));
+    s.pos = reinterpret_cast<int*>(b + align_up(n_pad * 64, 256) + 2 * align_up(n_pad * 4, 256));
+    return s;
+}
+
+// Build the sorted copies for the pivot features the batches use (lowest high feature of each).
+snaps_status build_pivots(const Workspace& w, int64_t N, const std::vector<snaps::BatchDesc>& batches,
+                          cudaStream_t st) {
+    bool need[9] = {false, false, false, false, false, false, false, false, false};
+    for (const snaps::BatchDesc& b : batches) {
+        const uint32_t hb = b.hmask >> snaps::kLow;
+        if (hb) need[__builtin_ctz(hb)] = true;
+    }
+    const int n_pad = n_blocks_for(N) * 32;
+    void* temp = w.pivot + 9 * pivot_set_bytes(N);
+    const size_t temp_bytes = snaps::pivot_sort_temp_bytes(n_pad);
+    for (int j = 0; j < 9; ++j) {
+        if (!need[j]) continue;
+        const PivotSet s = pivot_set(w, N, j);
+        CUDA_TRY(snaps::pivot_build(w.Xp, static_cast<int>(N), n_pad, snaps::kLow + j, s.Xs, s.piv, s.idmap,
+                                    s.pos, temp, temp_bytes, st));
+    }
     return SNAPS_OK;
 }
 
@@ -203,8 +265,15 @@ snaps_status knn_enqueue(const Workspace& w, const snaps::BatchDesc* d_batches, 
     p.Xp = w.Xp;
     p.Xb = w.Xb;
     p.n_blocks = n_blocks_for(N);
+    p.sweep = use_sweep(N) ? 1 : 0;
+    for (int j = 0; j < 9; ++j) {
+        const PivotSet s = p.sweep ? pivot_set(w, N, j) : PivotSet{nullptr, nullptr, nullptr, nullptr};
+        p.Xs[j] = s.Xs;
+        p.piv[j] = s.piv;
+        p.idmap[j] = s.idmap;
+        p.pos[j] = s.pos;
+    }
     p.N = static_cast<int>(N);
-    p.n_tiles = n_tiles_for(N);
     p.k = k;
     p.batches = d_batches;
     p.n_batches = nb;
@@ -244,7 +313,7 @@ const char* snaps_version(void) { return "snaps-b200 0.1 (sm_100a)"; }
 size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k) {
     if (N < 2 || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES || n_masks < 1 || k < 0 || k > SNAPS_MAX_K)
         return 0;
-    return base_workspace_bytes(N, n_masks);
+    return base_workspace_bytes(N, n_masks, k);
 }
 
 int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t* h_masks, int n_masks) {
@@ -267,7 +336,7 @@ snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t
     if (!out_idx && !out_dist && !out_kth && !out_mean && !out_indeg)
         return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
     Workspace w;
-    rc = carve(d_workspace, workspace_bytes, N, n_masks, &w);
+    rc = carve(d_workspace, workspace_bytes, N, n_masks, k, &w);
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     std::vector<snaps::BatchDesc> batches;
@@ -276,6 +345,10 @@ snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t
     CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
                                        n_tiles * snaps::kTileRows, st));
     CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
+    if (use_sweep(N)) {
+        rc = build_pivots(w, N, batches, st);
+        if (rc) return rc;
+    }
     if (out_indeg)
         CUDA_TRY(cudaMemsetAsync(out_indeg, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, st));
     CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
@@ -302,7 +375,7 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
         thr[m] = nextafterf(e2, INFINITY);
     }
     Workspace w;
-    rc = carve(d_workspace, workspace_bytes, N, n_masks, &w);
+    rc = carve(d_workspace, workspace_bytes, N, n_masks, 0, &w);
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     std::vector<snaps::BatchDesc> batches;
@@ -382,7 +455,7 @@ snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat
     if (!h_out_idx && !h_out_dist && !h_out_kth && !h_out_mean && !h_out_indeg)
         return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
     Workspace w;
-    rc = carve(d_workspace, workspace_bytes, N, n_masks, &w);
+    rc = carve(d_workspace, workspace_bytes, N, n_masks, k, &w);
     if (rc) return rc;
     const size_t ring_need = snaps_stream_ring_bytes(N, k, masks_per_batch);
     if (w.ring_bytes < ring_need)
@@ -422,6 +495,10 @@ snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat
         all_batches.insert(all_batches.end(), b.begin(), b.end());
     }
     group_off.push_back(all_batches.size());
+    if (use_sweep(N)) {
+        rc = build_pivots(w, N, all_batches, st);
+        if (rc) return rc;
+    }
     CUDA_TRY(cudaMemcpyAsync(w.batches, all_batches.data(), sizeof(snaps::BatchDesc) * all_batches.size(),
                              cudaMemcpyHostToDevice, st));
     cudaStream_t side;

@@ -74,7 +74,10 @@ __host__ __device__ constexpr int knn_warp_words(int k) {
 // ties are broken by the smaller id (reading A3).
 // The add order (high features by FMA in feature order -> features 2,3,4,5 -> 0 -> 1) is the
 // same wherever a squared distance is formed, so a value never depends on scheduling.
-template <int S>
+// ORD = candidates arrive in increasing id order (the plain scan).  The pivot sweep visits them
+// in sorted-feature order instead: then ties at the threshold must be let through (<=) and the
+// (d^2, id) key is compared explicitly.
+template <int S, bool ORD>
 __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N, int head, int n) {
     constexpr int NE = S > 32 ? 32 : S;   // list elements held (S = 36 carries 4 words of padding)
     int* wsi = reinterpret_cast<int*>(ws);
@@ -140,10 +143,10 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N
 #pragma unroll
         for (int j4 = 0; j4 < 8; ++j4) {
             const float4 m = *reinterpret_cast<const float4*>(&MT(lane, 4 * j4));
-            mask |= (m.x < thr ? 1u : 0u) << (4 * j4);
-            mask |= (m.y < thr ? 1u : 0u) << (4 * j4 + 1);
-            mask |= (m.z < thr ? 1u : 0u) << (4 * j4 + 2);
-            mask |= (m.w < thr ? 1u : 0u) << (4 * j4 + 3);
+            mask |= ((ORD ? m.x < thr : m.x <= thr) ? 1u : 0u) << (4 * j4);
+            mask |= ((ORD ? m.y < thr : m.y <= thr) ? 1u : 0u) << (4 * j4 + 1);
+            mask |= ((ORD ? m.z < thr : m.z <= thr) ? 1u : 0u) << (4 * j4 + 2);
+            mask |= ((ORD ? m.w < thr : m.w <= thr) ? 1u : 0u) << (4 * j4 + 3);
         }
         // ... merged in candidate order (= increasing id).  Every id already in the list is
         // smaller than the new one, so "list entry e precedes (d, id)" is v[e] <= d, and the
@@ -153,12 +156,14 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N
             const int j = __ffs(mask) - 1;
             mask &= mask - 1u;
             const float d = MT(lane, j);
-            if (d < thr) {
-                const int id = CANDID(j);
+            const int id = CANDID(j);
+            if (ORD ? (d < thr)
+                    : (d <= thr && ((d < v[NE - 1]) | ((d == v[NE - 1]) & (id < w[NE - 1]))))) {
                 changed = true;
                 bool below[NE];
 #pragma unroll
-                for (int e = 0; e < NE; ++e) below[e] = v[e] <= d;
+                for (int e = 0; e < NE; ++e)
+                    below[e] = ORD ? (v[e] <= d) : ((v[e] < d) | ((v[e] == d) & (w[e] < id)));
 #pragma unroll
                 for (int e = NE - 1; e >= 1; --e) {
                     v[e] = below[e] ? v[e] : (below[e - 1] ? d : v[e - 1]);
@@ -298,9 +303,17 @@ __device__ __noinline__ void knn_emit(float* ws, const KnnParams& p, int q, int 
             G[4 * i4 + 2] = v.z;                                              \
             G[4 * i4 + 3] = v.w;                                              \
         }                                                                     \
+        if (SWEEP) {                                                          \
+            Gall = G[0];                                                      \
+            _Pragma("unroll") for (int u = 1; u < 16; ++u) Gall = fmaxf(Gall, G[u]); \
+        }                                                                     \
     } while (0)
 
-template <int S>
+// SWEEP = false: every candidate block in id order (tables that fit the L2 / small N).
+// SWEEP = true: the pivot sweep (pivot_sort.cu): the batch's table copy sorted by the batch's
+// lowest high feature f is scanned outwards from the query's own position, and a direction stops
+// at the first block whose nearest value of f is farther than every threshold of the batch.
+template <int S, bool SWEEP>
 __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const KnnParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -343,7 +356,12 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             SLOT(lane + 32) = bd->slot[lane + 32];
             knn_seed<S>(ws, p.Xp, q, k, H, has_prev, lane);
             STAT_ADD(9, STAT_CLK() - tb_);
+            // group 0 = lattice slots {}, {0}, {1}, {0,1}: when only {0,1} is asked for (always so for
+            // masks of >= 2 features when H is empty), its own sum is the group's bound -- X[0] alone
+            // would be 0 there and let every candidate through
+            const bool g0_both = (SLOT(0) < 0) & (SLOT(1) < 0) & (SLOT(2) < 0);
             float G[16];
+            float Gall = 0.f;   // SWEEP: largest threshold of the batch
             RELOAD_G();
             float wq[9], w[9];  // high features: diff = c*w - q*w, w in {0,1}
 #pragma unroll
@@ -354,12 +372,12 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             int qhead = 0, qtail = 0;  // queue positions (warp-uniform, monotone)
             // candidates: block t = rows 32t..32t+31, lane = row, four coalesced 128-bit loads;
             // two register sets alternate (one in use, one in flight) -- no register moves
-#define LOAD_BLOCK(dst, t_)                                                                   \
+#define LOAD_BLOCK(dst, tab_, t_)                                                             \
     {                                                                                         \
-        const float4* b_ = p.Xb + static_cast<size_t>(t_) * 128 + lane;                        \
+        const float4* b_ = (tab_) + static_cast<size_t>(t_) * 128 + lane;                      \
         dst.v0 = __ldg(b_); dst.v1 = __ldg(b_ + 32); dst.v2 = __ldg(b_ + 64); dst.v3 = __ldg(b_ + 96); \
     }
-#define FILTER_BLOCK(r, t_)                                                                   \
+#define FILTER_BLOCK(r, t_, CAND_)                                                            \
     {                                                                                         \
         const float c[15] = {r.v0.x, r.v0.y, r.v0.z, r.v0.w, r.v1.x, r.v1.y, r.v1.z, r.v1.w,   \
                              r.v2.x, r.v2.y, r.v2.z, r.v2.w, r.v3.x, r.v3.y, r.v3.z};          \
@@ -383,10 +401,12 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             const int hb = 31 - __clz(u);                                                     \
             X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);                                  \
         }                                                                                     \
-        bool pa = false, pb = false;                                                          \
+        float x0 = X[0];                                                                      \
+        if (g0_both) x0 = __fadd_rn(__fadd_rn(X[0], sq[0]), sq[1]);                           \
+        bool pa = SWEEP ? (x0 <= G[0]) : (x0 < G[0]), pb = false;                             \
         _Pragma("unroll") for (int u = 0; u < 16; u += 2) {                                   \
-            pa |= (X[u] < G[u]);                                                              \
-            pb |= (X[u + 1] < G[u + 1]);                                                      \
+            if (u > 0) pa |= SWEEP ? (X[u] <= G[u]) : (X[u] < G[u]);                          \
+            pb |= SWEEP ? (X[u + 1] <= G[u + 1]) : (X[u + 1] < G[u + 1]);                     \
         }                                                                                     \
         const bool pass = pa | pb;                                                            \
         const unsigned bal = __ballot_sync(kFull, pass);                                      \
@@ -394,33 +414,75 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             /* COMPACT */                                                                     \
             if (pass) {                                                                       \
                 float4* e = QUEUE4((qtail + __popc(bal & lt)) % kQueue);                      \
-                e[0] = make_float4(__int_as_float((t_) * 32 + lane), base, sq[0], sq[1]);     \
+                e[0] = make_float4(__int_as_float(CAND_), base, sq[0], sq[1]);                \
                 e[1] = make_float4(sq[2], sq[3], sq[4], sq[5]);                               \
             }                                                                                 \
             qtail += __popc(bal);                                                             \
             if (qtail - qhead >= 32) {                                                        \
-                knn_refine<S>(ws, k, lane, q, p.N, qhead, 32);                                \
+                knn_refine<S, !SWEEP>(ws, k, lane, q, p.N, qhead, 32);                        \
                 qhead += 32;                                                                  \
                 RELOAD_G();                                                                   \
             }                                                                                 \
         }                                                                                     \
     }
-            struct Blk { float4 v0, v1, v2, v3; } ra, rb;
-            LOAD_BLOCK(ra, 0)
-            rb = ra;
+            struct Blk { float4 v0, v1, v2, v3; };
+            if (!SWEEP) {
+                Blk ra, rb;
+                LOAD_BLOCK(ra, p.Xb, 0)
+                rb = ra;
 #pragma unroll 1
-            for (int t = 0; t < n_blocks; t += 2) {
-                if (t + 1 < n_blocks) LOAD_BLOCK(rb, t + 1)
-                FILTER_BLOCK(ra, t)
-                if (t + 1 < n_blocks) {
-                    if (t + 2 < n_blocks) LOAD_BLOCK(ra, t + 2)
-                    FILTER_BLOCK(rb, t + 1)
+                for (int t = 0; t < n_blocks; t += 2) {
+                    if (t + 1 < n_blocks) LOAD_BLOCK(rb, p.Xb, t + 1)
+                    FILTER_BLOCK(ra, t, (t) * 32 + lane)
+                    if (t + 1 < n_blocks) {
+                        if (t + 2 < n_blocks) LOAD_BLOCK(ra, p.Xb, t + 2)
+                        FILTER_BLOCK(rb, t + 1, (t + 1) * 32 + lane)
+                    }
+                }
+            } else {
+                const int pf = (H >> kLow) ? __ffs(H >> kLow) - 1 : -1;   // pivot: lowest high feature
+                const float4* tab = pf >= 0 ? p.Xs[pf] : p.Xb;
+                const int* idm = pf >= 0 ? p.idmap[pf] : nullptr;
+                const float* pv = pf >= 0 ? p.piv[pf] : nullptr;
+                const int t0 = pf >= 0 ? (p.pos[pf][q] >> 5) : 0;
+                const float qf = pf >= 0 ? QROW(kLow + pf) : 0.f;
+#pragma unroll 1
+                for (int dir = 1; dir >= -1; dir -= 2) {
+                    int t = dir > 0 ? t0 : t0 - 1;
+                    const int t_end = dir > 0 ? n_blocks : -1;
+                    if (t != t_end) {
+                        const int eo = dir > 0 ? 31 : 0;   // the block's row farthest along the sweep
+                        Blk nx;
+                        float pe_n = 0.f;
+                        LOAD_BLOCK(nx, tab, t)
+                        if (pv) pe_n = __ldg(pv + 32 * t + eo);
+#pragma unroll 1
+                        for (;;) {
+                            const Blk r = nx;
+                            const float pe = pe_n;
+                            const int tn = t + dir;
+                            if (tn != t_end) {
+                                LOAD_BLOCK(nx, tab, tn)
+                                if (pv) pe_n = __ldg(pv + 32 * tn + eo);
+                            }
+                            FILTER_BLOCK(r, t, (idm ? __ldg(idm + t * 32 + lane) : t * 32 + lane))
+                            if (pv) {
+                                // every row further along has (x_f - q_f)^2 >= de^2, a lower bound of
+                                // all its sums (non-negative terms, monotone rounding)
+                                const float de = dir > 0 ? pe - qf : qf - pe;
+                                if (de > 0.f && __fmul_rn(de, de) > Gall) break;
+                            }
+                            if (tn == t_end) break;
+                            t = tn;
+                        }
+                    }
+                    if (!pv) break;   // unsorted table: one full pass
                 }
             }
 #undef LOAD_BLOCK
 #undef FILTER_BLOCK
             const long long te_ = STAT_CLK();
-            if (qtail > qhead) knn_refine<S>(ws, k, lane, q, p.N, qhead, qtail - qhead);
+            if (qtail > qhead) knn_refine<S, !SWEEP>(ws, k, lane, q, p.N, qhead, qtail - qhead);
             knn_emit<S>(ws, p, q, lane);
             STAT_ADD(10, STAT_CLK() - te_);
             STAT_ADD(3, STAT_CLK() - tb_);
@@ -448,8 +510,11 @@ extern "C" int snaps_debug_stats(unsigned long long* out16, int reset) {
 cudaError_t knn_lattice_launch(const KnnParams& p, int grid, cudaStream_t stream) {
     const size_t smem = knn_lattice_smem_bytes(p.k, p.warps);
     const int stride = knn_list_stride(p.k);
-    auto kernel = stride == 12 ? knn_lattice_kernel<12> : stride == 20 ? knn_lattice_kernel<20>
-                : stride == 28 ? knn_lattice_kernel<28> : knn_lattice_kernel<36>;
+    auto kernel = p.sweep
+        ? (stride == 12 ? knn_lattice_kernel<12, true> : stride == 20 ? knn_lattice_kernel<20, true>
+           : stride == 28 ? knn_lattice_kernel<28, true> : knn_lattice_kernel<36, true>)
+        : (stride == 12 ? knn_lattice_kernel<12, false> : stride == 20 ? knn_lattice_kernel<20, false>
+           : stride == 28 ? knn_lattice_kernel<28, false> : knn_lattice_kernel<36, false>);
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kernel<<<grid, p.warps * 32, smem, stream>>>(p);

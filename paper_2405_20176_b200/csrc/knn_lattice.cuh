@@ -10,8 +10,12 @@ struct KnnParams {
     const float* Xp;            // staged table, row-major, n_tiles*128 rows of 20 floats (seeds, query rows)
     const float4* Xb;           // staged table, blocked: [n_blocks][4 feature groups][32 rows] float4
     int n_blocks;               // ceil(N / 32)
+    int sweep;                  // 1: pivot sweep over the sorted copies below (pivot_sort.cuh)
+    const float4* Xs[9];        // per pivot feature 6+j: blocked table sorted by that feature
+    const float* piv[9];        //   its sorted values
+    const int* idmap[9];        //   sorted position -> object id
+    const int* pos[9];          //   object id -> sorted position
     int N;
-    int n_tiles;
     int k;
     const BatchDesc* batches;   // device
     int n_batches;

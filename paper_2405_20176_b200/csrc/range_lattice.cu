@@ -138,6 +138,9 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
                 R_SUM(L) = 0.f;
             }
             __syncwarp();
+            // group 0 = lattice slots {}, {0}, {1}, {0,1}: when only {0,1} is asked for, its own sum is
+            // the group's bound (X[0] alone is 0 when H is empty and would let every candidate through)
+            const bool g0_both = (R_SLOT(0) < 0) & (R_SLOT(1) < 0) & (R_SLOT(2) < 0);
             float G[16];   // group maxima of the (constant) thresholds
 #pragma unroll
             for (int u = 0; u < 16; ++u) {
@@ -176,9 +179,11 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
             const int hb = 31 - __clz(u);                                                     \
             X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);                                  \
         }                                                                                     \
-        bool pa = false, pb = false;                                                          \
+        float x0 = X[0];                                                                      \
+        if (g0_both) x0 = __fadd_rn(__fadd_rn(X[0], sq[0]), sq[1]);                           \
+        bool pa = x0 < G[0], pb = false;                                                      \
         _Pragma("unroll") for (int u = 0; u < 16; u += 2) {                                   \
-            pa |= (X[u] < G[u]);                                                              \
+            if (u > 0) pa |= (X[u] < G[u]);                                                   \
             pb |= (X[u + 1] < G[u + 1]);                                                      \
         }                                                                                     \
         const bool pass = pa | pb;                                                            \

@@ -307,3 +307,49 @@ def test_streamed_large_table_reduced_configs_4_5(snaps, oracle_mod):
         oi, od = oracle_mod.knn_selfjoin(X, masks[sel], k + 1, queries=qs)
         check_knn(st["idx"][sel][:, qs].numpy(), st["dist"][sel][:, qs].numpy(), oi, od, queries=qs)
         assert bool((st["indeg"].sum(dim=1) == n * k).all())
+
+
+# ---------------------------------------------------------------- pivot sweep (large-N path)
+@pytest.fixture
+def force_sweep(monkeypatch):
+    """The library switches to the pivot sweep at N >= 2^18; SNAPS_KNN_SWEEP=1 forces it so that the
+    path can be checked element by element at sizes the oracle finishes in seconds."""
+    monkeypatch.setenv("SNAPS_KNN_SWEEP", "1")
+    yield
+    monkeypatch.delenv("SNAPS_KNN_SWEEP", raising=False)
+
+
+@pytest.mark.parametrize("n,nf,k,seed", [(129, 15, 16, 5), (1537, 15, 10, 8), (3000, 12, 3, 7), (700, 9, 10, 11)])
+def test_pivot_sweep_random_tables(snaps, oracle_mod, force_sweep, n, nf, k, seed):
+    X = workloads.make_table(n, seed, cols=list(range(nf)), outlier_frac=0.02)
+    allm = workloads.all_masks(nf, 1)
+    rng = np.random.default_rng(seed)
+    masks = rng.choice(allm, min(len(allm), 60), replace=False)
+    _knn_case(snaps, oracle_mod, X, masks, k)
+
+
+def test_pivot_sweep_ties(snaps, oracle_mod, force_sweep):
+    # candidates no longer arrive in id order: ties at the threshold must still go to the smaller id
+    X = workloads.hypercube_table(9)
+    _knn_case(snaps, oracle_mod, X, workloads.all_masks(9, 1)[::7], 10)
+    X = workloads.duplicate_block_table(900, 3, frac=0.3)
+    masks = np.array([(1 << 13) | (1 << 14), (1 << 13) | 1, 0x7FFF, 1 << 14, (1 << 6) | 3], dtype=np.uint16)
+    g, _ = _knn_case(snaps, oracle_mod, X, masks, 10)
+    oi, od = oracle_mod.knn_selfjoin(X, masks, 10)
+    zero = od[0, :, -1] == 0
+    assert zero.sum() > 100 and (g["idx"][0][zero] == oi[0][zero]).all()
+
+
+def test_pivot_sweep_equals_plain_scan(snaps, oracle_mod, monkeypatch):
+    import torch
+    X = workloads.make_table(4000, 13, outlier_frac=0.01)
+    masks = workloads.pair_masks_plus_full(15)
+    Xd = _dev(X)
+    monkeypatch.setenv("SNAPS_KNN_SWEEP", "0")
+    a = snaps.knn_selfjoin(Xd, masks, 10)
+    monkeypatch.setenv("SNAPS_KNN_SWEEP", "1")
+    b = snaps.knn_selfjoin(Xd, masks, 10)
+    torch.cuda.synchronize()
+    monkeypatch.delenv("SNAPS_KNN_SWEEP", raising=False)
+    for n in ("idx", "dist", "kth", "mean", "indeg"):
+        assert torch.equal(a[n], b[n]), n
