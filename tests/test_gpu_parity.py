@@ -353,3 +353,23 @@ def test_pivot_sweep_equals_plain_scan(snaps, oracle_mod, monkeypatch):
     monkeypatch.delenv("SNAPS_KNN_SWEEP", raising=False)
     for n in ("idx", "dist", "kth", "mean", "indeg"):
         assert torch.equal(a[n], b[n]), n
+
+
+def test_config4_full_size_sampled(snaps, oracle_mod):
+    """BASELINE.json configs[3] at full size: N=1,000,000 x 15 (seed 3, 0.1% outliers), the 105
+    two-feature subspaces plus the full space, k=10, lists and scores batched through pinned host
+    memory.  The library takes the pivot sweep at this N.  Sampled rows against the oracle."""
+    import torch
+    cfg = workloads.get_config("c4_lsst_pairs")
+    X, masks, k = cfg.table(), cfg.masks(), cfg.k
+    n = len(X)
+    st = snaps.knn_selfjoin_streamed(_dev(X), masks, k, masks_per_batch=16, lists=True)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(9)
+    qs = np.sort(rng.choice(n, 24, replace=False))
+    sel = np.concatenate([np.arange(0, len(masks), 7), [len(masks) - 1]])
+    oi, od = oracle_mod.knn_selfjoin(X, masks[sel], k + 1, queries=qs)
+    check_knn(st["idx"][sel][:, qs].numpy(), st["dist"][sel][:, qs].numpy(), oi, od, queries=qs)
+    kth = st["kth"][sel][:, qs].numpy().astype(np.float64)
+    assert (np.abs(kth - od[:, :, k - 1]) <= 1e-4 * od[:, :, k - 1] + 1e-7).all()
+    assert bool((st["indeg"].sum(dim=1) == n * k).all())           # PAPER.md:136
