@@ -166,7 +166,7 @@ size_t base_workspace_bytes(int64_t N, int n_masks, int k) {
     const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
     const size_t blocked = align_up(static_cast<size_t>(n_blocks_for(N)) * 2048, 256);
     const size_t batches = align_up(static_cast<size_t>(n_masks) * sizeof(snaps::BatchDesc), 256);
-    const size_t pivot = (k > 0 && use_sweep(N)) ? pivot_region_bytes(N) : 0;
+    const size_t pivot = use_sweep(N) ? pivot_region_bytes(N) : 0;
     return table + blocked + 256 + batches + pivot;
 }
 
@@ -375,7 +375,7 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
         thr[m] = nextafterf(e2, INFINITY);
     }
     Workspace w;
-    rc = carve(d_workspace, workspace_bytes, N, n_masks, 0, &w);
+    rc = carve(d_workspace, workspace_bytes, N, n_masks, 1, &w);
     if (rc) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     std::vector<snaps::BatchDesc> batches;
@@ -388,10 +388,22 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
                              cudaMemcpyHostToDevice, st));
     CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
     CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
+    if (use_sweep(N)) {
+        rc = build_pivots(w, N, batches, st);
+        if (rc) return rc;
+    }
     snaps::RangeParams p;
     p.Xp = w.Xp;
     p.Xb = w.Xb;
     p.n_blocks = n_blocks_for(N);
+    p.sweep = use_sweep(N) ? 1 : 0;
+    for (int j = 0; j < 9; ++j) {
+        const PivotSet s = p.sweep ? pivot_set(w, N, j) : PivotSet{nullptr, nullptr, nullptr, nullptr};
+        p.Xs[j] = s.Xs;
+        p.piv[j] = s.piv;
+        p.idmap[j] = s.idmap;
+        p.pos[j] = s.pos;
+    }
     p.N = static_cast<int>(N);
     p.batches = w.batches;
     p.n_batches = nb;

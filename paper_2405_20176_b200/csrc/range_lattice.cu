@@ -97,7 +97,10 @@ __device__ __noinline__ void range_refine(float* ws, int lane, int q, int N, int
     }
 }
 
-template <bool WITH_SUM>
+// SWEEP: the pivot sweep of pivot_sort.cu (large N): scan the copy sorted by the batch's lowest
+// high feature outwards from the query, stop a direction once that feature alone is beyond the
+// batch's largest eps^2 (thresholds are constants here, so the bound never moves).
+template <bool WITH_SUM, bool SWEEP>
 __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(const RangeParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -123,6 +126,8 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
             for (int j = 0; j < kLow; ++j) qlo[j] = qr[j];
 #pragma unroll
             for (int j = 0; j < 9; ++j) qhi[j] = qr[kLow + j];
+            __syncwarp();
+            if (lane < 15) R_QROW(lane) = qr[lane];
         }
 #pragma unroll 1
         for (int b = b0; b < b1; ++b) {
@@ -154,12 +159,12 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
                 wq[j] = w[j] * qhi[j];
             }
             int qhead = 0, qtail = 0;
-#define LOAD_BLOCK(dst, t_)                                                                   \
+#define LOAD_BLOCK(dst, tab_, t_)                                                             \
     {                                                                                         \
-        const float4* b_ = p.Xb + static_cast<size_t>(t_) * 128 + lane;                        \
+        const float4* b_ = (tab_) + static_cast<size_t>(t_) * 128 + lane;                      \
         dst.v0 = __ldg(b_); dst.v1 = __ldg(b_ + 32); dst.v2 = __ldg(b_ + 64); dst.v3 = __ldg(b_ + 96); \
     }
-#define FILTER_BLOCK(r, t_)                                                                   \
+#define FILTER_BLOCK(r, t_, CAND_)                                                            \
     {                                                                                         \
         const float c[15] = {r.v0.x, r.v0.y, r.v0.z, r.v0.w, r.v1.x, r.v1.y, r.v1.z, r.v1.w,   \
                              r.v2.x, r.v2.y, r.v2.z, r.v2.w, r.v3.x, r.v3.y, r.v3.z};          \
@@ -191,7 +196,7 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
         if (bal) {                                                                            \
             if (pass) {                                                                       \
                 float4* e = R_QUEUE4((qtail + __popc(bal & lt)) % kRQueue);                   \
-                e[0] = make_float4(__int_as_float((t_) * 32 + lane), base, sq[0], sq[1]);     \
+                e[0] = make_float4(__int_as_float(CAND_), base, sq[0], sq[1]);                \
                 e[1] = make_float4(sq[2], sq[3], sq[4], sq[5]);                               \
             }                                                                                 \
             qtail += __popc(bal);                                                             \
@@ -201,16 +206,59 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
             }                                                                                 \
         }                                                                                     \
     }
-            struct Blk { float4 v0, v1, v2, v3; } ra, rb;
-            LOAD_BLOCK(ra, 0)
-            rb = ra;
+            struct Blk { float4 v0, v1, v2, v3; };
+            if (!SWEEP) {
+                Blk ra, rb;
+                LOAD_BLOCK(ra, p.Xb, 0)
+                rb = ra;
 #pragma unroll 1
-            for (int t = 0; t < n_blocks; t += 2) {
-                if (t + 1 < n_blocks) LOAD_BLOCK(rb, t + 1)
-                FILTER_BLOCK(ra, t)
-                if (t + 1 < n_blocks) {
-                    if (t + 2 < n_blocks) LOAD_BLOCK(ra, t + 2)
-                    FILTER_BLOCK(rb, t + 1)
+                for (int t = 0; t < n_blocks; t += 2) {
+                    if (t + 1 < n_blocks) LOAD_BLOCK(rb, p.Xb, t + 1)
+                    FILTER_BLOCK(ra, t, (t) * 32 + lane)
+                    if (t + 1 < n_blocks) {
+                        if (t + 2 < n_blocks) LOAD_BLOCK(ra, p.Xb, t + 2)
+                        FILTER_BLOCK(rb, t + 1, (t + 1) * 32 + lane)
+                    }
+                }
+            } else {
+                const int pf = (H >> kLow) ? __ffs(H >> kLow) - 1 : -1;   // pivot: lowest high feature
+                const float4* tab = pf >= 0 ? p.Xs[pf] : p.Xb;
+                const int* idm = pf >= 0 ? p.idmap[pf] : nullptr;
+                const float* pv = pf >= 0 ? p.piv[pf] : nullptr;
+                const int t0 = pf >= 0 ? (p.pos[pf][q] >> 5) : 0;
+                const float qf = pf >= 0 ? R_QROW(kLow + pf) : 0.f;
+                float Gall = G[0];
+#pragma unroll
+                for (int u = 1; u < 16; ++u) Gall = fmaxf(Gall, G[u]);
+#pragma unroll 1
+                for (int dir = 1; dir >= -1; dir -= 2) {
+                    int t = dir > 0 ? t0 : t0 - 1;
+                    const int t_end = dir > 0 ? n_blocks : -1;
+                    if (t != t_end) {
+                        const int eo = dir > 0 ? 31 : 0;
+                        Blk nx;
+                        float pe_n = 0.f;
+                        LOAD_BLOCK(nx, tab, t)
+                        if (pv) pe_n = __ldg(pv + 32 * t + eo);
+#pragma unroll 1
+                        for (;;) {
+                            const Blk r = nx;
+                            const float pe = pe_n;
+                            const int tn = t + dir;
+                            if (tn != t_end) {
+                                LOAD_BLOCK(nx, tab, tn)
+                                if (pv) pe_n = __ldg(pv + 32 * tn + eo);
+                            }
+                            FILTER_BLOCK(r, t, (idm ? __ldg(idm + t * 32 + lane) : t * 32 + lane))
+                            if (pv) {
+                                const float de = dir > 0 ? pe - qf : qf - pe;
+                                if (de > 0.f && __fmul_rn(de, de) >= Gall) break;
+                            }
+                            if (tn == t_end) break;
+                            t = tn;
+                        }
+                    }
+                    if (!pv) break;
                 }
             }
 #undef LOAD_BLOCK
@@ -241,7 +289,8 @@ size_t range_lattice_smem_bytes(int warps) { return static_cast<size_t>(warps) *
 cudaError_t range_lattice_launch(const RangeParams& p, int grid, cudaStream_t stream) {
     const bool with_sum = p.out_sum != nullptr || p.out_mean != nullptr;
     const size_t smem = range_lattice_smem_bytes(p.warps);
-    auto kernel = with_sum ? range_lattice_kernel<true> : range_lattice_kernel<false>;
+    auto kernel = p.sweep ? (with_sum ? range_lattice_kernel<true, true> : range_lattice_kernel<false, true>)
+                          : (with_sum ? range_lattice_kernel<true, false> : range_lattice_kernel<false, false>);
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kernel<<<grid, p.warps * 32, smem, stream>>>(p);

@@ -10,6 +10,11 @@ struct RangeParams {
     const float* Xp;            // staged table, row-major (query rows)
     const float4* Xb;           // staged table, blocked (candidate stream)
     int n_blocks;               // ceil(N / 32)
+    int sweep;                  // 1: pivot sweep over the sorted copies below (pivot_sort.cuh)
+    const float4* Xs[9];
+    const float* piv[9];
+    const int* idmap[9];
+    const int* pos[9];
     int N;
     const BatchDesc* batches;   // thr[] = nextafter(eps^2) per slot, -1 for unused slots
     int n_batches;

@@ -373,3 +373,19 @@ def test_config4_full_size_sampled(snaps, oracle_mod):
     kth = st["kth"][sel][:, qs].numpy().astype(np.float64)
     assert (np.abs(kth - od[:, :, k - 1]) <= 1e-4 * od[:, :, k - 1] + 1e-7).all()
     assert bool((st["indeg"].sum(dim=1) == n * k).all())
+
+
+@pytest.mark.parametrize("n,nf,seed", [(130, 5, 1), (1537, 15, 3), (3000, 15, 5)])
+def test_pivot_sweep_range_join(snaps, oracle_mod, force_sweep, n, nf, seed):
+    import torch
+    X = workloads.make_table(n, seed, cols=list(range(nf)), outlier_frac=0.02)
+    allm = workloads.all_masks(nf, 1)
+    rng = np.random.default_rng(seed)
+    masks = rng.choice(allm, min(len(allm), 48), replace=False)
+    _, od = oracle_mod.knn_selfjoin(X, masks, min(10, n - 1))
+    eps = np.array([max(1.003 * np.median(od[m, :, -1]), 1e-3) for m in range(len(masks))], dtype=np.float32)
+    out = snaps.range_selfjoin(_dev(X), masks, eps)
+    torch.cuda.synchronize()
+    lo, hi = check_range(out["count"].cpu().numpy(), out["sumdist"].cpu().numpy(), out["mean"].cpu().numpy(),
+                         oracle_mod, X, masks, eps)
+    assert (lo == hi).mean() > 0.99
