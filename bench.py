@@ -205,6 +205,9 @@ def run_range(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks
     masks = cfg.masks()
     eps = eps_per_dimension(X, masks, cfg.target_neighbours, seed=cfg.seed, max_masks_per_dim=4,
                             n_query_sample=300).astype(np.float32)
+    if args.profile_masks > 0:      # profiling aid, see --profile-masks
+        sl = slice(args.profile_offset, args.profile_offset + args.profile_masks)
+        masks, eps = masks[sl], eps[sl]
     N, n_masks = len(X), len(masks)
     Xd = torch.from_numpy(X).to(dev)
     out = snaps.range_selfjoin(Xd, masks, eps)
