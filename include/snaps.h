@@ -55,17 +55,24 @@ const char *snaps_last_error(void);
 const char *snaps_version(void);
 
 /*
- * Bytes of device scratch the joins need for these sizes (table staged as
- * 80-byte rows, per-query candidate seeds, batch descriptors).  k may be 0
- * for the range join.  Returns 0 on invalid sizes.
+ * Bytes of device scratch the joins need for these sizes: the table staged
+ * twice (80-byte rows; 32-row blocks of four float4 groups), batch
+ * descriptors, and -- for N >= 2^18, where the joins take the pivot sweep
+ * -- nine per-feature sorted copies of the table (72 bytes per
+ * object each) plus radix-sort scratch.  k may be 0 for the range join.
+ * Returns 0 on invalid sizes.  The environment variable SNAPS_KNN_SWEEP=0/1
+ * overrides the size rule (it must have the same value when the workspace is
+ * sized and when a join is called).
  */
 size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k);
 
 /*
- * Number of (ordered query-candidate pair, mask) distance evaluations the
- * join kernels perform for this mask list, INCLUDING the lattice slots the
- * planner computes but does not output; the algorithmic count is
- * N*(N)*n_masks.  Used by bench.py's roofline arithmetic.  h_masks: host.
+ * Number of (ordered query-candidate pair, mask) distance evaluations an
+ * unpruned pass over the planned sub-lattice batches amounts to, INCLUDING the
+ * lattice slots the planner enumerates but does not output (64 per batch); the
+ * algorithmic count is N*N*n_masks.  The kernels reach the same result with
+ * fewer operations (exact lower-bound filter).  Used by
+ * bench.py's roofline arithmetic.  h_masks: host.
  */
 int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t *h_masks, int n_masks);
 
