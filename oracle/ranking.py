@@ -1,0 +1,75 @@
+"""Ranking, top-n overlap and parameter selection -- TEST INFRASTRUCTURE (oracle side, NEXT-1).
+
+Plain numpy statements of PAPER.md section 3.4 (ranking function R), section 3.5.1 /
+3.6.1 (which end of each metric is outlying), Eq. 2 (top-n overlap
+f), Eq. 3 (parameter selection) and the nested-result rule
+for the k grid (the neighbours for k_max contain those of every k_j < k_max).
+
+Readings: ranks are DENSE and start at 0 = most outlying, ties share a rank
+(verified on Table 2); an object with no eps-neighbour has mean distance 0 and
+rank 0 in the distance-aware DSSJ metric; "top-n" = the first n objects of the
+stable sort by (outlyingness, id) (reading A15: with shared ranks "r_i < n" would select more
+than n objects); Eq. 3 takes the first index that attains the minimum.
+
+Pins (tests/test_oracle_ranking.py): Table 2's four rank columns from its four metric columns;
+the section 3.5.2 worked example (U_min = {1.0, 0.4, 0.2}, U_max = {0.2, 0.5, 1.0}).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+# metric -> True if SMALL values are outlying (fewest neighbours / lowest in-degree),
+# False if LARGE values are outlying (largest mean distance)
+SMALL_IS_OUTLYING = {"dssj_count": True, "knn_indegree": True, "dssj_mean": False, "knn_mean": False,
+                     "knn_kth": False}
+
+
+def outlyingness_key(metric: str, values, counts=None) -> np.ndarray:
+    """A float64 key that sorts most-outlying first (ascending).  For the distance-aware DSSJ
+    metric, objects without neighbours (count 0) come before everything else."""
+    v = np.asarray(values, dtype=np.float64)
+    key = v.copy() if SMALL_IS_OUTLYING[metric] else -v
+    if metric == "dssj_mean":
+        assert counts is not None
+        key = np.where(np.asarray(counts) == 0, -np.inf, key)
+    return key
+
+
+def dense_rank(metric: str, values, counts=None) -> np.ndarray:
+    """R: rank 0 = most outlying; equal keys share a rank; ranks are consecutive."""
+    key = outlyingness_key(metric, values, counts)
+    uniq = np.unique(key)                      # ascending distinct keys
+    return np.searchsorted(uniq, key).astype(np.int64)
+
+
+def topn_ids(metric: str, values, n: int, counts=None) -> np.ndarray:
+    """The n most outlying object ids: stable sort by (key, id) (reading A15)."""
+    key = outlyingness_key(metric, values, counts)
+    order = np.lexsort((np.arange(len(key)), key))
+    return order[:n]
+
+
+def overlap_fraction(ids_a, ids_b, n: int) -> float:
+    """Eq. 2: f = |R^A ∩ R^B| / n over the two top-n sets."""
+    return len(set(np.asarray(ids_a).tolist()) & set(np.asarray(ids_b).tolist())) / float(n)
+
+
+def similarity_curves(topn_sets, n: int):
+    """U_min[j] = f(top-n of grid point 0, of grid point j); U_max[j] = f(last, j)."""
+    g = len(topn_sets)
+    u_min = np.array([overlap_fraction(topn_sets[0], topn_sets[j], n) for j in range(g)])
+    u_max = np.array([overlap_fraction(topn_sets[g - 1], topn_sets[j], n) for j in range(g)])
+    return u_min, u_max
+
+
+def select_parameter(u_min, u_max) -> int:
+    """Eq. 3: argmin_j |U_min[j] - U_max[j]| (first minimiser)."""
+    return int(np.argmin(np.abs(np.asarray(u_min) - np.asarray(u_max))))
+
+
+def knn_scores_at_k(idx_kmax, dist_kmax, kj: int, N: int):
+    """Scores for k_j from the k_max lists: the first k_j columns.
+    idx/dist: [N][k_max] of one mask.  -> (kth, mean, indeg)."""
+    idx = np.asarray(idx_kmax)[:, :kj]
+    dist = np.asarray(dist_kmax, dtype=np.float64)[:, :kj]
+    return dist[:, -1], dist.mean(axis=1), np.bincount(idx.ravel(), minlength=N)

@@ -14,6 +14,7 @@ NVCC_FLAGS = [
     # main loop and the rare paths round identically
     "-fmad=false",
     "-Xcompiler", "-fPIC", "-shared",
+    "-diag-suppress", "177",   # phase-clock variables that only the developer stats build reads
 ]
 
 

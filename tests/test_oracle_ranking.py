@@ -1,0 +1,52 @@
+"""Pins for oracle/ranking.py against the paper's own worked examples (NEXT-1)."""
+import os
+
+import numpy as np
+
+from oracle import ranking
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _table2():
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "table2_paper.txt"))
+            if l.strip() and not l.startswith("#")]
+    a = np.array(rows, dtype=np.float64)
+    # point, dssj_count, rank, dssj_mean, rank, knn_indeg, rank, knn_mean, rank
+    return a
+
+
+def test_table2_ranks_from_table2_metrics():
+    # PAPER.md:282-295 Table 2: every rank column follows from its metric column
+    t = _table2()
+    cnt, cnt_r, mean, mean_r, indeg, indeg_r, kmean, kmean_r = (t[:, i] for i in range(1, 9))
+    assert ranking.dense_rank("dssj_count", cnt).tolist() == cnt_r.astype(int).tolist()
+    assert ranking.dense_rank("dssj_mean", mean, counts=cnt).tolist() == mean_r.astype(int).tolist()
+    assert ranking.dense_rank("knn_indegree", indeg).tolist() == indeg_r.astype(int).tolist()
+    assert ranking.dense_rank("knn_mean", kmean).tolist() == kmean_r.astype(int).tolist()
+    # point 10 is the only one with rank 0 in all four
+    all0 = (cnt_r == 0) & (mean_r == 0) & (indeg_r == 0) & (kmean_r == 0)
+    assert t[all0, 0].tolist() == [10.0]
+
+
+def test_section_352_worked_example():
+    rec = {}
+    for l in open(os.path.join(HERE, "golden", "section352_example.txt")):
+        if l.strip() and not l.startswith("#"):
+            p = l.split()
+            rec[p[0]] = [float(x) for x in p[1:]]
+    sets = [np.array(rec[k], dtype=np.int64) for k in ("eps_1", "eps_2", "eps_3")]
+    u_min, u_max = ranking.similarity_curves(sets, 10)
+    assert u_min.tolist() == rec["U_min"] and u_max.tolist() == rec["U_max"]
+    # Eq. 3: |U_min - U_max| = {0.8, 0.1, 0.8} -> the middle grid point is selected
+    assert ranking.select_parameter(u_min, u_max) == 1
+
+
+def test_topn_and_ties():
+    v = np.array([3, 1, 1, 0, 2, 1])
+    assert ranking.dense_rank("dssj_count", v).tolist() == [3, 1, 1, 0, 2, 1]
+    assert ranking.topn_ids("dssj_count", v, 3).tolist() == [3, 1, 2]          # ties -> smaller id
+    assert ranking.topn_ids("knn_mean", v.astype(float), 2).tolist() == [0, 4]  # largest first
+    kth, mean, indeg = ranking.knn_scores_at_k(np.array([[1, 2, 0], [0, 2, 1], [1, 0, 2]])[:, :3],
+                                               np.array([[1., 2., 3.], [1., 1., 4.], [2., 2., 2.]]), 2, 3)
+    assert kth.tolist() == [2., 1., 2.] and mean.tolist() == [1.5, 1., 2.] and indeg.tolist() == [2, 2, 2]
