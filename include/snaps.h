@@ -180,6 +180,56 @@ snaps_status snaps_knn_selfjoin_streamed(const float *d_X, int64_t N, int n_feat
 snaps_status snaps_probe_fp32_rate(int kind, double *h_lane_ops_per_s, void *stream);
 
 /*
+ * ---- NEXT-1 (PAPER.md sections 3.4, 3.5.2, 3.6): ranking and parameter selection ----
+ *
+ * Metric kinds: which end of a score is outlying.
+ */
+#define SNAPS_METRIC_DSSJ_COUNT 0   /* uint32 counts, fewest neighbours = most outlying */
+#define SNAPS_METRIC_DSSJ_MEAN 1    /* fp32 mean eps-distance, largest = most outlying; objects
+                                       with count 0 rank first; needs d_counts */
+#define SNAPS_METRIC_KNN_INDEGREE 2 /* int32 in-degree, lowest = most outlying */
+#define SNAPS_METRIC_KNN_MEAN 3     /* fp32 mean (or k-th) kNN distance, largest = most outlying */
+
+/* Device scratch snaps_rank_scores needs for n_rows score rows of N objects. */
+size_t snaps_rank_workspace_bytes(int64_t N, int n_rows);
+
+/*
+ * Ranking function R (Table 2): for each of n_rows rows of N
+ * scores, out_rank[row][i] = dense rank of object i, 0 = most outlying, equal scores share a
+ * rank; out_order[row][p] = id of the p-th most outlying object, ties in increasing id order
+ * (the "top-n" of Eq. 2 is its first n entries, reading A15).  d_values: device,
+ * [n_rows][N], uint32 / fp32 / int32 per metric kind (scores are non-negative); d_counts:
+ * device [n_rows][N], only for SNAPS_METRIC_DSSJ_MEAN.  Either output may be NULL.
+ */
+snaps_status snaps_rank_scores(int metric, const void *d_values, const uint32_t *d_counts,
+                               int64_t N, int n_rows, int32_t *out_rank, int32_t *out_order,
+                               void *d_workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Eq. 2: out_f[row] = |top-n(A[row]) ∩ top-n(B[row])| / n, from two
+ * out_order arrays ([n_rows][N] each, device).  1 <= n <= N.
+ */
+snaps_status snaps_topn_overlap(const int32_t *d_order_a, const int32_t *d_order_b, int64_t N,
+                                int n_rows, int n, float *out_f, void *stream);
+
+/*
+ * Eq. 3: out_j[row] = the first j in 0..G-1 that minimises
+ * |U_min[j][row] - U_max[j][row]|.  d_u_min, d_u_max: device, [G][n_rows] fp32.
+ */
+snaps_status snaps_select_parameter(const float *d_u_min, const float *d_u_max, int G, int n_rows,
+                                    int32_t *out_j, void *stream);
+
+/*
+ * k grid: scores for k_j <= k_max from lists computed once for k_max (their
+ * first k_j entries).  knn_idx/knn_dist: [n_masks][N][k_max] as written by
+ * snaps_knn_selfjoin; outputs [n_masks][N], any may be NULL; out_indeg is zeroed here.
+ */
+snaps_status snaps_knn_scores_at_k(int64_t N, int n_masks, int k_max, int k_j,
+                                   const int32_t *knn_idx, const float *knn_dist,
+                                   float *out_kth, float *out_mean, int32_t *out_indeg,
+                                   void *stream);
+
+/*
  * Kernel timing for roofline reports.  While enabled,
  * every join call records a CUDA event pair on `stream` around each launch of
  * its dominant (join) kernel; the pairs of the most recent call are kept.

@@ -13,6 +13,8 @@ EXPORTED_SYMBOLS = [
     "snaps_knn_selfjoin", "snaps_range_selfjoin", "snaps_outlier_scores",
     "snaps_stream_ring_bytes", "snaps_knn_selfjoin_streamed", "snaps_probe_fp32_rate",
     "snaps_profile_enable", "snaps_profile_last_kernel_ms",
+    "snaps_rank_workspace_bytes", "snaps_rank_scores", "snaps_topn_overlap", "snaps_select_parameter",
+    "snaps_knn_scores_at_k",
 ]
 
 _lib = None
@@ -59,6 +61,16 @@ def lib():
         L.snaps_profile_last_kernel_ms.restype = i32
         L.snaps_profile_last_kernel_ms.argtypes = [ctypes.POINTER(ctypes.c_float),
                                                    ctypes.POINTER(ctypes.c_int)]
+        L.snaps_rank_workspace_bytes.restype = sz
+        L.snaps_rank_workspace_bytes.argtypes = [i64, i32]
+        L.snaps_rank_scores.restype = i32
+        L.snaps_rank_scores.argtypes = [i32, vp, vp, i64, i32, vp, vp, vp, sz, vp]
+        L.snaps_topn_overlap.restype = i32
+        L.snaps_topn_overlap.argtypes = [vp, vp, i64, i32, i32, vp, vp]
+        L.snaps_select_parameter.restype = i32
+        L.snaps_select_parameter.argtypes = [vp, vp, i32, i32, vp, vp]
+        L.snaps_knn_scores_at_k.restype = i32
+        L.snaps_knn_scores_at_k.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -249,3 +261,55 @@ def profile_last_kernel_ms():
     ms, n = ctypes.c_float(0.0), ctypes.c_int(0)
     _check(lib().snaps_profile_last_kernel_ms(ctypes.byref(ms), ctypes.byref(n)))
     return float(ms.value), int(n.value)
+
+
+METRIC_KINDS = {"dssj_count": 0, "dssj_mean": 1, "knn_indegree": 2, "knn_mean": 3, "knn_kth": 3}
+
+
+def rank_scores(metric: str, values, counts=None, *, ranks=True, order=True, stream=None):
+    """snaps_rank_scores on a CUDA tensor values [n_rows, N] -> dict rank / order (int32)."""
+    import torch
+    assert values.is_cuda and values.dim() == 2 and values.is_contiguous()
+    n_rows, N = values.shape
+    out = {}
+    if ranks:
+        out["rank"] = torch.empty((n_rows, N), dtype=torch.int32, device=values.device)
+    if order:
+        out["order"] = torch.empty((n_rows, N), dtype=torch.int32, device=values.device)
+    ws = torch.empty(int(lib().snaps_rank_workspace_bytes(N, n_rows)), dtype=torch.uint8, device=values.device)
+    _check(lib().snaps_rank_scores(METRIC_KINDS[metric], _dptr(values), _dptr(counts), N, n_rows,
+                                   _dptr(out.get("rank")), _dptr(out.get("order")), _dptr(ws), ws.numel(),
+                                   _stream(stream)))
+    out["_workspace"] = ws
+    return out
+
+
+def topn_overlap(order_a, order_b, n: int, stream=None):
+    """snaps_topn_overlap (Eq. 2) -> fp32 tensor [n_rows]."""
+    import torch
+    n_rows, N = order_a.shape
+    f = torch.empty(n_rows, dtype=torch.float32, device=order_a.device)
+    _check(lib().snaps_topn_overlap(_dptr(order_a), _dptr(order_b), N, n_rows, n, _dptr(f), _stream(stream)))
+    return f
+
+
+def select_parameter(u_min, u_max, stream=None):
+    """snaps_select_parameter (Eq. 3): u_* [G, n_rows] fp32 -> int32 [n_rows]."""
+    import torch
+    G, n_rows = u_min.shape
+    j = torch.empty(n_rows, dtype=torch.int32, device=u_min.device)
+    _check(lib().snaps_select_parameter(_dptr(u_min), _dptr(u_max), G, n_rows, _dptr(j), _stream(stream)))
+    return j
+
+
+def knn_scores_at_k(knn_idx, knn_dist, k_j: int, stream=None):
+    """snaps_knn_scores_at_k: lists [n_masks, N, k_max] -> dict kth / mean / indeg for k_j."""
+    import torch
+    n_masks, N, k_max = knn_dist.shape
+    dev = knn_dist.device
+    out = {"kth": torch.empty((n_masks, N), dtype=torch.float32, device=dev),
+           "mean": torch.empty((n_masks, N), dtype=torch.float32, device=dev),
+           "indeg": torch.empty((n_masks, N), dtype=torch.int32, device=dev)}
+    _check(lib().snaps_knn_scores_at_k(N, n_masks, k_max, k_j, _dptr(knn_idx), _dptr(knn_dist),
+                                       _dptr(out["kth"]), _dptr(out["mean"]), _dptr(out["indeg"]), _stream(stream)))
+    return out

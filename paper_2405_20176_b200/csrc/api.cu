@@ -17,6 +17,7 @@
 #include "misc_kernels.cuh"
 #include "pivot_sort.cuh"
 #include "range_lattice.cuh"
+#include "ranking.cuh"
 
 namespace {
 
@@ -561,6 +562,56 @@ snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat
     }
     cudaStreamDestroy(side);
     return result;
+}
+
+size_t snaps_rank_workspace_bytes(int64_t N, int n_rows) {
+    if (N < 1 || n_rows < 1) return 0;
+    return snaps::rank_workspace_bytes(N, n_rows);
+}
+
+snaps_status snaps_rank_scores(int metric, const void* d_values, const uint32_t* d_counts, int64_t N,
+                               int n_rows, int32_t* out_rank, int32_t* out_order, void* d_workspace,
+                               size_t workspace_bytes, void* stream) {
+    if (metric < 0 || metric > 3) return fail(SNAPS_INVALID_ARG, "metric kind %d outside 0..3", metric);
+    if (!d_values || N < 1 || n_rows < 1) return fail(SNAPS_INVALID_ARG, "bad sizes or NULL values");
+    if (N > (int64_t)1 << 30) return fail(SNAPS_UNSUPPORTED, "N = %lld > 2^30", (long long)N);
+    if (metric == SNAPS_METRIC_DSSJ_MEAN && !d_counts) return fail(SNAPS_INVALID_ARG, "d_counts is NULL");
+    if (!out_rank && !out_order) return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
+    if (!d_workspace || workspace_bytes < snaps::rank_workspace_bytes(N, n_rows))
+        return fail(SNAPS_WORKSPACE_TOO_SMALL, "rank workspace %zu < %zu bytes", workspace_bytes,
+                    snaps::rank_workspace_bytes(N, n_rows));
+    CUDA_TRY(snaps::rank_launch(metric, d_values, d_counts, N, n_rows, out_rank, out_order, d_workspace,
+                                workspace_bytes, static_cast<cudaStream_t>(stream)));
+    return SNAPS_OK;
+}
+
+snaps_status snaps_topn_overlap(const int32_t* d_order_a, const int32_t* d_order_b, int64_t N, int n_rows,
+                                int n, float* out_f, void* stream) {
+    if (!d_order_a || !d_order_b || !out_f) return fail(SNAPS_INVALID_ARG, "NULL argument");
+    if (N < 1 || n_rows < 1 || n < 1 || n > N) return fail(SNAPS_INVALID_ARG, "bad sizes (n = %d, N = %lld)", n, (long long)N);
+    if ((N + 31) / 32 * 4 > 200 * 1024) return fail(SNAPS_UNSUPPORTED, "N = %lld: bitmap exceeds shared memory", (long long)N);
+    CUDA_TRY(snaps::topn_overlap_launch(d_order_a, d_order_b, N, n_rows, n, out_f, static_cast<cudaStream_t>(stream)));
+    return SNAPS_OK;
+}
+
+snaps_status snaps_select_parameter(const float* d_u_min, const float* d_u_max, int G, int n_rows,
+                                    int32_t* out_j, void* stream) {
+    if (!d_u_min || !d_u_max || !out_j || G < 1 || n_rows < 1) return fail(SNAPS_INVALID_ARG, "bad arguments");
+    CUDA_TRY(snaps::select_launch(d_u_min, d_u_max, G, n_rows, out_j, static_cast<cudaStream_t>(stream)));
+    return SNAPS_OK;
+}
+
+snaps_status snaps_knn_scores_at_k(int64_t N, int n_masks, int k_max, int k_j, const int32_t* knn_idx,
+                                   const float* knn_dist, float* out_kth, float* out_mean,
+                                   int32_t* out_indeg, void* stream) {
+    if (N < 2 || n_masks < 1 || k_max < 1 || k_j < 1 || k_j > k_max) return fail(SNAPS_INVALID_ARG, "bad sizes");
+    if ((out_kth || out_mean) && !knn_dist) return fail(SNAPS_INVALID_ARG, "knn_dist is NULL");
+    if (out_indeg && !knn_idx) return fail(SNAPS_INVALID_ARG, "knn_idx is NULL");
+    if (!out_kth && !out_mean && !out_indeg) return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (out_indeg) CUDA_TRY(cudaMemsetAsync(out_indeg, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, st));
+    CUDA_TRY(snaps::scores_at_k_launch(N, n_masks, k_max, k_j, knn_idx, knn_dist, out_kth, out_mean, out_indeg, st));
+    return SNAPS_OK;
 }
 
 snaps_status snaps_profile_enable(int on) {

@@ -1,0 +1,119 @@
+"""GPU parity for NEXT-1 (ranking, top-n overlap, parameter selection, k-grid scores) against
+oracle/ranking.py -- integer / index work: bit-exact on the same score arrays."""
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+from oracle import ranking as oracle_ranking
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.fixture(scope="module")
+def snaps():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2405_20176_b200 as s
+    s.lib()
+    return s
+
+
+def _t(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def test_table2_ranks_on_device(snaps):
+    import torch
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "table2_paper.txt"))
+            if l.strip() and not l.startswith("#")]
+    t = np.array(rows, dtype=np.float64)
+    cnt = t[:, 1].astype(np.uint32)
+    cases = [("dssj_count", cnt.view(np.int32), None, t[:, 2]),
+             ("dssj_mean", t[:, 3].astype(np.float32), cnt.view(np.int32), t[:, 4]),
+             ("knn_indegree", t[:, 5].astype(np.int32), None, t[:, 6]),
+             ("knn_mean", t[:, 7].astype(np.float32), None, t[:, 8])]
+    for metric, vals, counts, want in cases:
+        out = snaps.rank_scores(metric, _t(vals[None, :]), None if counts is None else _t(counts[None, :]))
+        torch.cuda.synchronize()
+        assert out["rank"][0].cpu().numpy().tolist() == want.astype(int).tolist(), metric
+
+
+@pytest.mark.parametrize("metric", ["dssj_count", "dssj_mean", "knn_indegree", "knn_mean"])
+@pytest.mark.parametrize("n_rows,N", [(1, 1), (3, 257), (7, 5000), (2, 31693)])
+def test_rank_and_order_match_oracle(snaps, metric, n_rows, N):
+    import torch
+    rng = np.random.default_rng(N + n_rows)
+    counts = None
+    if metric in ("dssj_count", "knn_indegree"):
+        vals = rng.integers(0, max(2, N // 20), (n_rows, N)).astype(np.int32)      # many ties
+    else:
+        vals = np.round(rng.random((n_rows, N)) * 50).astype(np.float32) / 50        # ties too
+        if metric == "dssj_mean":
+            counts = rng.integers(0, 4, (n_rows, N)).astype(np.int32)
+            vals[counts == 0] = 0.0                                                  # reading A6
+    out = snaps.rank_scores(metric, _t(vals), None if counts is None else _t(counts))
+    torch.cuda.synchronize()
+    for r in range(n_rows):
+        c = None if counts is None else counts[r]
+        assert (out["rank"][r].cpu().numpy() == oracle_ranking.dense_rank(metric, vals[r], c)).all()
+        assert (out["order"][r].cpu().numpy() == oracle_ranking.topn_ids(metric, vals[r], N, c)).all()
+
+
+def test_overlap_and_selection_worked_example(snaps):
+    # the section 3.5.2 example through the device kernels
+    import torch
+    rec = {}
+    for l in open(os.path.join(HERE, "golden", "section352_example.txt")):
+        if l.strip() and not l.startswith("#"):
+            p = l.split()
+            rec[p[0]] = [float(x) for x in p[1:]]
+    N, n = 128, 10
+    orders = []
+    for k in ("eps_1", "eps_2", "eps_3"):
+        top = np.array(rec[k], dtype=np.int32)
+        rest = np.setdiff1d(np.arange(N, dtype=np.int32), top)
+        orders.append(_t(np.concatenate([top, rest])[None, :]))
+    u_min = torch.stack([snaps.topn_overlap(orders[0], o, n) for o in orders])
+    u_max = torch.stack([snaps.topn_overlap(orders[2], o, n) for o in orders])
+    j = snaps.select_parameter(u_min.contiguous(), u_max.contiguous())
+    torch.cuda.synchronize()
+    assert np.allclose(u_min[:, 0].cpu().numpy(), rec["U_min"]) and np.allclose(u_max[:, 0].cpu().numpy(), rec["U_max"])
+    assert int(j[0]) == 1
+
+
+def test_k_grid_pipeline_matches_oracle(snaps):
+    """k_max join once, then every k_j of a grid from its prefix, ranking, Eq. 2 and
+    Eq. 3 -- device against the oracle functions on the same lists."""
+    import torch
+    N, k_max, n = 3000, 32, 30                      # n = 1% of N
+    X = workloads.make_table(N, 17, outlier_frac=0.01)
+    masks = workloads.all_masks(15)[::2111]
+    join = snaps.knn_selfjoin(_t(X), masks, k_max, scores=False)
+    torch.cuda.synchronize()
+    idx, dist = join["idx"].cpu().numpy(), join["dist"].cpu().numpy()
+    grid = [2, 3, 5, 8, 12, 20, 32]
+    for metric, key in (("knn_indegree", "indeg"), ("knn_mean", "mean")):
+        orders = []
+        for kj in grid:
+            sc = snaps.knn_scores_at_k(join["idx"], join["dist"], kj)
+            torch.cuda.synchronize()
+            for m in range(len(masks)):
+                kth, mean, indeg = oracle_ranking.knn_scores_at_k(idx[m], dist[m], kj, N)
+                assert (sc["indeg"][m].cpu().numpy() == indeg).all()
+                assert np.allclose(sc["kth"][m].cpu().numpy(), kth, rtol=1e-6)
+                assert np.allclose(sc["mean"][m].cpu().numpy(), mean, rtol=1e-5)
+            orders.append(snaps.rank_scores(metric, sc[key].contiguous(), ranks=False)["order"])
+        u_min = torch.stack([snaps.topn_overlap(orders[0], o, n) for o in orders]).contiguous()
+        u_max = torch.stack([snaps.topn_overlap(orders[-1], o, n) for o in orders]).contiguous()
+        sel = snaps.select_parameter(u_min, u_max)
+        torch.cuda.synchronize()
+        for m in range(len(masks)):
+            tops = [o[m, :n].cpu().numpy() for o in orders]
+            o_min, o_max = oracle_ranking.similarity_curves(tops, n)
+            assert np.allclose(u_min[:, m].cpu().numpy(), o_min) and np.allclose(u_max[:, m].cpu().numpy(), o_max)
+            assert int(sel[m]) == oracle_ranking.select_parameter(o_min, o_max)
+        assert float(u_min[0].min()) == 1.0 and float(u_max[-1].min()) == 1.0     # a set against itself
