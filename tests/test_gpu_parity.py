@@ -389,3 +389,20 @@ def test_pivot_sweep_range_join(snaps, oracle_mod, force_sweep, n, nf, seed):
     lo, hi = check_range(out["count"].cpu().numpy(), out["sumdist"].cpu().numpy(), out["mean"].cpu().numpy(),
                          oracle_mod, X, masks, eps)
     assert (lo == hi).mean() > 0.99
+
+
+def test_eps_grid_by_repeating_masks(snaps, oracle_mod):
+    """The eps grid of PAPER.md:181 through the existing entry point: a mask listed once per radius.
+    Result sets are nested, A(eps_1) within A(eps_2) within A(eps_3) (Fig. 3)."""
+    import torch
+    X = workloads.make_table(1500, 23, outlier_frac=0.01)
+    base = np.array([0b11, 0x7FFF, (1 << 7) | (1 << 2) | 1, 0b111100], dtype=np.uint16)
+    grid = np.array([0.02, 0.05, 0.11], dtype=np.float32)
+    masks = np.repeat(base, len(grid))
+    eps = np.tile(grid, len(base)) * np.repeat(np.array([1.0, 6.0, 2.0, 3.0], dtype=np.float32), len(grid))
+    out = snaps.range_selfjoin(_dev(X), masks, eps)
+    torch.cuda.synchronize()
+    cnt = out["count"].cpu().numpy()
+    check_range(cnt, out["sumdist"].cpu().numpy(), out["mean"].cpu().numpy(), oracle_mod, X, masks, eps)
+    c = cnt.reshape(len(base), len(grid), -1)
+    assert (np.diff(c, axis=1) >= 0).all() and (c[:, -1] > c[:, 0]).any()
