@@ -230,6 +230,22 @@ snaps_status snaps_knn_scores_at_k(int64_t N, int n_masks, int k_max, int k_j,
                                    void *stream);
 
 /*
+ * DSSJ for a grid of radii in ONE scan (Fig. 3: "we execute DSSJ once for
+ * eps_max and use this result set to derive the result sets for all eps_i in G").
+ *   h_eps_grid  host, [n_masks][G] fp32, per mask strictly ascending, finite, > 0; 1 <= G <= 32
+ *   out_count   device, [n_masks][G][N] uint32: neighbours within eps_g (self excluded)
+ *   out_sumdist, out_mean  device, same shape, fp32; may be NULL (mean = 0 when count = 0)
+ * Workspace: snaps_range_grid_workspace_bytes(N, n_feat, n_masks, G).
+ */
+size_t snaps_range_grid_workspace_bytes(int64_t N, int n_feat, int n_masks, int G);
+
+snaps_status snaps_range_selfjoin_grid(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                       const uint16_t *h_masks, int n_masks,
+                                       const float *h_eps_grid, int G, uint32_t *out_count,
+                                       float *out_sumdist, float *out_mean, void *d_workspace,
+                                       size_t workspace_bytes, void *stream);
+
+/*
  * Kernel timing for roofline reports.  While enabled,
  * every join call records a CUDA event pair on `stream` around each launch of
  * its dominant (join) kernel; the pairs of the most recent call are kept.

@@ -14,7 +14,7 @@ EXPORTED_SYMBOLS = [
     "snaps_stream_ring_bytes", "snaps_knn_selfjoin_streamed", "snaps_probe_fp32_rate",
     "snaps_profile_enable", "snaps_profile_last_kernel_ms",
     "snaps_rank_workspace_bytes", "snaps_rank_scores", "snaps_topn_overlap", "snaps_select_parameter",
-    "snaps_knn_scores_at_k",
+    "snaps_knn_scores_at_k", "snaps_range_grid_workspace_bytes", "snaps_range_selfjoin_grid",
 ]
 
 _lib = None
@@ -69,6 +69,10 @@ def lib():
         L.snaps_topn_overlap.argtypes = [vp, vp, i64, i32, i32, vp, vp]
         L.snaps_select_parameter.restype = i32
         L.snaps_select_parameter.argtypes = [vp, vp, i32, i32, vp, vp]
+        L.snaps_range_grid_workspace_bytes.restype = sz
+        L.snaps_range_grid_workspace_bytes.argtypes = [i64, i32, i32, i32]
+        L.snaps_range_selfjoin_grid.restype = i32
+        L.snaps_range_selfjoin_grid.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, vp, vp, vp, sz, vp]
         L.snaps_knn_scores_at_k.restype = i32
         L.snaps_knn_scores_at_k.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         _lib = L
@@ -312,4 +316,31 @@ def knn_scores_at_k(knn_idx, knn_dist, k_j: int, stream=None):
            "indeg": torch.empty((n_masks, N), dtype=torch.int32, device=dev)}
     _check(lib().snaps_knn_scores_at_k(N, n_masks, k_max, k_j, _dptr(knn_idx), _dptr(knn_dist),
                                        _dptr(out["kth"]), _dptr(out["mean"]), _dptr(out["indeg"]), _stream(stream)))
+    return out
+
+
+def range_selfjoin_grid(X, masks, eps_grid, *, sums=True, stream=None):
+    """snaps_range_selfjoin_grid: eps_grid [n_masks, G] ascending per mask -> dict count / sumdist /
+    mean, each [n_masks, G, N]."""
+    import torch
+    assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
+    m = _masks(masks)
+    e = np.ascontiguousarray(np.asarray(eps_grid, dtype=np.float32))
+    assert e.ndim == 2 and e.shape[0] == len(m)
+    G = e.shape[1]
+    N, n_feat = X.shape
+    dev = X.device
+    out = {"count": torch.empty((len(m), G, N), dtype=torch.int32, device=dev)}
+    if sums:
+        out["sumdist"] = torch.empty((len(m), G, N), dtype=torch.float32, device=dev)
+        out["mean"] = torch.empty((len(m), G, N), dtype=torch.float32, device=dev)
+    nbytes = int(lib().snaps_range_grid_workspace_bytes(N, n_feat, len(m), G))
+    if nbytes == 0:
+        raise SnapsError(1, "invalid sizes for the radius-grid workspace")
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    _check(lib().snaps_range_selfjoin_grid(
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
+        e.ctypes.data_as(ctypes.c_void_p), G, _dptr(out["count"]), _dptr(out.get("sumdist")),
+        _dptr(out.get("mean")), _dptr(ws), ws.numel(), _stream(stream)))
+    out["_workspace"] = ws
     return out

@@ -16,6 +16,7 @@
 #include "knn_lattice.cuh"
 #include "misc_kernels.cuh"
 #include "pivot_sort.cuh"
+#include "range_grid.cuh"
 #include "range_lattice.cuh"
 #include "ranking.cuh"
 
@@ -562,6 +563,70 @@ snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat
     }
     cudaStreamDestroy(side);
     return result;
+}
+
+size_t snaps_range_grid_workspace_bytes(int64_t N, int n_feat, int n_masks, int G) {
+    if (N < 2 || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES || n_masks < 1 || G < 1 || G > snaps::kRangeGridMaxRadii)
+        return 0;
+    return base_workspace_bytes(N, n_masks, 0) + align_up(static_cast<size_t>(n_masks) * G * 4, 256);
+}
+
+snaps_status snaps_range_selfjoin_grid(const float* d_X, int64_t N, int n_feat, int64_t ld,
+                                       const uint16_t* h_masks, int n_masks, const float* h_eps_grid, int G,
+                                       uint32_t* out_count, float* out_sumdist, float* out_mean,
+                                       void* d_workspace, size_t workspace_bytes, void* stream) {
+    prof_reset();
+    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    if (rc) return rc;
+    if (!h_eps_grid || !out_count) return fail(SNAPS_INVALID_ARG, "NULL eps grid or out_count");
+    if (G < 1 || G > snaps::kRangeGridMaxRadii) return fail(SNAPS_INVALID_ARG, "G = %d outside 1..%d", G, snaps::kRangeGridMaxRadii);
+    std::vector<float> thr(static_cast<size_t>(n_masks) * G);
+    for (int m = 0; m < n_masks; ++m)
+        for (int g = 0; g < G; ++g) {
+            const float e = h_eps_grid[static_cast<size_t>(m) * G + g];
+            if (!(e > 0.f) || !isfinite(e) || (g > 0 && !(e > h_eps_grid[static_cast<size_t>(m) * G + g - 1])))
+                return fail(SNAPS_INVALID_ARG, "eps_grid[%d][%d] = %g: radii must be finite, > 0 and ascending", m, g, (double)e);
+            const float e2 = static_cast<float>(static_cast<double>(e) * static_cast<double>(e));
+            thr[static_cast<size_t>(m) * G + g] = nextafterf(e2, INFINITY);   // closed ball, reading A2
+        }
+    Workspace w;
+    rc = carve(d_workspace, workspace_bytes, N, n_masks, 0, &w);
+    if (rc) return rc;
+    const size_t grid_bytes = align_up(static_cast<size_t>(n_masks) * G * 4, 256);
+    if (w.ring_bytes < grid_bytes)
+        return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace lacks %zu bytes for the radius grid", grid_bytes);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    std::vector<snaps::BatchDesc> batches;
+    plan_lattice(h_masks, n_masks, nullptr, &batches);
+    const int nb = static_cast<int>(batches.size());
+    CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
+                                       n_tiles_for(N) * snaps::kTileRows, st));
+    CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
+    CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * nb, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(w.ring, thr.data(), thr.size() * 4, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaStreamSynchronize(st));   // thr is a host temporary: the copy must land before it goes away
+    CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
+    snaps::RangeGridParams p;
+    p.Xp = w.Xp;
+    p.Xb = w.Xb;
+    p.n_blocks = n_blocks_for(N);
+    p.N = static_cast<int>(N);
+    p.G = G;
+    p.batches = w.batches;
+    p.n_batches = nb;
+    p.thr_grid = reinterpret_cast<const float*>(w.ring);
+    p.warps = snaps::kRangeGridMaxThreads / 32;
+    while (p.warps > 1 && snaps::range_grid_smem_bytes(G, p.warps) > 227 * 1024) --p.warps;
+    p.work_counter = reinterpret_cast<unsigned long long*>(w.counter);
+    p.out_count = out_count;
+    p.out_sum = out_sumdist;
+    p.out_mean = out_mean;
+    const int64_t items = N * nb;
+    const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
+    const bool prof = prof_begin(st);
+    CUDA_TRY(snaps::range_grid_launch(p, grid, st));
+    prof_end(prof, st);
+    return SNAPS_OK;
 }
 
 size_t snaps_rank_workspace_bytes(int64_t N, int n_rows) {

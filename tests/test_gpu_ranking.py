@@ -117,3 +117,31 @@ def test_k_grid_pipeline_matches_oracle(snaps):
             assert np.allclose(u_min[:, m].cpu().numpy(), o_min) and np.allclose(u_max[:, m].cpu().numpy(), o_max)
             assert int(sel[m]) == oracle_ranking.select_parameter(o_min, o_max)
         assert float(u_min[0].min()) == 1.0 and float(u_max[-1].min()) == 1.0     # a set against itself
+
+
+def test_radius_grid_single_scan_matches_oracle_per_radius(snaps):
+    """PAPER.md:235-239 (Fig. 3): one join at eps_max gives the result for every eps_j of the grid.
+    The oracle is the definition evaluated once per radius (no shared work)."""
+    import sys
+    import torch
+    sys.path.insert(0, HERE)
+    from parity import check_range
+    import oracle as oracle_mod
+    X = workloads.make_table(1500, 29, outlier_frac=0.01)
+    masks = np.array([0b11, 0x7FFF, (1 << 7) | (1 << 2) | 1, 0b111100, (1 << 14) | (1 << 9)], dtype=np.uint16)
+    scale = np.array([1.0, 6.0, 2.0, 3.0, 1.5], dtype=np.float32)
+    G = 7
+    grid = (np.linspace(0.015, 0.12, G, dtype=np.float32)[None, :] * scale[:, None]).astype(np.float32)
+    out = snaps.range_selfjoin_grid(_t(X), masks, grid)
+    torch.cuda.synchronize()
+    cnt = out["count"].cpu().numpy()
+    for g in range(G):
+        check_range(cnt[:, g], out["sumdist"][:, g].cpu().numpy(), out["mean"][:, g].cpu().numpy(),
+                    oracle_mod, X, masks, grid[:, g])
+    assert (np.diff(cnt, axis=1) >= 0).all()                      # nested result sets
+    # the single-radius entry point gives the same counts
+    one = snaps.range_selfjoin(_t(X), masks, grid[:, 3])
+    torch.cuda.synchronize()
+    assert (one["count"].cpu().numpy() == cnt[:, 3]).all()
+    with pytest.raises(snaps.SnapsError):
+        snaps.range_selfjoin_grid(_t(X), masks, grid[:, ::-1].copy())   # not ascending
