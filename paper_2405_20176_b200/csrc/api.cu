@@ -97,6 +97,8 @@ void plan_lattice(const uint16_t* masks, int n_masks, const float* thr,
             snaps::BatchDesc d;
             d.hmask = H;
             d.n_valid = 0;
+            d.pivot = (H >> snaps::kLow) ? snaps::kLow + __builtin_ctz(H >> snaps::kLow) : -1;
+            d.pad_ = 0;
             for (int t = 0; t < snaps::kLat; ++t) {
                 d.slot[t] = -1;
                 d.thr[t] = -1.f;
@@ -114,6 +116,37 @@ void plan_lattice(const uint16_t* masks, int n_masks, const float* thr,
     for (auto& kv : by_h)
         for (int bi : kv.second) ordered.push_back(B[bi]);
     B.swap(ordered);
+}
+
+// Pivot sweep only: a batch without high features has no pivot and would take a full pass.  Split
+// it by lattice feature instead -- the masks that contain feature 0, then of the rest those that
+// contain feature 1, ... -- so that every piece has a feature all its masks share (its pivot).
+void split_for_sweep(std::vector<snaps::BatchDesc>* batches) {
+    std::vector<snaps::BatchDesc> out;
+    for (const snaps::BatchDesc& b : *batches) {
+        if (b.pivot >= 0) {
+            out.push_back(b);
+            continue;
+        }
+        bool taken[snaps::kLat] = {false};
+        for (int f = 0; f < snaps::kLow; ++f) {
+            snaps::BatchDesc d = b;
+            d.n_valid = 0;
+            d.pivot = f;
+            for (int t = 0; t < snaps::kLat; ++t) {
+                const bool mine = b.slot[t] >= 0 && !taken[t] && ((t >> f) & 1);
+                if (mine) {
+                    taken[t] = true;
+                    d.n_valid += 1;
+                } else {
+                    d.slot[t] = -1;
+                    d.thr[t] = -1.f;
+                }
+            }
+            if (d.n_valid > 0) out.push_back(d);
+        }
+    }
+    batches->swap(out);
 }
 
 snaps_status check_common(const float* d_X, int64_t N, int n_feat, int64_t ld,
@@ -161,7 +194,7 @@ size_t pivot_set_bytes(int64_t N) {
 }
 
 size_t pivot_region_bytes(int64_t N) {
-    return 9 * pivot_set_bytes(N) + align_up(snaps::pivot_sort_temp_bytes(n_blocks_for(N) * 32), 256);
+    return 15 * pivot_set_bytes(N) + align_up(snaps::pivot_sort_temp_bytes(n_blocks_for(N) * 32), 256);
 }
 
 size_t base_workspace_bytes(int64_t N, int n_masks, int k) {
@@ -193,7 +226,7 @@ snaps_status carve(void* d_ws, size_t bytes, int64_t N, int n_masks, int k, Work
     return SNAPS_OK;
 }
 
-// Pointers of pivot set j (feature kLow + j) inside the pivot region.
+// Pointers of pivot set j (feature j) inside the pivot region.
 struct PivotSet {
     float4* Xs;
     float* piv;
@@ -215,18 +248,16 @@ PivotSet pivot_set(const Workspace& w, int64_t N, int j) {
 // Build the sorted copies for the pivot features the batches use (lowest high feature of each).
 snaps_status build_pivots(const Workspace& w, int64_t N, const std::vector<snaps::BatchDesc>& batches,
                           cudaStream_t st) {
-    bool need[9] = {false, false, false, false, false, false, false, false, false};
-    for (const snaps::BatchDesc& b : batches) {
-        const uint32_t hb = b.hmask >> snaps::kLow;
-        if (hb) need[__builtin_ctz(hb)] = true;
-    }
+    bool need[15] = {false};
+    for (const snaps::BatchDesc& b : batches)
+        if (b.pivot >= 0) need[b.pivot] = true;
     const int n_pad = n_blocks_for(N) * 32;
-    void* temp = w.pivot + 9 * pivot_set_bytes(N);
+    void* temp = w.pivot + 15 * pivot_set_bytes(N);
     const size_t temp_bytes = snaps::pivot_sort_temp_bytes(n_pad);
-    for (int j = 0; j < 9; ++j) {
+    for (int j = 0; j < 15; ++j) {
         if (!need[j]) continue;
         const PivotSet s = pivot_set(w, N, j);
-        CUDA_TRY(snaps::pivot_build(w.Xp, static_cast<int>(N), n_pad, snaps::kLow + j, s.Xs, s.piv, s.idmap,
+        CUDA_TRY(snaps::pivot_build(w.Xp, static_cast<int>(N), n_pad, j, s.Xs, s.piv, s.idmap,
                                     s.pos, temp, temp_bytes, st));
     }
     return SNAPS_OK;
@@ -268,7 +299,7 @@ snaps_status knn_enqueue(const Workspace& w, const snaps::BatchDesc* d_batches, 
     p.Xb = w.Xb;
     p.n_blocks = n_blocks_for(N);
     p.sweep = use_sweep(N) ? 1 : 0;
-    for (int j = 0; j < 9; ++j) {
+    for (int j = 0; j < 15; ++j) {
         const PivotSet s = p.sweep ? pivot_set(w, N, j) : PivotSet{nullptr, nullptr, nullptr, nullptr};
         p.Xs[j] = s.Xs;
         p.piv[j] = s.piv;
@@ -348,6 +379,7 @@ snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t
                                        n_tiles * snaps::kTileRows, st));
     CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
     if (use_sweep(N)) {
+        split_for_sweep(&batches);
         rc = build_pivots(w, N, batches, st);
         if (rc) return rc;
     }
@@ -382,6 +414,7 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     std::vector<snaps::BatchDesc> batches;
     plan_lattice(h_masks, n_masks, thr.data(), &batches);
+    if (use_sweep(N)) split_for_sweep(&batches);
     const int nb = static_cast<int>(batches.size());
     const int n_tiles = n_tiles_for(N);
     CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
@@ -399,7 +432,7 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
     p.Xb = w.Xb;
     p.n_blocks = n_blocks_for(N);
     p.sweep = use_sweep(N) ? 1 : 0;
-    for (int j = 0; j < 9; ++j) {
+    for (int j = 0; j < 15; ++j) {
         const PivotSet s = p.sweep ? pivot_set(w, N, j) : PivotSet{nullptr, nullptr, nullptr, nullptr};
         p.Xs[j] = s.Xs;
         p.piv[j] = s.piv;
@@ -505,6 +538,7 @@ snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat
     for (int m0 = 0; m0 < n_masks; m0 += masks_per_batch) {
         std::vector<snaps::BatchDesc> b;
         plan_lattice(h_masks + m0, std::min(masks_per_batch, n_masks - m0), nullptr, &b);
+        if (use_sweep(N)) split_for_sweep(&b);
         group_off.push_back(all_batches.size());
         all_batches.insert(all_batches.end(), b.begin(), b.end());
     }

@@ -440,12 +440,12 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
                     }
                 }
             } else {
-                const int pf = (H >> kLow) ? __ffs(H >> kLow) - 1 : -1;   // pivot: lowest high feature
+                const int pf = bd->pivot;   // a feature all valid masks of the batch contain, or -1
                 const float4* tab = pf >= 0 ? p.Xs[pf] : p.Xb;
                 const int* idm = pf >= 0 ? p.idmap[pf] : nullptr;
                 const float* pv = pf >= 0 ? p.piv[pf] : nullptr;
                 const int t0 = pf >= 0 ? (p.pos[pf][q] >> 5) : 0;
-                const float qf = pf >= 0 ? QROW(kLow + pf) : 0.f;
+                const float qf = pf >= 0 ? QROW(pf) : 0.f;
 #pragma unroll 1
                 for (int dir = 1; dir >= -1; dir -= 2) {
                     int t = dir > 0 ? t0 : t0 - 1;

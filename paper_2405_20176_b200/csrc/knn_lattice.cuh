@@ -11,10 +11,10 @@ struct KnnParams {
     const float4* Xb;           // staged table, blocked: [n_blocks][4 feature groups][32 rows] float4
     int n_blocks;               // ceil(N / 32)
     int sweep;                  // 1: pivot sweep over the sorted copies below (pivot_sort.cuh)
-    const float4* Xs[9];        // per pivot feature 6+j: blocked table sorted by that feature
-    const float* piv[9];        //   its sorted values
-    const int* idmap[9];        //   sorted position -> object id
-    const int* pos[9];          //   object id -> sorted position
+    const float4* Xs[15];        // per pivot feature: blocked table sorted by that feature
+    const float* piv[15];        //   its sorted values
+    const int* idmap[15];        //   sorted position -> object id
+    const int* pos[15];          //   object id -> sorted position
     int N;
     int k;
     const BatchDesc* batches;   // device

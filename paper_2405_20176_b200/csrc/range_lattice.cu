@@ -221,12 +221,12 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
                     }
                 }
             } else {
-                const int pf = (H >> kLow) ? __ffs(H >> kLow) - 1 : -1;   // pivot: lowest high feature
+                const int pf = bd->pivot;   // a feature all valid masks of the batch contain, or -1
                 const float4* tab = pf >= 0 ? p.Xs[pf] : p.Xb;
                 const int* idm = pf >= 0 ? p.idmap[pf] : nullptr;
                 const float* pv = pf >= 0 ? p.piv[pf] : nullptr;
                 const int t0 = pf >= 0 ? (p.pos[pf][q] >> 5) : 0;
-                const float qf = pf >= 0 ? R_QROW(kLow + pf) : 0.f;
+                const float qf = pf >= 0 ? R_QROW(pf) : 0.f;
                 float Gall = G[0];
 #pragma unroll
                 for (int u = 1; u < 16; ++u) Gall = fmaxf(Gall, G[u]);

@@ -11,10 +11,10 @@ struct RangeParams {
     const float4* Xb;           // staged table, blocked (candidate stream)
     int n_blocks;               // ceil(N / 32)
     int sweep;                  // 1: pivot sweep over the sorted copies below (pivot_sort.cuh)
-    const float4* Xs[9];
-    const float* piv[9];
-    const int* idmap[9];
-    const int* pos[9];
+    const float4* Xs[15];
+    const float* piv[15];
+    const int* idmap[15];
+    const int* pos[15];
     int N;
     const BatchDesc* batches;   // thr[] = nextafter(eps^2) per slot, -1 for unused slots
     int n_batches;

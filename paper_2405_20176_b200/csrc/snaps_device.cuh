@@ -32,7 +32,8 @@ struct alignas(16) BatchDesc {
     int32_t slot[kLat];
     uint32_t hmask;            // bits 6..14
     int32_t n_valid;
-    int32_t pad_[2];
+    int32_t pivot;             // pivot sweep: a feature every valid mask of the batch contains, or -1
+    int32_t pad_;
 };
 static_assert(sizeof(BatchDesc) % 16 == 0, "BatchDesc rows are read with 128-bit loads");
 
