@@ -406,3 +406,28 @@ def test_eps_grid_by_repeating_masks(snaps, oracle_mod):
     check_range(cnt, out["sumdist"].cpu().numpy(), out["mean"].cpu().numpy(), oracle_mod, X, masks, eps)
     c = cnt.reshape(len(base), len(grid), -1)
     assert (np.diff(c, axis=1) >= 0).all() and (c[:, -1] > c[:, 0]).any()
+
+
+def test_config5_scale_low_dimensional_masks(snaps, oracle_mod):
+    """BASELINE.json configs[4]'s N and k (N=5,000,000 x 15, seed 4, k=16; DSSJ beside it) on six
+    two- and three-feature masks, which the pivot sweep prunes; c5's own 256 random masks average 7.5
+    features and are out of reach at this N.  Sampled rows against the oracle."""
+    import torch
+    n, k = 5_000_000, 16
+    X = workloads.make_table(n, 4, outlier_frac=0.001)
+    masks = np.array([(1 << 6) | (1 << 9), (1 << 7) | (1 << 14), (1 << 0) | (1 << 3), (1 << 2) | (1 << 11),
+                      (1 << 4) | (1 << 5), (1 << 8) | (1 << 13) | (1 << 1)], dtype=np.uint16)
+    Xd = _dev(X)
+    out = snaps.knn_selfjoin(Xd, masks, k)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(3)
+    qs = np.sort(rng.choice(n, 12, replace=False))
+    oi, od = oracle_mod.knn_selfjoin(X, masks, k + 1, queries=qs)
+    check_knn(out["idx"][:, qs].cpu().numpy(), out["dist"][:, qs].cpu().numpy(), oi, od, queries=qs)
+    assert bool((out["indeg"].sum(dim=1) == n * k).all())
+    eps = (np.median(od[:, :, -1], axis=1) * 1.5).astype(np.float32)
+    del out
+    r = snaps.range_selfjoin(Xd, masks, eps)
+    torch.cuda.synchronize()
+    check_range(r["count"][:, qs].cpu().numpy(), r["sumdist"][:, qs].cpu().numpy(), r["mean"][:, qs].cpu().numpy(),
+                oracle_mod, X, masks, eps, queries=qs)
