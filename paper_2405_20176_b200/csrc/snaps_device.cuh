@@ -1,11 +1,10 @@
 // snaps_device.cuh -- device-side building blocks shared by the join kernels (sm_100a).
 //
-// Layout of the staged table ("a1" in DESIGN.md): row r of the caller's N x n_feat
-// fp32 matrix becomes 20 floats (80 bytes): features 0..14, then 5 zeros.  80 B
-// rows make per-lane 128-bit shared-memory reads conflict-free (lane stride 20
-// words -> the 8 lanes of a quarter-warp hit 8 disjoint 4-bank groups) and keep
-// a tile of rows one contiguous block, so a tile moves with ONE bulk async copy
-// (cp.async.bulk, SASS UBLKCP) that signals an mbarrier.
+// Layouts of the staged table ("a1" in DESIGN.md).  Row-major copy Xp: row r of the caller's
+// N x n_feat fp32 matrix becomes 20 floats (80 bytes): features 0..14, then 5 zeros; used for
+// query rows, seed evaluations and as the gather source of the sorted copies.  Blocked copy Xb
+// (the candidate stream of both join kernels): 32 rows per block, four feature groups of 32
+// float4 per block, read with four fully coalesced 128-bit loads per warp.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -14,9 +13,8 @@ namespace snaps {
 
 constexpr int kRowFloats = 20;                 // staged row: 15 features + 5 pad
 constexpr int kRowBytes = kRowFloats * 4;      // 80
-constexpr int kTileRows = 128;                 // candidates per smem tile
+constexpr int kTileRows = 128;                 // Xp is padded to a multiple of 128 rows
 constexpr int kTileBytes = kTileRows * kRowBytes;  // 10240
-constexpr int kStages = 3;                     // tile ring depth
 constexpr int kLow = 6;                        // lattice features per batch
 constexpr int kLat = 1 << kLow;                // 64 subset sums per (pair, batch)
 constexpr int kRing = 128;                     // kNN: per-warp ring of (list, id, d^2) triples awaiting merge
@@ -36,46 +34,6 @@ struct alignas(16) BatchDesc {
     int32_t pad_;
 };
 static_assert(sizeof(BatchDesc) % 16 == 0, "BatchDesc rows are read with 128-bit loads");
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_fence_init() {
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra DONE_%=;\n\t"
-        "bra WAIT_%=;\n\t"
-        "DONE_%=:\n\t"
-        "}" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-// 1-D bulk async copy global -> shared, completion counted in bytes on `bar`.
-__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes,
-                                         uint64_t* bar) {
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
-            "r"(smem_u32(smem_dst)),
-        "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
-        : "memory");
-}
 
 // Squared distance on a runtime mask from two staged rows (slow paths only).
 __device__ __forceinline__ float masked_d2(const float* __restrict__ a, const float* __restrict__ b,
