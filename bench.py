@@ -153,7 +153,7 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
-def run_lsst(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks):
+def run_lsst(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks, emit=True):
     """Extra line for the LSST-scale config (BASELINE.json configs[3]): N=1,000,000, the 105
     two-feature subspaces + the full space, k=10, lists and scores streamed to pinned host memory
     (`snaps_knn_selfjoin_streamed`; the pivot sweep prunes the scan exactly).  `value` here is end
@@ -180,7 +180,7 @@ def run_lsst(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks)
     if rank == 0:
         evals = float(N) * N * n_masks
         d2h = int(sum(t.numel() * t.element_size() for t in out.values()))
-        print(json.dumps({
+        line = ({
             "metric": "subspaces/sec (kNNSJ N=1,000,000, k=10, 105 pair subspaces + full space, pivot sweep)",
             "value": world * n_masks / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": 1,
             "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
@@ -191,8 +191,11 @@ def run_lsst(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks)
             "note": "exactly pruned scan: effective evals = N^2 x masks / time, not operations performed",
             "e2e": {"value": world * n_masks / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0,
                     "d2h_bytes_per_step": d2h},
-            "paper_context": "paper, LSST5M (N=5e6, k_max=256): ~100 s per feature space on 1xA100 (Table 4)"}),
-            flush=True)
+            "paper_context": "paper, LSST5M (N=5e6, k_max=256): ~100 s per feature space on 1xA100 (Table 4)"})
+        if emit:
+            print(json.dumps(line), flush=True)
+        return line
+    return None
 
 
 def run_range(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks):
@@ -261,6 +264,8 @@ def main():
     ap.add_argument("--cpu-queries", type=int, default=4096,
                     help="sampled queries of the cpu_baseline leg (0 = skip)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-lsst", action="store_true",
+                    help="skip the LSST-scale leg (config 4, N=1,000,000) that the default run reports beside config 2")
     ap.add_argument("--profile-masks", type=int, default=0,
                     help="profiling aid (ncu --set full replays every launch ~40x): keep only the "
                          "first M masks; the JSON line is then marked profile_only and is NOT a bench value")
@@ -436,6 +441,21 @@ def main():
         cpu = {"value": ev / dt / (float(N) * N), "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": what, "evals_per_s": ev / dt, "seconds": dt}
 
+    # ---- LSST-scale leg, side by side (north star): config 4 at full size, one warm + one timed pass
+    lsst = None
+    if rank == 0 and world == 1 and not args.no_lsst and args.profile_masks == 0 and args.config == "c2_snapshot1_knn":
+        try:
+            Xd = ws = out = hout = hws = xdev = Xh = None     # release config 2's device and pinned buffers
+            torch.cuda.empty_cache()
+            largs = argparse.Namespace(**{**vars(args), "steps": 1})
+            full = run_lsst(largs, workloads.get_config("c4_lsst_pairs"), snaps, torch, dev, rank, world,
+                            barrier, max_over_ranks, emit=False)
+            lsst = {k_: full[k_] for k_ in ("metric", "value", "unit", "ms_per_step", "effective_evals_per_s", "note")}
+            lsst["workload"] = full["config"]["workload"]
+            lsst["d2h_bytes_per_step"] = full["e2e"]["d2h_bytes_per_step"]
+        except Exception as e:                                   # the headline line must survive this leg
+            lsst = {"error": repr(e)[:200]}
+
     if rank == 0:
         line = {
             **({"profile_only": f"{n_masks} masks from index {args.profile_offset}"} if args.profile_masks > 0 else {}),
@@ -447,6 +467,7 @@ def main():
                        "outputs": "scores only (lists of this config are 83 GB)"},
             "evals_per_s": evals_per_s, "fp32_peak_frac": roofline["frac"],
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
+            "lsst_scale": lsst,
             "clocks": clocks,
             "paper_context": "paper: DSSJ all 32,752 spaces 2.64 h on 1xA100 (o=8) incl. CPU "
                              "post-processing; LSST5M kNNSJ ~100 s/feature space (PAPER.md:394, Table 4)",
