@@ -200,14 +200,12 @@ def run_lsst(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks,
 
 def run_range(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks):
     """Extra line for the DSSJ config (BASELINE.json configs[2]): one pass of snaps_range_selfjoin
-    over all masks with the oracle-calibrated eps_d (calibration outside the timed region).
+    over all masks with the stored eps_d of the configuration (workloads/config_eps.json).
     Not the headline metric; printed with the same keys so that the numbers in DESIGN.md can be
     reproduced with `python bench.py --config c3_snapshot1_dssj`."""
-    from oracle.calibrate import eps_per_dimension     # input preparation, as in the parity test
     X = workloads.make_table(cfg.n, cfg.seed + rank, cols=list(range(cfg.n_feat)), outlier_frac=0.01)
     masks = cfg.masks()
-    eps = eps_per_dimension(X, masks, cfg.target_neighbours, seed=cfg.seed, max_masks_per_dim=4,
-                            n_query_sample=300).astype(np.float32)
+    eps = workloads.config_eps(cfg.name, masks)        # stored inputs (oracle/write_config_eps.py)
     if args.profile_masks > 0:      # profiling aid, see --profile-masks
         sl = slice(args.profile_offset, args.profile_offset + args.profile_masks)
         masks, eps = masks[sl], eps[sl]

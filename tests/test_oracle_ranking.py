@@ -50,3 +50,16 @@ def test_topn_and_ties():
     kth, mean, indeg = ranking.knn_scores_at_k(np.array([[1, 2, 0], [0, 2, 1], [1, 0, 2]])[:, :3],
                                                np.array([[1., 2., 3.], [1., 1., 4.], [2., 2., 2.]]), 2, 3)
     assert kth.tolist() == [2., 1., 2.] and mean.tolist() == [1.5, 1., 2.] and indeg.tolist() == [2, 2, 2]
+
+
+def test_stored_config_eps_come_from_the_oracle_script():
+    # workloads/config_eps.json is written by oracle/write_config_eps.py (calls only oracle/);
+    # regenerate in memory and compare
+    import workloads
+    from oracle.calibrate import eps_per_dimension
+    cfg = workloads.get_config("c3_snapshot1_dssj")
+    X, masks = cfg.table(), cfg.masks()
+    eps = eps_per_dimension(X, masks, cfg.target_neighbours, seed=cfg.seed, max_masks_per_dim=4,
+                            n_query_sample=300).astype(np.float32)
+    assert (workloads.config_eps(cfg.name, masks) == eps).all()
+    assert (np.diff([eps[workloads.popcount(masks) == d][0] for d in range(2, 16)]) > 0).all()   # grows with d

@@ -6,10 +6,10 @@ BASELINE.json configurations.  Recipe: DESIGN.md "Input recipe"
 """
 from .tables import make_table, hypercube_table, duplicate_block_table, lattice_table, COLUMN_NAMES
 from .masks import all_masks, pair_masks_plus_full, sample_masks, popcount
-from .configs import CONFIGS, get_config
+from .configs import CONFIGS, get_config, config_eps
 
 __all__ = [
     "make_table", "hypercube_table", "duplicate_block_table", "lattice_table",
     "COLUMN_NAMES", "all_masks", "pair_masks_plus_full", "sample_masks",
-    "popcount", "CONFIGS", "get_config",
+    "popcount", "CONFIGS", "get_config", "config_eps",
 ]

@@ -44,3 +44,14 @@ CONFIGS = {
 
 def get_config(name: str) -> Config:
     return CONFIGS[name]
+
+
+def config_eps(name: str, masks) -> np.ndarray:
+    """Per-mask radii of a DSSJ configuration from workloads/config_eps.json (written by
+    `python -m oracle.write_config_eps`; inputs, like the tables): eps_d by mask dimension."""
+    import json
+    import os
+    from .masks import popcount
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "config_eps.json")) as f:
+        by_d = json.load(f)[name]["eps_by_dimension"]
+    return np.array([by_d[str(int(d))] for d in popcount(masks)], dtype=np.float32)
