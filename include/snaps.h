@@ -214,10 +214,12 @@ snaps_status snaps_topn_overlap(const int32_t *d_order_a, const int32_t *d_order
 
 /*
  * Eq. 3: out_j[row] = the first j in 0..G-1 that minimises
- * |U_min[j][row] - U_max[j][row]|.  d_u_min, d_u_max: device, [G][n_rows] fp32.
+ * |U_min[j][row] - U_max[j][row]|.  d_u_min, d_u_max: device, [G][n_rows] fp32.  n_top > 0: the n
+ * of Eq. 2 that made the fractions; they are taken back to integer hit counts first so that equal
+ * differences compare equal (ties must not hang on rounding).  n_top = 0: compare the floats.
  */
 snaps_status snaps_select_parameter(const float *d_u_min, const float *d_u_max, int G, int n_rows,
-                                    int32_t *out_j, void *stream);
+                                    int n_top, int32_t *out_j, void *stream);
 
 /*
  * k grid: scores for k_j <= k_max from lists computed once for k_max (their
@@ -228,6 +230,27 @@ snaps_status snaps_knn_scores_at_k(int64_t N, int n_masks, int k_max, int k_j,
                                    const int32_t *knn_idx, const float *knn_dist,
                                    float *out_kth, float *out_mean, int32_t *out_indeg,
                                    void *stream);
+
+/*
+ * k^select per feature space (Eq. 2 and Eq. 3 applied to the k grid): from lists
+ * computed once for k_max, for every k_j of the grid derive the scores (prefix), rank them, compare
+ * the top-n sets with those of the smallest and the largest k, and select the k_j that minimises
+ * |U_min - U_max| -- for the distance-oblivious metric (in-degree) and the distance-aware metric
+ * (mean kNN distance).
+ *   knn_idx, knn_dist  device, [n_masks][N][k_max] as written by snaps_knn_selfjoin
+ *   h_k_grid           host, [G] ascending, 1 <= k_j <= k_max, G >= 2
+ *   n_top              n of Eq. 2 (the paper uses 0.01 |D|), 1 <= n_top <= N
+ *   out_j_indeg, out_j_mean   device, [n_masks] int32: index into the grid of the selected k
+ *   out_u                     device, [4][G][n_masks] fp32 or NULL: U_min / U_max of the in-degree
+ *                             metric, then U_min / U_max of the mean-distance metric
+ * Workspace: snaps_select_k_workspace_bytes(N, n_masks).
+ */
+size_t snaps_select_k_workspace_bytes(int64_t N, int n_masks);
+
+snaps_status snaps_knn_select_k(int64_t N, int n_masks, int k_max, const int32_t *knn_idx,
+                                const float *knn_dist, const int32_t *h_k_grid, int G, int n_top,
+                                int32_t *out_j_indeg, int32_t *out_j_mean, float *out_u,
+                                void *d_workspace, size_t workspace_bytes, void *stream);
 
 /*
  * DSSJ for a grid of radii in ONE scan (Fig. 3: "we execute DSSJ once for

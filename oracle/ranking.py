@@ -62,9 +62,14 @@ def similarity_curves(topn_sets, n: int):
     return u_min, u_max
 
 
-def select_parameter(u_min, u_max) -> int:
-    """Eq. 3: argmin_j |U_min[j] - U_max[j]| (first minimiser)."""
-    return int(np.argmin(np.abs(np.asarray(u_min) - np.asarray(u_max))))
+def select_parameter(u_min, u_max, n: int | None = None) -> int:
+    """Eq. 3: argmin_j |U_min[j] - U_max[j]| (first minimiser).  With n given the
+    fractions are taken back to their integer hit counts first, so that equal differences are
+    exactly equal (f = hits / n: ties must not be decided by floating-point rounding)."""
+    a, b = np.asarray(u_min, dtype=np.float64), np.asarray(u_max, dtype=np.float64)
+    if n is not None:
+        a, b = np.rint(a * n), np.rint(b * n)
+    return int(np.argmin(np.abs(a - b)))
 
 
 def knn_scores_at_k(idx_kmax, dist_kmax, kj: int, N: int):
@@ -73,3 +78,19 @@ def knn_scores_at_k(idx_kmax, dist_kmax, kj: int, N: int):
     idx = np.asarray(idx_kmax)[:, :kj]
     dist = np.asarray(dist_kmax, dtype=np.float64)[:, :kj]
     return dist[:, -1], dist.mean(axis=1), np.bincount(idx.ravel(), minlength=N)
+
+
+def select_k(idx_kmax, dist_kmax, k_grid, n: int, N: int):
+    """The k-grid procedure of PAPER.md:256-258 for ONE mask, step by step: for every k_j the scores
+    from the k_max lists, their top-n sets, U_min / U_max against the smallest and largest k
+    (Eq. 2), and the selected grid index (Eq. 3) -- for the in-degree and the mean-distance metric.
+    -> dict metric -> (j_select, u_min, u_max)."""
+    out = {}
+    for metric, pick in (("knn_indegree", 2), ("knn_mean", 1)):
+        tops = []
+        for kj in k_grid:
+            sc = knn_scores_at_k(idx_kmax, dist_kmax, int(kj), N)
+            tops.append(topn_ids(metric, sc[pick], n))
+        u_min, u_max = similarity_curves(tops, n)
+        out[metric] = (select_parameter(u_min, u_max, n), u_min, u_max)
+    return out

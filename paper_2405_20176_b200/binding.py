@@ -15,6 +15,7 @@ EXPORTED_SYMBOLS = [
     "snaps_profile_enable", "snaps_profile_last_kernel_ms",
     "snaps_rank_workspace_bytes", "snaps_rank_scores", "snaps_topn_overlap", "snaps_select_parameter",
     "snaps_knn_scores_at_k", "snaps_range_grid_workspace_bytes", "snaps_range_selfjoin_grid",
+    "snaps_select_k_workspace_bytes", "snaps_knn_select_k",
 ]
 
 _lib = None
@@ -68,11 +69,15 @@ def lib():
         L.snaps_topn_overlap.restype = i32
         L.snaps_topn_overlap.argtypes = [vp, vp, i64, i32, i32, vp, vp]
         L.snaps_select_parameter.restype = i32
-        L.snaps_select_parameter.argtypes = [vp, vp, i32, i32, vp, vp]
+        L.snaps_select_parameter.argtypes = [vp, vp, i32, i32, i32, vp, vp]
         L.snaps_range_grid_workspace_bytes.restype = sz
         L.snaps_range_grid_workspace_bytes.argtypes = [i64, i32, i32, i32]
         L.snaps_range_selfjoin_grid.restype = i32
         L.snaps_range_selfjoin_grid.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, vp, vp, vp, sz, vp]
+        L.snaps_select_k_workspace_bytes.restype = sz
+        L.snaps_select_k_workspace_bytes.argtypes = [i64, i32]
+        L.snaps_knn_select_k.restype = i32
+        L.snaps_knn_select_k.argtypes = [i64, i32, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp, sz, vp]
         L.snaps_knn_scores_at_k.restype = i32
         L.snaps_knn_scores_at_k.argtypes = [i64, i32, i32, i32, vp, vp, vp, vp, vp, vp]
         _lib = L
@@ -297,12 +302,12 @@ def topn_overlap(order_a, order_b, n: int, stream=None):
     return f
 
 
-def select_parameter(u_min, u_max, stream=None):
+def select_parameter(u_min, u_max, n_top: int = 0, stream=None):
     """snaps_select_parameter (Eq. 3): u_* [G, n_rows] fp32 -> int32 [n_rows]."""
     import torch
     G, n_rows = u_min.shape
     j = torch.empty(n_rows, dtype=torch.int32, device=u_min.device)
-    _check(lib().snaps_select_parameter(_dptr(u_min), _dptr(u_max), G, n_rows, _dptr(j), _stream(stream)))
+    _check(lib().snaps_select_parameter(_dptr(u_min), _dptr(u_max), G, n_rows, n_top, _dptr(j), _stream(stream)))
     return j
 
 
@@ -342,5 +347,24 @@ def range_selfjoin_grid(X, masks, eps_grid, *, sums=True, stream=None):
         _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
         e.ctypes.data_as(ctypes.c_void_p), G, _dptr(out["count"]), _dptr(out.get("sumdist")),
         _dptr(out.get("mean")), _dptr(ws), ws.numel(), _stream(stream)))
+    out["_workspace"] = ws
+    return out
+
+
+def knn_select_k(knn_idx, knn_dist, k_grid, n_top: int, stream=None):
+    """snaps_knn_select_k: lists [n_masks, N, k_max] -> dict j_indeg / j_mean (grid index per mask)
+    and u [4, G, n_masks] (U_min, U_max of the in-degree metric, then of the mean-distance metric)."""
+    import torch
+    n_masks, N, k_max = knn_dist.shape
+    grid = np.ascontiguousarray(np.asarray(k_grid, dtype=np.int32))
+    G = len(grid)
+    dev = knn_dist.device
+    out = {"j_indeg": torch.empty(n_masks, dtype=torch.int32, device=dev),
+           "j_mean": torch.empty(n_masks, dtype=torch.int32, device=dev),
+           "u": torch.empty((4, G, n_masks), dtype=torch.float32, device=dev)}
+    ws = torch.empty(int(lib().snaps_select_k_workspace_bytes(N, n_masks)), dtype=torch.uint8, device=dev)
+    _check(lib().snaps_knn_select_k(N, n_masks, k_max, _dptr(knn_idx), _dptr(knn_dist),
+                                    grid.ctypes.data_as(ctypes.c_void_p), G, n_top, _dptr(out["j_indeg"]),
+                                    _dptr(out["j_mean"]), _dptr(out["u"]), _dptr(ws), ws.numel(), _stream(stream)))
     out["_workspace"] = ws
     return out

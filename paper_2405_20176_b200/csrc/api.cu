@@ -663,6 +663,81 @@ snaps_status snaps_range_selfjoin_grid(const float* d_X, int64_t N, int n_feat, 
     return SNAPS_OK;
 }
 
+size_t snaps_select_k_workspace_bytes(int64_t N, int n_masks) {
+    if (N < 2 || n_masks < 1) return 0;
+    const size_t arr = align_up(static_cast<size_t>(N) * n_masks * 4, 256);
+    // score array, three order arrays (smallest k, largest k, current k), ranking scratch
+    return 4 * arr + align_up(snaps::rank_workspace_bytes(N, n_masks), 256);
+}
+
+snaps_status snaps_knn_select_k(int64_t N, int n_masks, int k_max, const int32_t* knn_idx, const float* knn_dist,
+                                const int32_t* h_k_grid, int G, int n_top, int32_t* out_j_indeg,
+                                int32_t* out_j_mean, float* out_u, void* d_workspace, size_t workspace_bytes,
+                                void* stream) {
+    if (N < 2 || n_masks < 1 || k_max < 1 || !knn_idx || !knn_dist || !h_k_grid)
+        return fail(SNAPS_INVALID_ARG, "bad sizes or NULL inputs");
+    if (G < 2 || G > 256) return fail(SNAPS_INVALID_ARG, "G = %d outside 2..256", G);
+    for (int j = 0; j < G; ++j)
+        if (h_k_grid[j] < 1 || h_k_grid[j] > k_max || (j > 0 && h_k_grid[j] <= h_k_grid[j - 1]))
+            return fail(SNAPS_INVALID_ARG, "k grid must ascend within 1..k_max (entry %d = %d)", j, h_k_grid[j]);
+    if (n_top < 1 || n_top > N) return fail(SNAPS_INVALID_ARG, "n_top = %d outside 1..N", n_top);
+    if (!out_j_indeg || !out_j_mean) return fail(SNAPS_INVALID_ARG, "NULL outputs");
+    if ((N + 31) / 32 * 4 > 200 * 1024) return fail(SNAPS_UNSUPPORTED, "N too large for the top-n bitmap");
+    if (!d_workspace || workspace_bytes < snaps_select_k_workspace_bytes(N, n_masks))
+        return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", workspace_bytes,
+                    snaps_select_k_workspace_bytes(N, n_masks));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t arr = align_up(static_cast<size_t>(N) * n_masks * 4, 256);
+    unsigned char* p = static_cast<unsigned char*>(d_workspace);
+    void* score = p;
+    int32_t* ord_min = reinterpret_cast<int32_t*>(p + arr);
+    int32_t* ord_max = reinterpret_cast<int32_t*>(p + 2 * arr);
+    int32_t* ord_cur = reinterpret_cast<int32_t*>(p + 3 * arr);
+    void* rws = p + 4 * arr;
+    const size_t rws_bytes = workspace_bytes - 4 * arr;
+    float* u_tmp = nullptr;   // U arrays live in out_u if given, else in a temporary device buffer
+    float* u = out_u;
+    if (!u) {
+        CUDA_TRY(cudaMallocAsync(&u_tmp, sizeof(float) * 4 * G * static_cast<size_t>(n_masks), st));
+        u = u_tmp;
+    }
+    snaps_status rc = SNAPS_OK;
+    for (int metric = 0; metric < 2 && rc == SNAPS_OK; ++metric) {
+        const int kind = metric == 0 ? SNAPS_METRIC_KNN_INDEGREE : SNAPS_METRIC_KNN_MEAN;
+        float* u_min = u + static_cast<size_t>(2 * metric) * G * n_masks;
+        float* u_max = u + static_cast<size_t>(2 * metric + 1) * G * n_masks;
+        auto order_for = [&](int kj, int32_t* ord) -> cudaError_t {
+            cudaError_t e;
+            if (metric == 0) {
+                e = cudaMemsetAsync(score, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, st);
+                if (e != cudaSuccess) return e;
+                e = snaps::scores_at_k_launch(N, n_masks, k_max, kj, knn_idx, nullptr, nullptr, nullptr,
+                                              static_cast<int32_t*>(score), st);
+            } else {
+                e = snaps::scores_at_k_launch(N, n_masks, k_max, kj, nullptr, knn_dist, nullptr,
+                                              static_cast<float*>(score), nullptr, st);
+            }
+            if (e != cudaSuccess) return e;
+            return snaps::rank_launch(kind, score, nullptr, N, n_masks, nullptr, ord, rws, rws_bytes, st);
+        };
+        cudaError_t e = order_for(h_k_grid[0], ord_min);
+        if (e == cudaSuccess) e = order_for(h_k_grid[G - 1], ord_max);
+        for (int j = 0; j < G && e == cudaSuccess; ++j) {
+            const int32_t* oc = j == 0 ? ord_min : (j == G - 1 ? ord_max : ord_cur);
+            if (j > 0 && j < G - 1) e = order_for(h_k_grid[j], ord_cur);
+            if (e == cudaSuccess)
+                e = snaps::topn_overlap_launch(ord_min, oc, N, n_masks, n_top, u_min + static_cast<size_t>(j) * n_masks, st);
+            if (e == cudaSuccess)
+                e = snaps::topn_overlap_launch(ord_max, oc, N, n_masks, n_top, u_max + static_cast<size_t>(j) * n_masks, st);
+        }
+        if (e == cudaSuccess)
+            e = snaps::select_launch(u_min, u_max, G, n_masks, n_top, metric == 0 ? out_j_indeg : out_j_mean, st);
+        if (e != cudaSuccess) rc = fail(SNAPS_CUDA_ERROR, "select_k: %s", cudaGetErrorString(e));
+    }
+    if (u_tmp) cudaFreeAsync(u_tmp, st);
+    return rc;
+}
+
 size_t snaps_rank_workspace_bytes(int64_t N, int n_rows) {
     if (N < 1 || n_rows < 1) return 0;
     return snaps::rank_workspace_bytes(N, n_rows);
@@ -693,10 +768,10 @@ snaps_status snaps_topn_overlap(const int32_t* d_order_a, const int32_t* d_order
     return SNAPS_OK;
 }
 
-snaps_status snaps_select_parameter(const float* d_u_min, const float* d_u_max, int G, int n_rows,
+snaps_status snaps_select_parameter(const float* d_u_min, const float* d_u_max, int G, int n_rows, int n_top,
                                     int32_t* out_j, void* stream) {
-    if (!d_u_min || !d_u_max || !out_j || G < 1 || n_rows < 1) return fail(SNAPS_INVALID_ARG, "bad arguments");
-    CUDA_TRY(snaps::select_launch(d_u_min, d_u_max, G, n_rows, out_j, static_cast<cudaStream_t>(stream)));
+    if (!d_u_min || !d_u_max || !out_j || G < 1 || n_rows < 1 || n_top < 0) return fail(SNAPS_INVALID_ARG, "bad arguments");
+    CUDA_TRY(snaps::select_launch(d_u_min, d_u_max, G, n_rows, n_top, out_j, static_cast<cudaStream_t>(stream)));
     return SNAPS_OK;
 }
 

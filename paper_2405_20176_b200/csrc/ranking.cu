@@ -153,13 +153,17 @@ cudaError_t topn_overlap_launch(const int32_t* order_a, const int32_t* order_b, 
 }
 
 // Eq. 3 per row: argmin_j |U_min[j] - U_max[j]| (first minimiser).  u_*: [G][n_rows].
+// With n_top > 0 the fractions are taken back to integer hit counts (f = hits / n), so that equal
+// differences compare equal and the first minimiser is well defined.
 __global__ void select_kernel(const float* __restrict__ u_min, const float* __restrict__ u_max, int G,
-                              int n_rows, int32_t* __restrict__ out_j) {
+                              int n_rows, int n_top, int32_t* __restrict__ out_j) {
+    const float sc = n_top > 0 ? static_cast<float>(n_top) : 1.f;
     for (int r = blockIdx.x * blockDim.x + threadIdx.x; r < n_rows; r += gridDim.x * blockDim.x) {
         int best = 0;
-        float bd = fabsf(u_min[r] - u_max[r]);
+        float bd = fabsf(n_top > 0 ? rintf(u_min[r] * sc) - rintf(u_max[r] * sc) : u_min[r] - u_max[r]);
         for (int j = 1; j < G; ++j) {
-            const float d = fabsf(u_min[static_cast<size_t>(j) * n_rows + r] - u_max[static_cast<size_t>(j) * n_rows + r]);
+            const float a = u_min[static_cast<size_t>(j) * n_rows + r], b = u_max[static_cast<size_t>(j) * n_rows + r];
+            const float d = fabsf(n_top > 0 ? rintf(a * sc) - rintf(b * sc) : a - b);
             if (d < bd) {
                 bd = d;
                 best = j;
@@ -169,9 +173,9 @@ __global__ void select_kernel(const float* __restrict__ u_min, const float* __re
     }
 }
 
-cudaError_t select_launch(const float* u_min, const float* u_max, int G, int n_rows, int32_t* out_j,
+cudaError_t select_launch(const float* u_min, const float* u_max, int G, int n_rows, int n_top, int32_t* out_j,
                           cudaStream_t stream) {
-    select_kernel<<<(n_rows + 255) / 256, 256, 0, stream>>>(u_min, u_max, G, n_rows, out_j);
+    select_kernel<<<(n_rows + 255) / 256, 256, 0, stream>>>(u_min, u_max, G, n_rows, n_top, out_j);
     return cudaGetLastError();
 }
 
