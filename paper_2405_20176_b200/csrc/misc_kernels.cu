@@ -105,27 +105,38 @@ cudaError_t eps_mean_launch(int64_t total, const uint32_t* cnt, const float* sum
 }
 
 // ---- FP32 instruction-rate probes (roofline denominator) ----
-constexpr int kProbeIters = 4096;
+constexpr int kProbeIters = 1024;
 constexpr int kProbeIlp = 16;
+constexpr int kProbeUnroll = 8;   // 128 arithmetic instructions per loop trip: loop overhead < 3%
 
 template <int KIND>
 __global__ void __launch_bounds__(512, 1) probe_kernel(float* out, float a, float b) {
     float v[kProbeIlp];
 #pragma unroll
     for (int i = 0; i < kProbeIlp; ++i) v[i] = a * static_cast<float>(threadIdx.x + i);
-    int hits = 0;
+    unsigned hits = 0u;
 #pragma unroll 1
     for (int it = 0; it < kProbeIters; ++it) {
 #pragma unroll
-        for (int i = 0; i < kProbeIlp; ++i) {
-            if (KIND == 0) {
-                v[i] = __fmaf_rn(v[i], a, b);
-            } else if (KIND == 1) {
-                v[i] = __fadd_rn(v[i], b);
-            } else {
-                v[i] = __fadd_rn(v[i], b);
-                // one compare per add, OR-chained into a predicate like the join's filter
-                hits |= (v[i] < a) ? 1 : 0;
+        for (int r = 0; r < kProbeUnroll; ++r) {
+#pragma unroll
+            for (int i = 0; i < kProbeIlp; ++i) {
+                if (KIND == 0) {
+                    v[i] = __fmaf_rn(v[i], a, b);
+                } else if (KIND == 1) {
+                    v[i] = __fadd_rn(v[i], b);
+                } else {
+                    // the join's filter mix: one add and one compare per value, the compares OR-ed
+                    // into two predicate chains (FSETP.LT.OR), as in FILTER
+                    v[i] = __fadd_rn(v[i], b);
+                    unsigned p;
+                    asm volatile(
+                        "{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %1, 0;\n\tsetp.lt.or.f32 q, %2, %3, q;\n\t"
+                        "selp.u32 %0, 1, 0, q;\n\t}"
+                        : "=r"(p)
+                        : "r"(hits), "f"(v[i]), "f"(a));
+                    hits = p;
+                }
             }
         }
     }
@@ -153,7 +164,7 @@ cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, cudaStream_
     e = cudaEventSynchronize(e1);
     if (e == cudaSuccess) e = cudaGetLastError();
     cudaEventElapsedTime(ms, e0, e1);
-    const double per_thread = static_cast<double>(kProbeIters) * kProbeIlp * (kind == 2 ? 2.0 : 1.0);
+    const double per_thread = static_cast<double>(kProbeIters) * kProbeUnroll * kProbeIlp * (kind == 2 ? 2.0 : 1.0);
     *lane_ops = per_thread * grid * block;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
