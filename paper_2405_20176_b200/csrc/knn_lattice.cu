@@ -210,22 +210,16 @@ __device__ __noinline__ void knn_seed(float* ws, const float* __restrict__ Xp, i
         float bound = -1.f;
         if (SLOT(L) >= 0) {
             const uint32_t mask = H | static_cast<uint32_t>(L);
+            // k known objects bound the k-th distance: the previous batch's neighbours of this slot
+            // (consecutive batches differ in one feature) if that list is full, else the first k ids
+            const bool from_prev = has_prev && L_D2(NE - 1, L) < __int_as_float(0x7f800000);
             float b1 = 0.f;
 #pragma unroll 1
             for (int e = 0; e < k; ++e) {
-                const int c = e + (e >= q ? 1 : 0);
+                const int c = from_prev ? L_ID(NE - k + e, L) : e + (e >= q ? 1 : 0);
                 b1 = fmaxf(b1, masked_d2(Xp + static_cast<size_t>(c) * kRowFloats, qrow, mask));
             }
             bound = b1;
-            if (has_prev && L_D2(NE - 1, L) < __int_as_float(0x7f800000)) {   // previous list is full
-                float b2 = 0.f;
-#pragma unroll 1
-                for (int e = NE - k; e < NE; ++e) {
-                    const int c = L_ID(e, L);
-                    b2 = fmaxf(b2, masked_d2(Xp + static_cast<size_t>(c) * kRowFloats, qrow, mask));
-                }
-                bound = fminf(bound, b2);
-            }
             // the stream re-evaluates these objects in another summation order: leave
             // room for rounding (<= 15 * 2^-24 relative) so that none of them is lost
             bound = fmaxf(bound * 1.00002f, 1e-30f);
