@@ -269,6 +269,37 @@ snaps_status snaps_range_selfjoin_grid(const float *d_X, int64_t N, int n_feat, 
                                        size_t workspace_bytes, void *stream);
 
 /*
+ * ---- NEXT-2: search radius for a target selectivity ----
+ *
+ * Sampled distance histogram: for every mask, out_hist[mask][b] = number of ordered pairs (q in
+ * the query sample, c in the candidate sample, c != q by index) whose distance D(q, c; mask) falls
+ * in bin b of n_bins equal bins over [0, h_rmax[mask]); farther pairs are not counted.
+ *   h_sample_q [nq], h_sample_c [nc]  host, object ids in 0..N-1
+ *   h_rmax [n_masks]                  host, > 0: the largest radius of interest per mask
+ *   out_hist                          device, [n_masks][n_bins] uint64, zeroed by the call
+ *   1 <= n_bins <= 8192; workspace: snaps_dist_hist_workspace_bytes(nq, nc, n_masks)
+ */
+size_t snaps_dist_hist_workspace_bytes(int nq, int nc, int n_masks);
+
+snaps_status snaps_sample_distance_histogram(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                             const uint16_t *h_masks, int n_masks,
+                                             const int32_t *h_sample_q, int nq,
+                                             const int32_t *h_sample_c, int nc, const float *h_rmax,
+                                             int n_bins, unsigned long long *out_hist,
+                                             void *d_workspace, size_t workspace_bytes, void *stream);
+
+/*
+ * Host arithmetic on a histogram copied back from the device: the cumulative histogram gives the
+ * mean number of neighbours per point at each bin edge, mean(r_b) = cum[b] * (N-1) / (nq * nc')
+ * with nc' = candidates per query (nc, minus one where the query is in the candidate sample --
+ * passed as pairs_per_mask = total ordered pairs examined); h_eps[mask] = the smallest bin edge
+ * whose mean reaches target_s, or h_rmax[mask] if none does.
+ */
+snaps_status snaps_eps_from_histogram(const unsigned long long *h_hist, int n_masks, int n_bins,
+                                      const float *h_rmax, int64_t N, int64_t pairs_per_mask,
+                                      double target_s, float *h_eps);
+
+/*
  * Kernel timing for roofline reports.  While enabled,
  * every join call records a CUDA event pair on `stream` around each launch of
  * its dominant (join) kernel; the pairs of the most recent call are kept.

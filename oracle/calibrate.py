@@ -46,3 +46,39 @@ def eps_per_dimension(X, masks, target_neighbours, seed, n_query_sample=1000,
         pooled = np.concatenate(pooled)
         eps[sel] = np.quantile(pooled, frac)
     return eps
+
+
+def sampled_histogram(X, masks, q_ids, c_ids, rmax, n_bins: int):
+    """NEXT-2 oracle: per mask the histogram of D(q, c; mask) over the sampled
+    queries x sampled candidates (c != q by index), n_bins equal half-open bins [b w, (b+1) w) over
+    [0, rmax); pairs at or beyond rmax are not counted.  fp64, one distance at a time.
+    -> (hist int64 [n_masks][n_bins], distances list per mask for band checks)."""
+    X = np.ascontiguousarray(X, dtype=np.float32)
+    masks = np.asarray(masks, dtype=np.uint16)
+    q_ids = np.asarray(q_ids, dtype=np.int64)
+    c_ids = np.asarray(c_ids, dtype=np.int64)
+    hist = np.zeros((len(masks), n_bins), dtype=np.int64)
+    all_d = []
+    for mi, m in enumerate(masks):
+        ds = []
+        for q in q_ids:
+            row = dist_row(X, m, int(q))[c_ids]
+            ds.append(row[c_ids != q])
+        d = np.concatenate(ds)
+        all_d.append(d)
+        b = np.floor(d / float(rmax[mi]) * n_bins).astype(np.int64)
+        hist[mi] = np.bincount(b[b < n_bins], minlength=n_bins)[:n_bins]
+    return hist, all_d
+
+
+def eps_from_histogram(hist, rmax, N: int, pairs_per_mask: int, target_s: float):
+    """Cumulative histogram -> smallest bin edge whose mean neighbour count (selectivity s,
+    PAPER.md:221) reaches target_s; rmax if none does."""
+    hist = np.asarray(hist, dtype=np.float64)
+    eps = np.array(rmax, dtype=np.float64).copy()
+    for mi in range(hist.shape[0]):
+        mean = np.cumsum(hist[mi]) * (N - 1) / float(pairs_per_mask)
+        hit = np.flatnonzero(mean >= target_s)
+        if len(hit):
+            eps[mi] = float(rmax[mi]) * (hit[0] + 1) / hist.shape[1]
+    return eps

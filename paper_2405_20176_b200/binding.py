@@ -16,6 +16,7 @@ EXPORTED_SYMBOLS = [
     "snaps_rank_workspace_bytes", "snaps_rank_scores", "snaps_topn_overlap", "snaps_select_parameter",
     "snaps_knn_scores_at_k", "snaps_range_grid_workspace_bytes", "snaps_range_selfjoin_grid",
     "snaps_select_k_workspace_bytes", "snaps_knn_select_k",
+    "snaps_dist_hist_workspace_bytes", "snaps_sample_distance_histogram", "snaps_eps_from_histogram",
 ]
 
 _lib = None
@@ -74,6 +75,12 @@ def lib():
         L.snaps_range_grid_workspace_bytes.argtypes = [i64, i32, i32, i32]
         L.snaps_range_selfjoin_grid.restype = i32
         L.snaps_range_selfjoin_grid.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, vp, vp, vp, sz, vp]
+        L.snaps_dist_hist_workspace_bytes.restype = sz
+        L.snaps_dist_hist_workspace_bytes.argtypes = [i32, i32, i32]
+        L.snaps_sample_distance_histogram.restype = i32
+        L.snaps_sample_distance_histogram.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, i32, vp, i32, vp, vp, sz, vp]
+        L.snaps_eps_from_histogram.restype = i32
+        L.snaps_eps_from_histogram.argtypes = [vp, i32, i32, vp, i64, i64, ctypes.c_double, vp]
         L.snaps_select_k_workspace_bytes.restype = sz
         L.snaps_select_k_workspace_bytes.argtypes = [i64, i32]
         L.snaps_knn_select_k.restype = i32
@@ -368,3 +375,31 @@ def knn_select_k(knn_idx, knn_dist, k_grid, n_top: int, stream=None):
                                     _dptr(out["j_mean"]), _dptr(out["u"]), _dptr(ws), ws.numel(), _stream(stream)))
     out["_workspace"] = ws
     return out
+
+
+def sample_distance_histogram(X, masks, sample_q, sample_c, rmax, n_bins: int, stream=None):
+    """snaps_sample_distance_histogram -> int64 CUDA tensor [n_masks, n_bins]."""
+    import torch
+    m = _masks(masks)
+    q = np.ascontiguousarray(np.asarray(sample_q, dtype=np.int32))
+    c = np.ascontiguousarray(np.asarray(sample_c, dtype=np.int32))
+    r = np.ascontiguousarray(np.asarray(rmax, dtype=np.float32))
+    N, n_feat = X.shape
+    hist = torch.empty((len(m), n_bins), dtype=torch.int64, device=X.device)
+    ws = torch.empty(int(lib().snaps_dist_hist_workspace_bytes(len(q), len(c), len(m))), dtype=torch.uint8, device=X.device)
+    _check(lib().snaps_sample_distance_histogram(
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
+        q.ctypes.data_as(ctypes.c_void_p), len(q), c.ctypes.data_as(ctypes.c_void_p), len(c),
+        r.ctypes.data_as(ctypes.c_void_p), n_bins, _dptr(hist), _dptr(ws), ws.numel(), _stream(stream)))
+    return hist
+
+
+def eps_from_histogram(hist_host, rmax, N: int, pairs_per_mask: int, target_s: float) -> np.ndarray:
+    """snaps_eps_from_histogram on a host copy of the histogram -> fp32 [n_masks]."""
+    h = np.ascontiguousarray(np.asarray(hist_host, dtype=np.uint64))
+    r = np.ascontiguousarray(np.asarray(rmax, dtype=np.float32))
+    eps = np.empty(h.shape[0], dtype=np.float32)
+    _check(lib().snaps_eps_from_histogram(h.ctypes.data_as(ctypes.c_void_p), h.shape[0], h.shape[1],
+                                          r.ctypes.data_as(ctypes.c_void_p), N, pairs_per_mask, float(target_s),
+                                          eps.ctypes.data_as(ctypes.c_void_p)))
+    return eps

@@ -7,7 +7,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libsnaps.so")
-SOURCES = ["api.cu", "knn_lattice.cu", "range_lattice.cu", "misc_kernels.cu", "pivot_sort.cu", "ranking.cu", "range_grid.cu"]
+SOURCES = ["api.cu", "knn_lattice.cu", "range_lattice.cu", "misc_kernels.cu", "pivot_sort.cu", "ranking.cu", "range_grid.cu", "eps_search.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     # no implicit mul+add contraction: the kernels place their FMAs explicitly so that the

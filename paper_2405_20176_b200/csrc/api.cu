@@ -16,6 +16,7 @@
 #include "knn_lattice.cuh"
 #include "misc_kernels.cuh"
 #include "pivot_sort.cuh"
+#include "eps_search.cuh"
 #include "range_grid.cuh"
 #include "range_lattice.cuh"
 #include "ranking.cuh"
@@ -660,6 +661,53 @@ snaps_status snaps_range_selfjoin_grid(const float* d_X, int64_t N, int n_feat, 
     const bool prof = prof_begin(st);
     CUDA_TRY(snaps::range_grid_launch(p, grid, st));
     prof_end(prof, st);
+    return SNAPS_OK;
+}
+
+size_t snaps_dist_hist_workspace_bytes(int nq, int nc, int n_masks) {
+    if (nq < 1 || nc < 1 || n_masks < 1) return 0;
+    return snaps::dist_hist_workspace_bytes(nq, nc, n_masks);
+}
+
+snaps_status snaps_sample_distance_histogram(const float* d_X, int64_t N, int n_feat, int64_t ld,
+                                             const uint16_t* h_masks, int n_masks, const int32_t* h_sample_q,
+                                             int nq, const int32_t* h_sample_c, int nc, const float* h_rmax,
+                                             int n_bins, unsigned long long* out_hist, void* d_workspace,
+                                             size_t workspace_bytes, void* stream) {
+    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    if (rc) return rc;
+    if (!h_sample_q || !h_sample_c || !h_rmax || !out_hist || nq < 1 || nc < 1)
+        return fail(SNAPS_INVALID_ARG, "NULL or empty samples");
+    if (n_bins < 1 || n_bins > 8192) return fail(SNAPS_INVALID_ARG, "n_bins = %d outside 1..8192", n_bins);
+    for (int i = 0; i < nq; ++i)
+        if (h_sample_q[i] < 0 || h_sample_q[i] >= N) return fail(SNAPS_INVALID_ARG, "query sample id out of range");
+    for (int i = 0; i < nc; ++i)
+        if (h_sample_c[i] < 0 || h_sample_c[i] >= N) return fail(SNAPS_INVALID_ARG, "candidate sample id out of range");
+    for (int m = 0; m < n_masks; ++m)
+        if (!(h_rmax[m] > 0.f) || !isfinite(h_rmax[m])) return fail(SNAPS_INVALID_ARG, "rmax[%d] not finite and > 0", m);
+    if (!d_workspace || workspace_bytes < snaps::dist_hist_workspace_bytes(nq, nc, n_masks))
+        return fail(SNAPS_WORKSPACE_TOO_SMALL, "histogram workspace too small");
+    CUDA_TRY(snaps::dist_hist_launch(d_X, ld, n_feat, h_sample_q, nq, h_sample_c, nc, h_masks, h_rmax, n_masks,
+                                     n_bins, out_hist, d_workspace, static_cast<cudaStream_t>(stream)));
+    return SNAPS_OK;
+}
+
+snaps_status snaps_eps_from_histogram(const unsigned long long* h_hist, int n_masks, int n_bins, const float* h_rmax,
+                                      int64_t N, int64_t pairs_per_mask, double target_s, float* h_eps) {
+    if (!h_hist || !h_rmax || !h_eps || n_masks < 1 || n_bins < 1 || N < 2 || pairs_per_mask < 1 || !(target_s > 0.0))
+        return fail(SNAPS_INVALID_ARG, "bad arguments");
+    for (int m = 0; m < n_masks; ++m) {
+        unsigned long long cum = 0;
+        h_eps[m] = h_rmax[m];
+        for (int b = 0; b < n_bins; ++b) {
+            cum += h_hist[static_cast<size_t>(m) * n_bins + b];
+            const double mean = static_cast<double>(cum) * static_cast<double>(N - 1) / static_cast<double>(pairs_per_mask);
+            if (mean >= target_s) {
+                h_eps[m] = static_cast<float>(static_cast<double>(h_rmax[m]) * (b + 1) / n_bins);
+                break;
+            }
+        }
+    }
     return SNAPS_OK;
 }
 

@@ -1,0 +1,86 @@
+// eps_search.cu -- NEXT-2: the search radius for a target selectivity from a
+// sampled distance histogram.  "The distances between a sample of points and points within the
+// dataset are computed to create a histogram of distances between points.  Using this histogram,
+// a cumulative distance distribution histogram is computed which yields the relationship between
+// a search distance and the average number of neighbors" -- selectivity s = mean neighbours per
+// point, self excluded.  Device: the histogram of D(q, c; mask) over sampled
+// queries x sampled candidates (q != c) per mask.  Host: cumulative histogram -> radius.
+#include "eps_search.cuh"
+
+namespace snaps {
+
+__global__ void gather_rows_kernel(const float* __restrict__ X, int64_t ld, int n_feat,
+                                   const int32_t* __restrict__ ids, int n, float* __restrict__ out) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n * 16; i += gridDim.x * blockDim.x) {
+        const int r = i >> 4, j = i & 15;
+        out[i] = j < n_feat ? X[static_cast<int64_t>(ids[r]) * ld + j] : 0.f;
+    }
+}
+
+// grid = (n_masks, query chunks); one thread per (query of the chunk) loops over all candidates
+__global__ void dist_hist_kernel(const float* __restrict__ Xq, const int32_t* __restrict__ qid, int nq,
+                                 const float* __restrict__ Xc, const int32_t* __restrict__ cid, int nc,
+                                 const uint16_t* __restrict__ masks, const float* __restrict__ rmax, int n_bins,
+                                 unsigned long long* __restrict__ hist) {
+    extern __shared__ unsigned int sh[];
+    const int m = blockIdx.x;
+    for (int i = threadIdx.x; i < n_bins; i += blockDim.x) sh[i] = 0u;
+    __syncthreads();
+    const uint32_t mask = masks[m];
+    const float scale = static_cast<float>(n_bins) / rmax[m];
+    for (int qi = blockIdx.y * blockDim.x + threadIdx.x; qi < nq; qi += gridDim.y * blockDim.x) {
+        float q[15];
+#pragma unroll
+        for (int j = 0; j < 15; ++j) q[j] = Xq[qi * 16 + j];
+        const int my = qid[qi];
+        for (int ci = 0; ci < nc; ++ci) {
+            if (cid[ci] == my) continue;   // self excluded by index
+            const float* c = Xc + ci * 16;
+            float acc = 0.f;
+#pragma unroll
+            for (int j = 0; j < 15; ++j) {
+                const float diff = c[j] - q[j];
+                const float sq = __fmul_rn(diff, diff);
+                if ((mask >> j) & 1u) acc = __fadd_rn(acc, sq);
+            }
+            const float b = sqrtf(acc) * scale;
+            if (b < static_cast<float>(n_bins)) atomicAdd(&sh[static_cast<int>(b)], 1u);
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n_bins; i += blockDim.x)
+        if (sh[i]) atomicAdd(&hist[static_cast<size_t>(m) * n_bins + i], static_cast<unsigned long long>(sh[i]));
+}
+
+size_t dist_hist_workspace_bytes(int nq, int nc, int n_masks) {
+    auto al = [](size_t x) { return (x + 255) / 256 * 256; };
+    return al(static_cast<size_t>(nq) * 64) + al(static_cast<size_t>(nc) * 64) + al(static_cast<size_t>(nq) * 4) +
+           al(static_cast<size_t>(nc) * 4) + al(static_cast<size_t>(n_masks) * 2) + al(static_cast<size_t>(n_masks) * 4);
+}
+
+cudaError_t dist_hist_launch(const float* X, int64_t ld, int n_feat, const int32_t* h_q, int nq, const int32_t* h_c,
+                             int nc, const uint16_t* h_masks, const float* h_rmax, int n_masks, int n_bins,
+                             unsigned long long* out_hist, void* ws, cudaStream_t st) {
+    auto al = [](size_t x) { return (x + 255) / 256 * 256; };
+    unsigned char* p = static_cast<unsigned char*>(ws);
+    float* Xq = reinterpret_cast<float*>(p); p += al(static_cast<size_t>(nq) * 64);
+    float* Xc = reinterpret_cast<float*>(p); p += al(static_cast<size_t>(nc) * 64);
+    int32_t* dq = reinterpret_cast<int32_t*>(p); p += al(static_cast<size_t>(nq) * 4);
+    int32_t* dc = reinterpret_cast<int32_t*>(p); p += al(static_cast<size_t>(nc) * 4);
+    uint16_t* dm = reinterpret_cast<uint16_t*>(p); p += al(static_cast<size_t>(n_masks) * 2);
+    float* dr = reinterpret_cast<float*>(p);
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(dq, h_q, sizeof(int32_t) * nq, cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(dc, h_c, sizeof(int32_t) * nc, cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(dm, h_masks, sizeof(uint16_t) * n_masks, cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(dr, h_rmax, sizeof(float) * n_masks, cudaMemcpyHostToDevice, st)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(out_hist, 0, sizeof(unsigned long long) * static_cast<size_t>(n_masks) * n_bins, st)) != cudaSuccess) return e;
+    gather_rows_kernel<<<(nq * 16 + 255) / 256, 256, 0, st>>>(X, ld, n_feat, dq, nq, Xq);
+    gather_rows_kernel<<<(nc * 16 + 255) / 256, 256, 0, st>>>(X, ld, n_feat, dc, nc, Xc);
+    const int chunks = (nq + 127) / 128 < 16 ? (nq + 127) / 128 : 16;
+    dist_hist_kernel<<<dim3(n_masks, chunks), 128, static_cast<size_t>(n_bins) * 4, st>>>(Xq, dq, nq, Xc, dc, nc, dm, dr,
+                                                                                         n_bins, out_hist);
+    return cudaGetLastError();
+}
+
+}  // namespace snaps

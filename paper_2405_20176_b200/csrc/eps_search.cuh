@@ -1,0 +1,13 @@
+// eps_search.cuh -- NEXT-2: sampled distance histogram per mask (device part of the eps search).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace snaps {
+
+size_t dist_hist_workspace_bytes(int nq, int nc, int n_masks);
+cudaError_t dist_hist_launch(const float* X, int64_t ld, int n_feat, const int32_t* h_q, int nq, const int32_t* h_c,
+                             int nc, const uint16_t* h_masks, const float* h_rmax, int n_masks, int n_bins,
+                             unsigned long long* out_hist, void* ws, cudaStream_t st);
+
+}  // namespace snaps

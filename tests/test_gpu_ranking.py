@@ -174,3 +174,39 @@ def test_select_k_pipeline_matches_oracle(snaps):
     assert (u[0][0] == 1.0).all() and (u[1][-1] == 1.0).all() and (u[2][0] == 1.0).all() and (u[3][-1] == 1.0).all()
     with pytest.raises(snaps.SnapsError):
         snaps.knn_select_k(join["idx"], join["dist"], [4, 2, 8], n)
+
+
+def test_sampled_distance_histogram_and_eps_search(snaps):
+    """NEXT-2: device histogram of sampled pair distances against the oracle's,
+    bin by bin (pairs within 1e-6 relative of a bin edge may fall on either side: fp32 vs fp64),
+    and the radius for a target selectivity from its cumulative form."""
+    import torch
+    from oracle.calibrate import sampled_histogram, eps_from_histogram
+    N = 4000
+    X = workloads.make_table(N, 37, outlier_frac=0.01)
+    masks = np.array([0b11, 0x7FFF, (1 << 9) | (1 << 3) | 1, 0b1111000], dtype=np.uint16)
+    rng = np.random.default_rng(5)
+    q = np.sort(rng.choice(N, 300, replace=False)).astype(np.int32)
+    c = np.sort(rng.choice(N, 1500, replace=False)).astype(np.int32)
+    rmax = np.array([0.05, 0.6, 0.2, 0.3], dtype=np.float32)
+    n_bins = 256
+    hist = snaps.sample_distance_histogram(_t(X), masks, q, c, rmax, n_bins)
+    torch.cuda.synchronize()
+    g = hist.cpu().numpy()
+    ref, dists = sampled_histogram(X, masks, q, c, rmax, n_bins)
+    for mi in range(len(masks)):
+        edges = np.arange(1, n_bins + 1) * (float(rmax[mi]) / n_bins)
+        d = dists[mi]
+        # cumulative counts may differ by the pairs inside the band around each edge
+        lo = np.array([(d < e * (1 - 1e-6)).sum() for e in edges])
+        hi = np.array([(d < e * (1 + 1e-6)).sum() for e in edges])
+        cum = np.cumsum(g[mi])
+        assert (lo <= cum).all() and (cum <= hi).all()
+        assert np.abs(g[mi] - ref[mi]).sum() <= 2 * (hi - lo).sum()
+    pairs = int(sum(len(c) - int(qq in set(c.tolist())) for qq in q))
+    e_dev = snaps.eps_from_histogram(g, rmax, N, pairs, 20.0)
+    e_ref = eps_from_histogram(ref, rmax, N, pairs, 20.0)
+    assert np.abs(e_dev - e_ref).max() <= (rmax / n_bins).max() * 1.001        # at most one bin apart
+    # the radius does what it is for: the eps-join at it finds about the target number of neighbours
+    cnt = snaps.range_selfjoin(_t(X), masks, e_dev)["count"].float().mean(dim=1).cpu().numpy()
+    assert (cnt > 10).all() and (cnt < 40).all()

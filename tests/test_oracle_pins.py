@@ -256,3 +256,22 @@ def test_oracle_rejects_bad_arguments(oracle_mod):
         oracle_mod.knn_selfjoin(X, [0b1000], 2)           # bit >= n_feat
     with pytest.raises(ValueError):
         oracle_mod.range_selfjoin(X, [0b1], [0.0])        # eps > 0
+
+
+# ---------------------------------------------------------------- NEXT-2: sampled distance histogram
+def test_sampled_histogram_closed_form_and_selectivity(oracle_mod):
+    from oracle.calibrate import sampled_histogram, eps_from_histogram
+    n, h = 64, 2.0 ** -7
+    X = workloads.lattice_table(n, 3, h, seed=2)
+    ids = np.arange(n)
+    # 1-D lattice, all points sampled: |i-j| h for i != j -> 2 (n - r) ordered pairs at distance r h
+    hist, _ = sampled_histogram(X, [0b001], ids, ids, [n * h], n)          # bin width = h, bin r holds r h
+    assert hist[0, 0] == 0 and all(hist[0, r] == 2 * (n - r) for r in range(1, n))
+    # with every object sampled the cumulative histogram IS the eps-join: sum of counts at radius
+    # just below a bin edge (open bins, closed ball: keep eps off the lattice distances)
+    cnt, _, _ = oracle_mod.range_selfjoin(X, [0b001], [4.5 * h])
+    assert hist[0, :5].sum() == cnt[0].sum()
+    # selectivity: mean neighbours = cum * (N-1) / pairs; target 6 -> first edge reaching it
+    eps = eps_from_histogram(hist, [n * h], n, n * (n - 1), 6.0)
+    mean_at = lambda r: oracle_mod.range_selfjoin(X, [0b001], [r])[0].mean()
+    assert mean_at(eps[0] * (1 - 1e-9)) >= 6.0 > mean_at((eps[0] - h) * (1 - 1e-9))
