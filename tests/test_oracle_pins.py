@@ -72,6 +72,21 @@ def test_lattice_closed_form(oracle_mod):
         others = sorted((abs(i - j) * h, j) for j in range(n) if j != i)[:k]
         assert idx[0, i].tolist() == [j for _, j in others]
         assert dist[0, i].tolist() == [d for d, _ in others]
+    # in-degree: object j counts the queries i whose list holds j.  Closed form on
+    # the lattice from the id lists derived above (NOT from the oracle's own idx): interior
+    # objects are listed by their k nearest lattice sites (k), the sites near a boundary also by
+    # the boundary queries whose lists are one-sided -- in-degree != out-degree there.
+    exp_indeg = np.zeros(n, dtype=np.int64)
+    for i in range(n):
+        for _, j in sorted((abs(i - j) * h, j) for j in range(n) if j != i)[:k]:
+            exp_indeg[j] += 1
+    assert indeg[0].tolist() == exp_indeg.tolist()
+    # written out: site j <= k is listed by k/2 + j queries (the one-sided lists of the first k/2
+    # queries pile up on sites 0..k), sites k < j < n-1-k by exactly k, mirrored at the far end
+    closed = np.full(n, k)
+    closed[:k + 1] = k // 2 + np.arange(k + 1)
+    closed[n - k - 1:] = (k // 2 + np.arange(k + 1))[::-1]
+    assert indeg[0].tolist() == closed.tolist()
     interior = np.arange(k // 2, n - k // 2)
     assert (kth[0, interior] == (k // 2) * h).all()
     np.testing.assert_allclose(mean[0, interior], h * (k / 2 + 1) / 2, rtol=1e-15)
@@ -82,6 +97,32 @@ def test_lattice_closed_form(oracle_mod):
     # closed ball (reading A2): eps exactly on a lattice distance includes it
     cnt2, _, _ = oracle_mod.range_selfjoin(X, [0b001], [2.0 * h])
     assert (cnt2[0, 2:-2] == 4).all()
+
+
+def test_indegree_asymmetric_hand_example(oracle_mod):
+    # Four collinear objects at x = 0, 1, 2, 10 (scaled into [0,1]), k = 1.  Nearest neighbours by
+    # hand: 0 -> 1, 1 -> 0 (tie |1-0| = |1-2| goes to the smaller id, reading A3), 2 -> 1, 3 -> 2.
+    # In-degree ("number of occurrences that a point is found within another point's
+    # set of kNN") = {1, 2, 1, 0}: differs from the out-degree k = 1 of every object, so an
+    # accumulation at the query index instead of the neighbour id cannot pass.  Table 2's own
+    # in-degree column (5,6,6,3,2,3,2,2,1,0 for k = 3) shows the same asymmetry.
+    X = (np.array([[0.0], [1.0], [2.0], [10.0]]) / 16.0).astype(np.float32)
+    idx, dist = oracle_mod.knn_selfjoin(X, [0b1], 1)
+    assert idx[0, :, 0].tolist() == [1, 0, 1, 2]
+    kth, mean, indeg = oracle_mod.knn_scores(4, idx, dist)
+    assert indeg[0].tolist() == [1, 2, 1, 0]
+    assert kth[0].tolist() == [1 / 16, 1 / 16, 1 / 16, 8 / 16]
+    # k = 2: 0 -> {1,2}, 1 -> {0,2}, 2 -> {1,0}, 3 -> {2,1}
+    idx2, dist2 = oracle_mod.knn_selfjoin(X, [0b1], 2)
+    assert idx2[0].tolist() == [[1, 2], [0, 2], [1, 0], [2, 1]]
+    _, mean2, indeg2 = oracle_mod.knn_scores(4, idx2, dist2)
+    assert indeg2[0].tolist() == [2, 3, 3, 0]
+    assert mean2[0].tolist() == [1.5 / 16, 1 / 16, 1.5 / 16, 8.5 / 16]
+    # the k-grid helper of the ranking oracle reads the same lists
+    from oracle import ranking
+    _, _, g1 = ranking.knn_scores_at_k(idx2[0], dist2[0], 1, 4)
+    _, _, g2 = ranking.knn_scores_at_k(idx2[0], dist2[0], 2, 4)
+    assert g1.tolist() == [1, 2, 1, 0] and g2.tolist() == [2, 3, 3, 0]
 
 
 # ---------------------------------------------------------------- hypercube (closed form B, ties)
