@@ -5,16 +5,25 @@ A step = one pass of the whole hot path over one syn
 SNAPShot1-shaped table: stage the N x 15 fp32 table, plan the 32,752 subspace masks into
 sub-lattice batches, per-pair squared differences, add-only subset sums, per-(query, subspace)
 top-k selection, and the fused per-object outlier scores (k-th distance, mean kNN distance,
-kNN-graph in-degree).  `value` is timed with inputs resident in HBM; `e2e` goes through the
-public host-buffer call with the H2D of the table and the D2H of the scores inside the timed
-region.  Multi-GPU: every rank joins its own catalogue (seed 1 + rank) -- the path has no
-exchange step, so scaling is "weak" and there is no collective on the data path.
+kNN-graph in-degree).  `value` is timed with inputs resident in HBM; `e2e` is ONE C-ABI call with
+host buffers (pinned table in, pinned scores out; both copies inside the timed region).
+
+The default line also carries `dssj` (config 3: the eps range self-join over all 32,752 subspaces),
+`lsst_scale` (config 4: N = 1,000,000 through the grid engine, outputs streamed to pinned host)
+and `cpu_baseline` (the fp64 oracle on the host cores).  `--config c5_lsst_oversub` runs config 5
+(N = 5,000,000, 256 sampled masks, kNN k=16 + DSSJ, outputs through the recycling sink).
+
+Multi-GPU (`--gpus N` under torchrun): ONE catalogue, replicated; the mask list is dealt to the
+ranks by sub-lattice batch (`sharding.shard_masks`), no data-path collective --
+strong scaling.  `--scaling weak` gives every rank its own catalogue instead.  Configs 4-5 shard
+by query range; the only exchange is the sum of the in-degree rows.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config NAME]
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -32,15 +41,12 @@ import workloads  # noqa: E402
 
 METRIC = "subspaces/sec and pair-distance evals/sec (kNNSJ N=31,693,k=10); % FP32 peak"
 UNIT = "subspaces/s"
-
-# Roofline denominator: the path is bound by plain FP32/ALU issue, so the
-# peak is derived from unit counts and clocks: 148 SMs x 128 FP32 lanes x 1.965 GHz lane-ops/s
-# (one FADD, FMUL, FSUB, FFMA or FP32 compare = one lane-op; an FMA-counts-2 "FP32 peak" is twice
-# this number in FLOP/s, which an add-and-compare workload cannot reach by construction).
 N_SM, LANES_PER_SM = 148, 128
+KERNEL_SOURCES = ("paper_2405_20176_b200/csrc/knn_lattice.cu", "paper_2405_20176_b200/csrc/snaps_device.cuh")
 
 
-def peaks():
+def derived_peak():
+    """148 SMs x 128 FP32 lanes x max SM clock, lane-ops/s (context beside the measured FFMA rate)."""
     sm_max_mhz = 1965.0
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -48,6 +54,27 @@ def peaks():
     except OSError:
         pass
     return N_SM * LANES_PER_SM * sm_max_mhz * 1e6, sm_max_mhz
+
+
+def kernel_source_sha():
+    h = hashlib.sha256()
+    for rel in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, rel), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def stored_traffic():
+    """DRAM bytes per launch from the committed ncu capture -- only if it was taken from the kernel
+    source as it stands (profiles/traffic.json carries the hash of the kernel files)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            t = json.load(f)
+    except OSError:
+        return None, "profiles/traffic.json missing"
+    if t.get("kernel_source_sha") != kernel_source_sha():
+        return None, "profiles/traffic.json is stale (kernel source changed since the ncu capture)"
+    return t.get("knn_lattice_kernel_dram_bytes_per_launch"), t.get("source")
 
 
 def stratified_masks(masks, per_dim, seed):
@@ -107,7 +134,7 @@ def run_reference(args, rank):
 
 def workload_name(cfg, n_masks):
     return (f"{cfg.name}: kNNSJ k={cfg.k} over N={cfg.n} x {cfg.n_feat} fp32 (SNAPShot1-shaped, "
-            f"seed {cfg.seed}+rank), all {n_masks} subspaces of 2-15 features, scores kth/mean/indeg")
+            f"seed {cfg.seed}), all {n_masks} subspaces of 2-15 features, scores kth/mean/indeg")
 
 
 class ClockSampler:
@@ -153,101 +180,248 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
-def run_lsst(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks, emit=True):
-    """Extra line for the LSST-scale config (BASELINE.json configs[3]): N=1,000,000, the 105
-    two-feature subspaces + the full space, k=10, lists and scores streamed to pinned host memory
-    (`snaps_knn_selfjoin_streamed`; the pivot sweep prunes the scan exactly).  `value` here is end
-    to end by construction (device -> pinned host copies inside the timed region)."""
-    X = workloads.make_table(cfg.n, cfg.seed + rank, cols=list(range(cfg.n_feat)), outlier_frac=0.001)
+class Dist:
+    """torch.distributed plumbing of one run (NCCL for barriers, the max over ranks and the
+    in-degree sum; no collective touches the join itself)."""
+
+    def __init__(self, torch, dist, dev, rank, world):
+        self.torch, self.dist, self.dev, self.rank, self.world = torch, dist, dev, rank, world
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+
+    def max_over_ranks(self, x):
+        if self.world == 1:
+            return x
+        t = self.torch.tensor([x], dtype=self.torch.float64, device=self.dev)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(self, x):
+        if self.world == 1:
+            return x
+        t = self.torch.tensor([x], dtype=self.torch.float64, device=self.dev)
+        self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM)
+        return float(t.item())
+
+
+def measured_peak(snaps, local_rank):
+    """FFMA / FADD / FADD+FSETP lane-op rates of the in-library probes, with the clocks seen during them."""
+    sampler = ClockSampler(local_rank)
+    kinds = {"ffma": 0, "fadd": 1, "fadd+fsetp": 2, "ffma_3reg": 3, "ffma2_packed": 4, "fadd2_packed": 5}
+    rates = {name: 0.0 for name in kinds}
+    for _ in range(3):          # a second of probes so that the 200 ms clock sampler sees them
+        for name, kind in kinds.items():
+            rates[name] = max(rates[name], snaps.probe_fp32_rate(kind))
+    return rates, sampler.stop()
+
+
+def alu_roofline(kernel, evals, n_batches, N, k_ms, peak_meas, peak_der, sm_max, probes, probe_clocks):
+    """bound = plain FP32/ALU issue.  achieved = algorithmic lane-ops / kernel time; peak = the measured
+    FFMA lane-op rate.  frac_evals_only drops the per-(pair, batch) term, which depends on the batch size."""
+    lane_ops = 2.0 * evals + 30.0 * float(N) * N * n_batches
+    achieved = lane_ops / (k_ms * 1e-3)
+    return {
+        "bound": "alu", "kernel": kernel, "achieved": achieved / 1e12, "peak": peak_meas / 1e12,
+        "unit": "TFLOP/s", "frac": achieved / peak_meas,
+        "frac_evals_only": 2.0 * evals / (k_ms * 1e-3) / peak_meas,
+        "peak_source": "measured: snaps_probe_fp32_rate FFMA lane-ops/s on this GPU during this run (one FFMA = 1 lane-op)",
+        "peak_derived": peak_der / 1e12,
+        "peak_derived_source": f"{N_SM} SMs x {LANES_PER_SM} FP32 lanes x {sm_max:.0f} MHz",
+        "frac_of_fma2_peak": achieved / (2 * peak_meas),
+        "probe_lane_ops_per_s": probes, "probe_clocks": probe_clocks,
+        "kernel_ms": k_ms, "algorithmic_lane_ops_per_launch": lane_ops,
+        "evals_per_s_kernel": evals / (k_ms * 1e-3),
+        "note": "effective figure: algorithmic lane-ops (2 per (pair, subspace) evaluation + 30 per pair and batch) / "
+                "kernel time.  The kernel reaches the exact result with fewer executed operations (lower-bound filter); "
+                "executed-instruction and pipe figures (issue-slot, ALU, FMA utilisation) are in profiles/ (see profiles/README.md)",
+    }
+
+
+def run_lsst(args, cfg, snaps, torch, D, steps, emit=True):
+    """LSST-scale config (BASELINE.json configs[3]): N=1,000,000, the 105 two-feature subspaces + the
+    full space, k=10, lists and scores streamed to pinned host memory through the grid engine.
+    Multi-GPU: query ranges (`sharding.shard_queries`), in-degree rows summed over ranks."""
+    from paper_2405_20176_b200.sharding import shard_queries
+    X = workloads.make_table(cfg.n, cfg.seed, cols=list(range(cfg.n_feat)), outlier_frac=0.001)
     masks = cfg.masks()
     N, n_masks, k = len(X), len(masks), cfg.k
-    Xd = torch.from_numpy(X).to(dev)
-    mpb = 53   # two groups: the second group's join overlaps the first group's copy-out
-    out = snaps.knn_selfjoin_streamed(Xd, masks, k, mpb, lists=True)
+    q0, q1 = shard_queries(N, D.rank, D.world)
+    Xd = torch.from_numpy(X).to(D.dev)
+    mpb = 27   # four groups: a group's join overlaps the previous group's copy-out
+    out = snaps.knn_selfjoin_streamed(Xd, masks, k, mpb, lists=True, q_range=(q0, q1))
     torch.cuda.synchronize()
     ws = out.pop("_workspace")
-    steps = max(1, min(args.steps, 2))
-    barrier()
+    snaps.profile_enable(True)
+    D.barrier()
+    sampler = ClockSampler(D.dev.index or 0) if D.rank == 0 else None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kernel_ms = []
     ev0.record()
     for _ in range(steps):
-        snaps.knn_selfjoin_streamed(Xd, masks, k, mpb, lists=True, out=out, workspace=ws)
+        snaps.knn_selfjoin_streamed(Xd, masks, k, mpb, lists=True, out=out, workspace=ws, q_range=(q0, q1))
+        torch.cuda.current_stream().synchronize()
+        kernel_ms.append(snaps.profile_last_kernel_ms()[0])
+        if D.world > 1:     # the one exchange of query-range sharding: in-degree rows add up (SURVEY 8(e)(ii))
+            ind = out["indeg"].to(D.dev, non_blocking=True)
+            D.dist.all_reduce(ind)
     ev1.record()
     torch.cuda.synchronize()
-    barrier()
-    ms = max_over_ranks(ev0.elapsed_time(ev1) / steps)
-    assert int(out["indeg"][0].sum().item()) == N * k
-    if rank == 0:
-        evals = float(N) * N * n_masks
-        d2h = int(sum(t.numel() * t.element_size() for t in out.values()))
-        line = ({
-            "metric": "subspaces/sec (kNNSJ N=1,000,000, k=10, 105 pair subspaces + full space, pivot sweep)",
-            "value": world * n_masks / (ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": 1,
-            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-            "data": "synthetic",
-            "config": {"workload": f"{cfg.name}: kNNSJ k={k} over N={N} x 15 (LSST-scale, seed {cfg.seed}+rank), "
-                                   f"{n_masks} subspaces, lists + scores to pinned host in groups of {mpb} masks"},
-            "effective_evals_per_s": world * evals / (ms * 1e-3),
-            "note": "exactly pruned scan: effective evals = N^2 x masks / time, not operations performed",
-            "e2e": {"value": world * n_masks / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0,
-                    "d2h_bytes_per_step": d2h},
-            "paper_context": "paper, LSST5M (N=5e6, k_max=256): ~100 s per feature space on 1xA100 (Table 4)"})
-        if emit:
-            print(json.dumps(line), flush=True)
-        return line
-    return None
+    D.barrier()
+    clocks = sampler.stop() if sampler else None
+    ms = D.max_over_ranks(ev0.elapsed_time(ev1) / steps)
+    tot = D.sum_over_ranks(float(out["indeg"][0].sum().item()))
+    assert int(tot) == N * k, (tot, N * k)
+    if D.rank != 0:
+        return None
+    evals = float(N) * N * n_masks
+    d2h = int(sum(t.numel() * t.element_size() for t in out.values())) * D.world
+    line = {
+        "metric": "subspaces/sec (kNNSJ N=1,000,000, k=10, 105 pair subspaces + full space, grid engine)",
+        "value": n_masks / (ms * 1e-3), "unit": UNIT, "n_gpus": D.world, "steps": steps, "warmup": 1,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: kNNSJ k={k} over N={N} x 15 (LSST-scale, seed {cfg.seed}), "
+                               f"{n_masks} subspaces, lists + scores to pinned host in groups of {mpb} masks",
+                   "sharding": "query ranges over ranks; in-degree rows all-reduced" if D.world > 1 else "none"},
+        "effective_evals_per_s": evals / (ms * 1e-3),
+        "join_kernel_ms": float(np.mean(kernel_ms)),
+        "note": "exactly pruned scan (grid index per subspace): effective evals = N^2 x masks / time, not operations performed",
+        "e2e": {"value": n_masks / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": d2h},
+        "clocks": clocks,
+        "paper_context": "paper, LSST5M (N=5e6, k_max=256): ~100 s per feature space on 1xA100 (Table 4)"}
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
 
 
-def run_range(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks):
-    """Extra line for the DSSJ config (BASELINE.json configs[2]): one pass of snaps_range_selfjoin
-    over all masks with the stored eps_d of the configuration (workloads/config_eps.json).
-    Not the headline metric; printed with the same keys so that the numbers in DESIGN.md can be
-    reproduced with `python bench.py --config c3_snapshot1_dssj`."""
-    X = workloads.make_table(cfg.n, cfg.seed + rank, cols=list(range(cfg.n_feat)), outlier_frac=0.01)
-    masks = cfg.masks()
-    eps = workloads.config_eps(cfg.name, masks)        # stored inputs (oracle/write_config_eps.py)
-    if args.profile_masks > 0:      # profiling aid, see --profile-masks
-        sl = slice(args.profile_offset, args.profile_offset + args.profile_masks)
-        masks, eps = masks[sl], eps[sl]
-    N, n_masks = len(X), len(masks)
-    Xd = torch.from_numpy(X).to(dev)
+def run_range(args, cfg, snaps, torch, D, steps, warmup, peakinfo, emit=True):
+    """DSSJ config (BASELINE.json configs[2]): snaps_range_selfjoin over all masks with the stored
+    eps_d of the configuration (workloads/config_eps.json)."""
+    from paper_2405_20176_b200.sharding import shard_masks
+    X = workloads.make_table(cfg.n, cfg.seed, cols=list(range(cfg.n_feat)), outlier_frac=0.01)
+    masks_all = cfg.masks()
+    eps_all = workloads.config_eps(cfg.name, masks_all)        # stored inputs (oracle/write_config_eps.py)
+    mine = shard_masks(masks_all, D.rank, D.world)
+    masks, eps = masks_all[mine], eps_all[mine]
+    N, n_masks = len(X), len(masks_all)
+    Xd = torch.from_numpy(X).to(D.dev)
     out = snaps.range_selfjoin(Xd, masks, eps)
     ws = out.pop("_workspace")
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=D.dev)
     snaps.profile_enable(True)
 
     def step():
         flush.zero_()
         snaps.range_selfjoin(Xd, masks, eps, out=out, workspace=ws)
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     torch.cuda.synchronize()
-    barrier()
+    D.barrier()
+    sampler = ClockSampler(D.dev.index or 0) if D.rank == 0 else None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     kernel_ms = []
     ev0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
         kernel_ms.append(snaps.profile_last_kernel_ms()[0])
     ev1.record()
     torch.cuda.synchronize()
-    barrier()
-    ms = max_over_ranks(ev0.elapsed_time(ev1) / args.steps)
-    if rank == 0:
-        evals = float(N) * N * n_masks
-        peak, _ = peaks()
-        lane_ops = 2.0 * evals + 30.0 * float(N) * N * 512
-        print(json.dumps({
-            "metric": "subspaces/sec (DSSJ N=31,693, eps_d for ~50 neighbours)", "value": world * n_masks / (ms * 1e-3),
-            "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": f"{cfg.name}: DSSJ over N={N} x 15, all {n_masks} subspaces, counts + sums + means"},
-            "evals_per_s": world * evals / (ms * 1e-3), "mean_neighbours": float(out["count"].float().mean().item()),
-            "roofline": {"bound": "alu", "kernel": "range_lattice_kernel", "achieved": lane_ops / (np.mean(kernel_ms) * 1e-3) / 1e12,
-                         "peak": peak / 1e12, "unit": "TFLOP/s", "frac": lane_ops / (np.mean(kernel_ms) * 1e-3) / peak,
-                         "traffic": None, "kernel_ms": float(np.mean(kernel_ms))},
-            "gpu_launches": 4 * args.steps}), flush=True)
+    D.barrier()
+    clocks = sampler.stop() if sampler else None
+    ms = D.max_over_ranks(ev0.elapsed_time(ev1) / steps)
+    if D.rank != 0:
+        return None
+    evals = float(N) * N * len(masks)            # this rank's share (the kernel time is this rank's)
+    n_batches = float(snaps.planned_evals(N, X.shape[1], masks)) / (64.0 * N * N)
+    line = {
+        "metric": "subspaces/sec (DSSJ N=31,693, eps_d for ~50 neighbours)", "value": n_masks / (ms * 1e-3),
+        "unit": UNIT, "n_gpus": D.world, "steps": steps, "warmup": warmup, "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: DSSJ over N={N} x 15 (seed {cfg.seed}), all {n_masks} subspaces, counts + sums + means",
+                   "l2": "256 MB flush fill before every step"},
+        "evals_per_s": float(N) * N * n_masks / (ms * 1e-3),
+        "mean_neighbours": float(out["count"].float().mean().item()),
+        "roofline": alu_roofline("range_lattice_kernel", evals, n_batches, N, float(np.mean(kernel_ms)), *peakinfo),
+        "gpu_launches": 4 * steps, "clocks": clocks}
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
+
+
+def run_c5(args, cfg, snaps, torch, D):
+    """Config 5 (BASELINE.json configs[4]): N=5,000,000 x 15, 256 subspace masks sampled from the 32,752,
+    kNNSJ k=16 plus DSSJ (eps_d for ~100 neighbours), outputs through the recycling sink (two pinned host
+    buffers; the consumer checksums each group and the buffer is reused) -- the lists (164 GB) never
+    exist anywhere at once.  One pass each (minutes); --c5-n reduces N for quick runs."""
+    from paper_2405_20176_b200.sharding import shard_queries
+    n = args.c5_n or cfg.n
+    X = workloads.make_table(n, cfg.seed, cols=list(range(cfg.n_feat)), outlier_frac=0.001)
+    masks = cfg.masks()
+    if args.c5_masks:
+        masks = masks[:args.c5_masks]
+    N, n_masks, k = len(X), len(masks), cfg.k
+    q0, q1 = shard_queries(N, D.rank, D.world)
+    Xd = torch.from_numpy(X).to(D.dev)
+    mpb = 4
+    acc = {"kth": 0.0, "indeg": 0, "groups": 0, "idx_xor": 0, "count": 0, "bytes": 0}
+
+    def consume_knn(m0, m1, arrays):
+        acc["groups"] += 1
+        acc["kth"] += float(arrays["kth"].sum(dtype=np.float64))
+        acc["indeg"] += int(arrays["indeg"].sum(dtype=np.int64))
+        acc["idx_xor"] ^= int(np.bitwise_xor.reduce(arrays["idx"][:, ::997].ravel()))
+        acc["bytes"] += sum(a.nbytes for a in arrays.values())
+
+    def consume_range(m0, m1, arrays):
+        acc["count"] += int(arrays["count"].sum(dtype=np.int64))
+        acc["bytes"] += sum(a.nbytes for a in arrays.values())
+
+    # radii for ~100 neighbours: the library's own sampled-histogram search (NEXT-2) on the device
+    eps = snaps.eps_for_selectivity(Xd, masks, cfg.target_neighbours, seed=cfg.seed)
+    snaps.profile_enable(True)
+    D.barrier()
+    sampler = ClockSampler(D.dev.index or 0) if D.rank == 0 else None
+    t = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    t[0].record()
+    ws = snaps.knn_selfjoin_sink(Xd, masks, k, mpb, consume_knn, want=("idx", "dist", "kth", "mean", "indeg"),
+                                 q_range=(q0, q1))
+    knn_kernel_ms = snaps.profile_last_kernel_ms()[0]
+    t[1].record()
+    snaps.range_selfjoin_sink(Xd, masks, eps, mpb, consume_range, q_range=(q0, q1), workspace=ws)
+    rng_kernel_ms = snaps.profile_last_kernel_ms()[0]
+    t[2].record()
+    torch.cuda.synchronize()
+    D.barrier()
+    clocks = sampler.stop() if sampler else None
+    knn_ms = D.max_over_ranks(t[0].elapsed_time(t[1]))
+    rng_ms = D.max_over_ranks(t[1].elapsed_time(t[2]))
+    indeg = D.sum_over_ranks(float(acc["indeg"]))
+    cnt = D.sum_over_ranks(float(acc["count"]))
+    assert int(indeg) == N * k * n_masks, (indeg, N * k * n_masks)       # PAPER.md:136 over every mask
+    if D.rank != 0:
+        return
+    evals = float(N) * N * n_masks
+    print(json.dumps({
+        "metric": "subspaces/sec (kNNSJ k=16 + DSSJ ~100 neighbours, N=5,000,000, 256 sampled subspaces, grid engine, sink)",
+        "value": n_masks / ((knn_ms + rng_ms) * 1e-3), "unit": UNIT, "n_gpus": D.world, "steps": 1, "warmup": 0,
+        "ms_per_step": knn_ms + rng_ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: N={N} x 15 (seed {cfg.seed}), {n_masks} masks sampled from the 32,752 (seed 4), "
+                               f"kNNSJ k={k} (lists + scores) then DSSJ (counts, sums, means), groups of {mpb} masks "
+                               "through two recycled pinned host buffers"},
+        "knn": {"ms": knn_ms, "subspaces_per_s": n_masks / (knn_ms * 1e-3), "effective_evals_per_s": evals / (knn_ms * 1e-3),
+                "join_kernel_ms": knn_kernel_ms, "s_per_subspace": knn_ms * 1e-3 / n_masks},
+        "dssj": {"ms": rng_ms, "subspaces_per_s": n_masks / (rng_ms * 1e-3), "effective_evals_per_s": evals / (rng_ms * 1e-3),
+                 "join_kernel_ms": rng_kernel_ms, "mean_neighbours": cnt / (float(N) * n_masks)},
+        "e2e": {"value": n_masks / ((knn_ms + rng_ms) * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": int(acc["bytes"]) * D.world},
+        "sink": {"groups": acc["groups"], "kth_checksum": acc["kth"], "idx_xor": acc["idx_xor"]},
+        "clocks": clocks,
+        "paper_context": "paper, LSST5M on 1xA100 (k_max=256, s_max=256): kNNSJ ~100 s, DSSJ ~24 s per feature space (Table 4)",
+    }), flush=True)
 
 
 def main():
@@ -257,18 +431,17 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="snaps", choices=["snaps", "reference"])
     ap.add_argument("--config", default="c2_snapshot1_knn")
+    ap.add_argument("--scaling", default="strong", choices=["strong", "weak"],
+                    help="N > 1: strong = one catalogue, masks dealt to ranks; weak = one catalogue per rank")
     ap.add_argument("--ref-queries", type=int, default=1024,
                     help="sampled queries per step of --impl reference")
     ap.add_argument("--cpu-queries", type=int, default=4096,
                     help="sampled queries of the cpu_baseline leg (0 = skip)")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-lsst", action="store_true",
-                    help="skip the LSST-scale leg (config 4, N=1,000,000) that the default run reports beside config 2")
-    ap.add_argument("--profile-masks", type=int, default=0,
-                    help="profiling aid (ncu --set full replays every launch ~40x): keep only the "
-                         "first M masks; the JSON line is then marked profile_only and is NOT a bench value")
-    ap.add_argument("--profile-offset", type=int, default=0,
-                    help="with --profile-masks: index of the first mask kept")
+    ap.add_argument("--no-lsst", action="store_true", help="skip the LSST-scale leg (config 4) of the default run")
+    ap.add_argument("--no-dssj", action="store_true", help="skip the DSSJ leg (config 3) of the default run")
+    ap.add_argument("--c5-n", type=int, default=0, help="config 5 with a reduced N (quick runs)")
+    ap.add_argument("--c5-masks", type=int, default=0, help="config 5 on its first M masks only (quick runs)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -281,44 +454,48 @@ def main():
     import torch
     import torch.distributed as dist
     import paper_2405_20176_b200 as snaps
+    from paper_2405_20176_b200.sharding import shard_masks
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback exists)"
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # the communicator log shows the ranks
         dist.init_process_group("nccl", device_id=dev)
     snaps.lib()
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    D = Dist(torch, dist, dev, rank, world)
 
     cfg = workloads.get_config(args.config)
-    if cfg.join == "knn" and cfg.n >= 100000:
-        run_lsst(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks)
+    probes, probe_clocks = measured_peak(snaps, local_rank)
+    peak_der, sm_max = derived_peak()
+    peakinfo = (probes["ffma"], peak_der, sm_max, probes, probe_clocks)
+    try:
+        if cfg.name == "c5_lsst_oversub":
+            run_c5(args, cfg, snaps, torch, D)
+            return
+        if cfg.join == "knn" and cfg.n >= 100000:
+            run_lsst(args, cfg, snaps, torch, D, max(1, args.steps))
+            return
+        if cfg.join == "range":
+            run_range(args, cfg, snaps, torch, D, args.steps, args.warmup, peakinfo)
+            return
+        run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo)
+    finally:
         if world > 1:
             dist.destroy_process_group()
-        return
-    if cfg.join == "range":
-        run_range(args, cfg, snaps, torch, dev, rank, world, barrier, max_over_ranks)
-        if world > 1:
-            dist.destroy_process_group()
-        return
-    X = workloads.make_table(cfg.n, cfg.seed + rank, cols=list(range(cfg.n_feat)),
-                             outlier_frac=0.01 if cfg.n < 100000 else 0.001)
-    masks = cfg.masks()
-    if args.profile_masks > 0:
-        masks = masks[args.profile_offset:args.profile_offset + args.profile_masks]
+
+
+def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
+    rank, world, dev = D.rank, D.world, D.dev
+    weak = world > 1 and args.scaling == "weak"
+    X = workloads.make_table(cfg.n, cfg.seed + (rank if weak else 0), cols=list(range(cfg.n_feat)), outlier_frac=0.01)
+    masks_all = cfg.masks()
+    mine = np.arange(len(masks_all)) if (world == 1 or weak) else shard_masks(masks_all, rank, world)
+    masks = masks_all[mine]
     N, n_feat, k, n_masks = len(X), X.shape[1], cfg.k, len(masks)
-    evals = float(N) * N * n_masks                 # algorithmic (pair, subspace) evaluations
+    job_masks = len(masks_all) * (world if weak else 1)       # subspaces the whole job finishes per step
+    evals = float(N) * N * n_masks                            # this rank's (pair, subspace) evaluations
     planned = float(snaps.planned_evals(N, n_feat, masks))
 
     Xd = torch.from_numpy(X).to(dev)
@@ -336,8 +513,8 @@ def main():
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
-    barrier()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
+    D.barrier()
+    sampler = ClockSampler(dev.index or 0) if rank == 0 else None
     kernel_ms, launches = [], 0
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
@@ -349,52 +526,25 @@ def main():
         launches += n + 3                          # + the two staging kernels + the L2 flush fill
     ev1.record()
     torch.cuda.synchronize()
-    barrier()
+    D.barrier()
     clocks = sampler.stop() if sampler else None
-    ms_per_step = max_over_ranks(ev0.elapsed_time(ev1) / args.steps)
-    value = world * n_masks / (ms_per_step * 1e-3)
-    evals_per_s = world * evals / (ms_per_step * 1e-3)
+    ms_per_step = D.max_over_ranks(ev0.elapsed_time(ev1) / args.steps)
+    value = job_masks / (ms_per_step * 1e-3)
+    evals_per_s = float(N) * N * job_masks / (ms_per_step * 1e-3)
 
-    # sanity on the last step's result: every object has in-degree sum N*k
+    # sanity on the last step's result: every mask's in-degree row sums to N*k
     chk = int(out["indeg"][n_masks // 2].sum().item())
     assert chk == N * k, f"in-degree sum {chk} != N*k = {N * k}"
 
     # ---- roofline of the dominant kernel (knn_lattice_kernel): ALU/FP32-issue bound
-    peak_lane_ops, sm_max = peaks()
     k_ms = float(np.mean(kernel_ms))
     n_batches = planned / (64.0 * N * N)
-    lane_ops = 2.0 * evals + 30.0 * float(N) * N * n_batches   # per launch, algorithmic
-    achieved = lane_ops / (k_ms * 1e-3)
-    traffic = None
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get("knn_lattice_kernel_dram_bytes_per_launch")
-    except OSError:
-        pass
-    roofline = {
-        "bound": "alu", "kernel": "knn_lattice_kernel", "achieved": achieved / 1e12,
-        "peak": peak_lane_ops / 1e12, "unit": "TFLOP/s", "frac": achieved / peak_lane_ops,
-        "traffic": traffic, "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
-        "peak_source": f"derived: {N_SM} SMs x {LANES_PER_SM} FP32 lanes x {sm_max:.0f} MHz "
-                       "(FADD/FMUL/compare = 1 flop, no FMA in the path; FMA-counts-2 peak is 2x)",
-        "frac_of_fma2_peak": achieved / (2 * peak_lane_ops),
-        "algorithmic_lane_ops_per_launch": lane_ops,
-        "evals_per_s_kernel": evals / (k_ms * 1e-3),
-        "planned_lattice_slots_over_masks": planned / evals,
-        "note": "achieved = ALGORITHMIC lane-ops (2 per (pair, subspace) evaluation + 30 per pair and batch) / "
-                "kernel time; the kernel reaches the exact result with fewer executed operations (lower-bound "
-                "filter, 3-4% of candidates refined): executed instruction counts and pipe utilisation are in "
-                "profiles/r01d_full_set.md",
-    }
-    if rank == 0:
-        try:
-            roofline["probe_lane_ops_per_s"] = {
-                "ffma": snaps.probe_fp32_rate(0), "fadd": snaps.probe_fp32_rate(1),
-                "fadd+fsetp": snaps.probe_fp32_rate(2)}
-        except snaps.SnapsError as e:                      # pragma: no cover
-            roofline["probe_lane_ops_per_s"] = str(e)
+    roofline = alu_roofline("knn_lattice_kernel", evals, n_batches, N, k_ms, *peakinfo)
+    roofline["traffic"], roofline["traffic_source"] = stored_traffic()
+    roofline["kernel_share_of_step"] = k_ms / ms_per_step
+    roofline["planned_lattice_slots_over_masks"] = planned / evals
 
-    # ---- end to end through the host-buffer API: pinned X -> device, join, scores -> pinned host
+    # ---- end to end: ONE C call with host buffers (pinned X in, pinned scores out)
     e2e = None
     if not args.no_e2e:
         import psutil
@@ -404,36 +554,36 @@ def main():
             torch.cuda.empty_cache()
             Xh = torch.from_numpy(X).pin_memory()
             mpb = 2048
-            hws = torch.empty(snaps.workspace_bytes(N, n_feat, n_masks, k) +
-                              snaps.stream_ring_bytes(N, k, mpb), dtype=torch.uint8, device=dev)
+            hws = torch.empty(snaps.workspace_bytes(N, n_feat, n_masks, k, x_on_host=True) +
+                              snaps.stream_ring_bytes(N, N, k, mpb), dtype=torch.uint8, device=dev)
             hout = {"kth": torch.empty((n_masks, N), dtype=torch.float32, pin_memory=True),
                     "mean": torch.empty((n_masks, N), dtype=torch.float32, pin_memory=True),
                     "indeg": torch.empty((n_masks, N), dtype=torch.int32, pin_memory=True)}
-            xdev = torch.empty_like(Xd)
 
             def host_step():
-                snaps.knn_selfjoin_host(Xh, masks, k, mpb, lists=False, out=hout, workspace=hws,
-                                        x_device=xdev)
+                snaps.knn_selfjoin_host(Xh, masks, k, mpb, lists=False, out=hout, workspace=hws)
                 torch.cuda.current_stream().synchronize()
                 return float(hout["kth"][-1, -1])          # the host reads the result
 
             host_step()
-            barrier()
+            D.barrier()
             t0 = time.perf_counter()
             g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             g0.record()
-            n_e2e = max(1, min(args.steps, 2))
+            n_e2e = max(1, min(args.steps, 3))
             for _ in range(n_e2e):
                 host_step()
             g1.record()
             torch.cuda.synchronize()
             wall = (time.perf_counter() - t0) / n_e2e
-            e_ms = max_over_ranks(max(g0.elapsed_time(g1) / n_e2e, wall * 1e3))
+            e_ms = D.max_over_ranks(max(g0.elapsed_time(g1) / n_e2e, wall * 1e3))
             assert int(hout["indeg"][n_masks // 2].sum().item()) == N * k
-            e2e = {"value": world * n_masks / (e_ms * 1e-3), "unit": UNIT,
-                   "h2d_bytes_per_step": int(X.nbytes + masks.nbytes),
-                   "d2h_bytes_per_step": int(score_bytes), "ms_per_step": e_ms, "steps": n_e2e,
-                   "api": "knn_selfjoin_host -> snaps_knn_selfjoin_streamed (pinned host in/out)"}
+            e2e = {"value": job_masks / (e_ms * 1e-3), "unit": UNIT,
+                   "h2d_bytes_per_step": int(X.nbytes + masks.nbytes) * world,
+                   "d2h_bytes_per_step": int(score_bytes) * world, "ms_per_step": e_ms, "steps": n_e2e,
+                   "api": "snaps_knn_selfjoin_streamed with SNAPS_FLAG_X_ON_HOST: one C call, pinned host table in, "
+                          "pinned host scores out"}
+            del hout, hws, Xh
         else:
             e2e = {"value": None, "unit": UNIT, "skipped": "host RAM too small for pinned scores"}
 
@@ -443,40 +593,48 @@ def main():
         cpu = {"value": ev / dt / (float(N) * N), "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": what, "evals_per_s": ev / dt, "seconds": dt}
 
-    # ---- LSST-scale leg, side by side (north star): config 4 at full size, one warm + one timed pass
-    lsst = None
-    if rank == 0 and world == 1 and not args.no_lsst and args.profile_masks == 0 and args.config == "c2_snapshot1_knn":
+    # ---- the other configs, side by side (north star): DSSJ (config 3), LSST scale (config 4)
+    dssj = lsst = None
+    default_run = world == 1 and args.config == "c2_snapshot1_knn"
+    Xd = ws = out = None
+    torch.cuda.empty_cache()
+    if default_run and not args.no_dssj:
         try:
-            Xd = ws = out = hout = hws = xdev = Xh = None     # release config 2's device and pinned buffers
-            torch.cuda.empty_cache()
-            largs = argparse.Namespace(**{**vars(args), "steps": 1})
-            full = run_lsst(largs, workloads.get_config("c4_lsst_pairs"), snaps, torch, dev, rank, world,
-                            barrier, max_over_ranks, emit=False)
-            lsst = {k_: full[k_] for k_ in ("metric", "value", "unit", "ms_per_step", "effective_evals_per_s", "note")}
+            full = run_range(args, workloads.get_config("c3_snapshot1_dssj"), snaps, torch, D, 3, 1, peakinfo, emit=False)
+            dssj = {k_: full[k_] for k_ in ("metric", "value", "unit", "steps", "ms_per_step", "evals_per_s",
+                                            "mean_neighbours", "roofline", "clocks")}
+            dssj["workload"] = full["config"]["workload"]
+        except Exception as e:                                   # the headline line must survive this leg
+            dssj = {"error": repr(e)[:200]}
+        torch.cuda.empty_cache()
+    if default_run and not args.no_lsst:
+        try:
+            full = run_lsst(args, workloads.get_config("c4_lsst_pairs"), snaps, torch, D, 3, emit=False)
+            lsst = {k_: full[k_] for k_ in ("metric", "value", "unit", "steps", "ms_per_step", "effective_evals_per_s",
+                                            "join_kernel_ms", "note", "clocks")}
             lsst["workload"] = full["config"]["workload"]
             lsst["d2h_bytes_per_step"] = full["e2e"]["d2h_bytes_per_step"]
-        except Exception as e:                                   # the headline line must survive this leg
+        except Exception as e:
             lsst = {"error": repr(e)[:200]}
 
     if rank == 0:
         line = {
-            **({"profile_only": f"{n_masks} masks from index {args.profile_offset}"} if args.profile_masks > 0 else {}),
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_name(cfg, n_masks),
+            "scaling": "weak" if weak else "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg, len(masks_all)),
                        "l2": "256 MB flush fill before every step; each step also writes 12.5 GB of scores",
-                       "outputs": "scores only (lists of this config are 83 GB)"},
+                       "outputs": "scores only (lists of this config are 83 GB)",
+                       "sharding": ("one catalogue per rank" if weak else
+                                    "one catalogue; masks dealt to ranks by sub-lattice batch, no collective") if world > 1 else "none"},
             "evals_per_s": evals_per_s, "fp32_peak_frac": roofline["frac"],
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
-            "lsst_scale": lsst,
+            "dssj": dssj, "lsst_scale": lsst,
             "clocks": clocks,
             "paper_context": "paper: DSSJ all 32,752 spaces 2.64 h on 1xA100 (o=8) incl. CPU "
                              "post-processing; LSST5M kNNSJ ~100 s/feature space (PAPER.md:394, Table 4)",
         }
         print(json.dumps(line), flush=True)
-    if world > 1:
-        dist.destroy_process_group()
 
 
 if __name__ == "__main__":

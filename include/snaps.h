@@ -8,10 +8,12 @@
  * Conventions for every entry point
  *   - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  Output
  *     pointers named out_* are device pointers unless stated otherwise.
- *   - The caller owns every buffer; the library allocates nothing that
- *     outlives a call and never frees caller memory.  Scratch comes from
- *     d_workspace (size from snaps_workspace_bytes with the same N, n_feat,
- *     n_masks, k).
+ *   - The caller owns every buffer; the library allocates no device or pinned
+ *     memory and never frees caller memory.  Scratch comes from d_workspace
+ *     (size from snaps_workspace_bytes with the same N, n_feat, n_masks, k and
+ *     flags).  The batched calls keep one side stream and a few events per
+ *     calling thread, created on first use.  No environment variable or other
+ *     process-global state changes what a call does.
  *   - All device work is enqueued on `stream` (a cudaStream_t passed as
  *     void*; NULL = the legacy default stream).  The call returns when the
  *     work is enqueued; host-side planning may block the calling thread but
@@ -46,7 +48,28 @@ typedef int snaps_status;
 #define SNAPS_UNSUPPORTED 4
 
 #define SNAPS_MAX_FEATURES 15 /* PAPER.md:109 "We examine d <= 15" */
-#define SNAPS_MAX_K 32
+#define SNAPS_MAX_K 256        /* grid engine (k_max = 256 on LSST5M) */
+#define SNAPS_LATTICE_MAX_K 32 /* sub-lattice engine: lists live in shared memory */
+
+/*
+ * `flags` of the join entry points.  Bits 0..2 choose the engine:
+ *   SNAPS_ENGINE_AUTO     sub-lattice engine for N < 2^18 and k <= 32, grid engine otherwise
+ *   SNAPS_ENGINE_LATTICE  batches of 64 subspaces {H u T : T within features 0..5} share every
+ *                         pair's squared differences; brute force with an exact filter.  For
+ *                         mask lists with sub-lattice structure (all subsets) on L2-sized tables.
+ *   SNAPS_ENGINE_GRID     one subspace at a time through a grid index on up to three of its
+ *                         features.  For arbitrary mask lists, large N, k <= 256.
+ * Both engines compute the same joins; a pair's fp32 distance may differ in the last bit between
+ * them (different summation order), so equal-distance ties may resolve differently.
+ * SNAPS_FLAG_X_ON_HOST: the table pointer is a HOST pointer (pinned or pageable); the call copies
+ * it into the workspace first (the copy is part of the enqueued work).
+ * snaps_workspace_bytes must be given the same flags as the join that uses the workspace.
+ */
+#define SNAPS_ENGINE_AUTO 0
+#define SNAPS_ENGINE_LATTICE 1
+#define SNAPS_ENGINE_GRID 2
+#define SNAPS_ENGINE_MASK 7
+#define SNAPS_FLAG_X_ON_HOST 8
 
 /* Message for the last non-OK status on this thread (static storage). */
 const char *snaps_last_error(void);
@@ -55,16 +78,13 @@ const char *snaps_last_error(void);
 const char *snaps_version(void);
 
 /*
- * Bytes of device scratch the joins need for these sizes: the table staged
- * twice (80-byte rows; 32-row blocks of four float4 groups), batch
- * descriptors, and -- for N >= 2^18, where the joins take the pivot sweep
- * -- nine per-feature sorted copies of the table (72 bytes per
- * object each) plus radix-sort scratch.  k may be 0 for the range join.
- * Returns 0 on invalid sizes.  The environment variable SNAPS_KNN_SWEEP=0/1
- * overrides the size rule (it must have the same value when the workspace is
- * sized and when a join is called).
+ * Bytes of device scratch the joins need for these sizes and flags.  Sub-lattice engine: the
+ * table staged twice (80-byte rows; 32-row blocks of four float4 groups) and batch descriptors.
+ * Grid engine: staged rows, 4096 quantile edges and a 12-bit bin per object and feature, and one
+ * subspace's index (sorted cell keys, permutation, cell starts, compact rows; ~110 bytes per
+ * object).  k may be 0 for the range joins.  Returns 0 on invalid sizes.
  */
-size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k);
+size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k, int flags);
 
 /*
  * Number of (ordered query-candidate pair, mask) distance evaluations an
@@ -78,55 +98,61 @@ int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t *h_masks, int 
 
 /*
  * kNN self-join, kNNSJ (section 3.6): for every mask S and
- * every object i, the k objects j != i with the smallest (D(i,j;S), j).
- * Self is excluded by index (reading A4): a different object at
- * distance 0 is a neighbour.
+ * every query object i in [q_begin, q_end), the k objects j != i (of all N) with
+ * the smallest (D(i,j;S), j).  Self is excluded by index (reading
+ * A4): a different object at distance 0 is a neighbour.
  *
- *   d_X        device, [N][ld] fp32
+ *   d_X        device (host with SNAPS_FLAG_X_ON_HOST), [N][ld] fp32; every column finite,
+ *              including columns no mask uses
  *   h_masks    host, [n_masks] uint16
- *   k          1 <= k <= min(N-1, SNAPS_MAX_K)
- *   out_idx    device or pinned host, [n_masks][N][k] int32 neighbour ids,
- *              ascending by (distance, id); may be NULL
- *   out_dist   device or pinned host, [n_masks][N][k] fp32 distances D (not
- *              D^2), ascending; may be NULL
- *   out_kth    device, [n_masks][N] fp32, D_(k): k-th-neighbour distance
+ *   k          1 <= k <= min(N-1, SNAPS_MAX_K); the sub-lattice engine holds k <= 32
+ *   q_begin, q_end   the queries: 0 <= q_begin < q_end <= N; nq = q_end - q_begin.  A rank of a
+ *              multi-GPU run owns one slice (no exchange step);
+ *              (0, N) is the whole self-join
+ *   out_idx    device, [n_masks][nq][k] int32 neighbour ids, ascending by (distance, id); may be NULL
+ *   out_dist   device, [n_masks][nq][k] fp32 distances D (not D^2), ascending; may be NULL
+ *   out_kth    device, [n_masks][nq] fp32, D_(k): k-th-neighbour distance
  *              (BASELINE.json configs[0], reading A11); may be NULL
- *   out_mean   device, [n_masks][N] fp32, (1/k) sum_r D_(r): the distance-aware
+ *   out_mean   device, [n_masks][nq] fp32, (1/k) sum_r D_(r): the distance-aware
  *              kNN metric (reading A5); may be NULL
- *   out_indeg  device, [n_masks][N] int32, in-degree of the kNN graph: number
- *              of objects that list i among their kNN, the distance-oblivious
- *              metric; ZEROED by the call; may be NULL
+ *   out_indeg  device, [n_masks][N] int32, in-degree of the kNN graph restricted to the queries of
+ *              this call: number of queries that list object j among their kNN, the
+ *              distance-oblivious metric; summing the arrays of disjoint query
+ *              slices gives the full in-degree; ZEROED by the call; may be NULL
  *
  * Scores-only operation (out_idx == out_dist == NULL) is supported because
  * the lists of the all-subspace run are 83 GB.  Errors: SNAPS_INVALID_ARG for
  * N < 2, n_feat outside 1..15, ld < n_feat, NULL d_X/h_masks, n_masks < 1, a
- * zero mask or a mask bit >= n_feat, k outside its range, d_X not 4-byte
- * aligned, all five outputs NULL; SNAPS_WORKSPACE_TOO_SMALL; SNAPS_CUDA_ERROR.
+ * zero mask or a mask bit >= n_feat, k or the query range outside their ranges,
+ * d_X not 4-byte aligned, all five outputs NULL, an unknown engine;
+ * SNAPS_WORKSPACE_TOO_SMALL; SNAPS_CUDA_ERROR.
  */
 snaps_status snaps_knn_selfjoin(const float *d_X, int64_t N, int n_feat, int64_t ld,
                                 const uint16_t *h_masks, int n_masks, int k,
+                                int64_t q_begin, int64_t q_end, int flags,
                                 int32_t *out_idx, float *out_dist,
                                 float *out_kth, float *out_mean, int32_t *out_indeg,
                                 void *d_workspace, size_t workspace_bytes, void *stream);
 
 /*
  * eps range self-join, DSSJ (section 3.5): for
- * every mask S and object i, the objects j != i with D(i,j;S) <= eps_S
- * (closed ball, reading A2; pairs within 1e-6 relative of eps may fall on
- * either side in fp32).
+ * every mask S and query object i in [q_begin, q_end), the objects j != i with
+ * D(i,j;S) <= eps_S (closed ball, reading A2; pairs within 1e-6 relative of eps
+ * may fall on either side in fp32).
  *
  *   h_eps        host, [n_masks] fp32, each finite and > 0
- *   out_count    device, [n_masks][N] uint32: number of neighbours within eps,
+ *   out_count    device, [n_masks][nq] uint32: number of neighbours within eps,
  *                self excluded = the distance-oblivious DSSJ
  *                metric; required
- *   out_sumdist  device, [n_masks][N] fp32: sum of D over those neighbours
+ *   out_sumdist  device, [n_masks][nq] fp32: sum of D over those neighbours
  *                (numerator of the distance-aware metric); may be
  *                NULL
- *   out_mean     device, [n_masks][N] fp32: sumdist/count, 0 when count == 0
+ *   out_mean     device, [n_masks][nq] fp32: sumdist/count, 0 when count == 0
  *                (reading A6); may be NULL
  */
 snaps_status snaps_range_selfjoin(const float *d_X, int64_t N, int n_feat, int64_t ld,
                                   const uint16_t *h_masks, int n_masks, const float *h_eps,
+                                  int64_t q_begin, int64_t q_end, int flags,
                                   uint32_t *out_count, float *out_sumdist, float *out_mean,
                                   void *d_workspace, size_t workspace_bytes, void *stream);
 
@@ -147,37 +173,100 @@ snaps_status snaps_outlier_scores(int64_t N, int n_masks, int k,
                                   float *out_eps_mean, void *stream);
 
 /*
- * Batched ("oversubscribed") kNN self-join for outputs that
- * exceed device memory: masks are processed in groups of masks_per_batch; each
- * group's lists and scores are produced into a device staging ring inside
- * d_workspace and copied on a side stream into the caller's PINNED HOST
- * buffers while the next group computes.
+ * ---- a8: batched ("oversubscribed") joins for outputs that exceed device
+ * (or host) memory.  Masks are processed in groups of masks_per_batch; each group's outputs are
+ * produced into a two-slot device staging ring inside d_workspace and copied on a side stream
+ * to the host while the next group computes.  The workspace must hold
+ * snaps_workspace_bytes(...) + snaps_stream_ring_bytes(nq, N, k, masks_per_batch).
  *
- *   h_out_*   pinned host buffers with the shapes of snaps_knn_selfjoin's
- *             outputs; any may be NULL (at least one non-NULL)
- *   masks_per_batch  >= 1; workspace must hold snaps_workspace_bytes(...) +
- *             snaps_stream_ring_bytes(N, k, masks_per_batch)
- * `stream` completes only after the last host copy has landed.
+ * snaps_knn_selfjoin_streamed: the destination is the caller's full-size PINNED HOST arrays
+ * (shapes of snaps_knn_selfjoin's outputs; any may be NULL, at least one non-NULL); `stream`
+ * completes only after the last host copy has landed.
  */
-size_t snaps_stream_ring_bytes(int64_t N, int k, int masks_per_batch);
+size_t snaps_stream_ring_bytes(int64_t nq, int64_t N, int k, int masks_per_batch);
 
 snaps_status snaps_knn_selfjoin_streamed(const float *d_X, int64_t N, int n_feat, int64_t ld,
                                          const uint16_t *h_masks, int n_masks, int k,
                                          int masks_per_batch,
+                                         int64_t q_begin, int64_t q_end, int flags,
                                          int32_t *h_out_idx, float *h_out_dist,
                                          float *h_out_kth, float *h_out_mean,
                                          int32_t *h_out_indeg,
                                          void *d_workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * The recycling sink: when the whole output does not fit on the host either (the kNN lists of the
+ * all-subspace run are 83 GB, of the LSST-scale run 164 GB), each group is copied into one of a
+ * few pinned host buffers and handed to a consumer callback, after which the buffer is reused.
+ *
+ *   want        which outputs to produce (SNAPS_OUT_* bits)
+ *   h_buffers   n_buffers >= 2 pinned host buffers of buffer_bytes >=
+ *               snaps_sink_batch_bytes(nq, N, k, masks_per_batch, want) each
+ *   consume     called on the calling thread, once per group in mask order, with pointers into
+ *               the buffer; the buffer is recycled when it returns
+ * These two calls return after the last group has been consumed (the consumer runs on the host).
+ */
+#define SNAPS_OUT_IDX 1u
+#define SNAPS_OUT_DIST 2u
+#define SNAPS_OUT_KTH 4u
+#define SNAPS_OUT_MEAN 8u
+#define SNAPS_OUT_INDEG 16u
+#define SNAPS_OUT_COUNT 32u
+#define SNAPS_OUT_SUMDIST 64u
+#define SNAPS_OUT_EPSMEAN 128u
+
+typedef struct snaps_batch_view {
+    int mask_begin, mask_end;   /* this group = masks [mask_begin, mask_end) of the caller's list */
+    int64_t q_begin, q_end;     /* its queries */
+    int64_t N;
+    int k;
+    const int32_t *idx;         /* [mask_end - mask_begin][nq][k], or NULL */
+    const float *dist;
+    const float *kth;           /* [..][nq] */
+    const float *mean;
+    const int32_t *indeg;       /* [..][N] */
+    const uint32_t *count;      /* [..][nq] */
+    const float *sumdist;
+    const float *eps_mean;
+} snaps_batch_view;
+
+typedef void (*snaps_batch_fn)(void *user, const snaps_batch_view *view);
+
+typedef struct snaps_batch_sink {
+    void **h_buffers;
+    int n_buffers;
+    size_t buffer_bytes;
+    unsigned want;
+    snaps_batch_fn consume;
+    void *user;
+} snaps_batch_sink;
+
+size_t snaps_sink_batch_bytes(int64_t nq, int64_t N, int k, int masks_per_batch, unsigned want);
+
+snaps_status snaps_knn_selfjoin_sink(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                     const uint16_t *h_masks, int n_masks, int k, int masks_per_batch,
+                                     int64_t q_begin, int64_t q_end, int flags,
+                                     const snaps_batch_sink *sink,
+                                     void *d_workspace, size_t workspace_bytes, void *stream);
+
+snaps_status snaps_range_selfjoin_sink(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                       const uint16_t *h_masks, int n_masks, const float *h_eps,
+                                       int masks_per_batch,
+                                       int64_t q_begin, int64_t q_end, int flags,
+                                       const snaps_batch_sink *sink,
+                                       void *d_workspace, size_t workspace_bytes, void *stream);
+
+/*
  * Peak-rate probe used for the roofline denominator:
  * runs an FP32 instruction-throughput microkernel on `stream` and returns the
- * measured warp-instruction lane rate.  kind: 0 = FFMA (3-register), 1 = FADD,
- * 2 = FADD + FSETP pairs (the join's inner-loop mix).  *h_lane_ops_per_s
+ * measured warp-instruction lane rate.  kind: 0 = FFMA (two of three operands uniform), 1 = FADD,
+ * 2 = FADD + FSETP pairs (the sub-lattice join's inner-loop mix), 3 = FFMA with three
+ * register operands, 4 = packed FFMA2 (fma.rn.f32x2, two results per lane: counted as two
+ * lane-ops), 5 = packed FADD2.  *h_lane_ops_per_s
  * receives executed lane-ops per second (one FFMA counts as ONE lane-op).
- * Synchronises `stream`.
+ * d_scratch: device, >= 4096 bytes.  Synchronises `stream` (it returns a measurement).
  */
-snaps_status snaps_probe_fp32_rate(int kind, double *h_lane_ops_per_s, void *stream);
+snaps_status snaps_probe_fp32_rate(int kind, double *h_lane_ops_per_s, void *d_scratch, void *stream);
 
 /*
  * ---- NEXT-1 (PAPER.md sections 3.4, 3.5.2, 3.6): ranking and parameter selection ----
@@ -243,9 +332,9 @@ snaps_status snaps_knn_scores_at_k(int64_t N, int n_masks, int k_max, int k_j,
  *   out_j_indeg, out_j_mean   device, [n_masks] int32: index into the grid of the selected k
  *   out_u                     device, [4][G][n_masks] fp32 or NULL: U_min / U_max of the in-degree
  *                             metric, then U_min / U_max of the mean-distance metric
- * Workspace: snaps_select_k_workspace_bytes(N, n_masks).
+ * Workspace: snaps_select_k_workspace_bytes(N, n_masks, G).
  */
-size_t snaps_select_k_workspace_bytes(int64_t N, int n_masks);
+size_t snaps_select_k_workspace_bytes(int64_t N, int n_masks, int G);
 
 snaps_status snaps_knn_select_k(int64_t N, int n_masks, int k_max, const int32_t *knn_idx,
                                 const float *knn_dist, const int32_t *h_k_grid, int G, int n_top,
@@ -256,17 +345,21 @@ snaps_status snaps_knn_select_k(int64_t N, int n_masks, int k_max, const int32_t
  * DSSJ for a grid of radii in ONE scan (Fig. 3: "we execute DSSJ once for
  * eps_max and use this result set to derive the result sets for all eps_i in G").
  *   h_eps_grid  host, [n_masks][G] fp32, per mask strictly ascending, finite, > 0; 1 <= G <= 32
- *   out_count   device, [n_masks][G][N] uint32: neighbours within eps_g (self excluded)
+ *   out_count   device, [n_masks][G][nq] uint32: neighbours within eps_g (self excluded)
  *   out_sumdist, out_mean  device, same shape, fp32; may be NULL (mean = 0 when count = 0)
- * Workspace: snaps_range_grid_workspace_bytes(N, n_feat, n_masks, G).
+ *   q_begin, q_end, flags  as for snaps_range_selfjoin (both engines have a radius-grid kernel;
+ *               the grid engine is the one for large selectivities such as PAPER.md:229's
+ *               s_max ~ 0.15 |D|, where nearly every pair is a hit)
+ * Workspace: snaps_range_grid_workspace_bytes(N, n_feat, n_masks, G, flags).
  */
-size_t snaps_range_grid_workspace_bytes(int64_t N, int n_feat, int n_masks, int G);
+size_t snaps_range_grid_workspace_bytes(int64_t N, int n_feat, int n_masks, int G, int flags);
 
 snaps_status snaps_range_selfjoin_grid(const float *d_X, int64_t N, int n_feat, int64_t ld,
                                        const uint16_t *h_masks, int n_masks,
-                                       const float *h_eps_grid, int G, uint32_t *out_count,
-                                       float *out_sumdist, float *out_mean, void *d_workspace,
-                                       size_t workspace_bytes, void *stream);
+                                       const float *h_eps_grid, int G,
+                                       int64_t q_begin, int64_t q_end, int flags,
+                                       uint32_t *out_count, float *out_sumdist, float *out_mean,
+                                       void *d_workspace, size_t workspace_bytes, void *stream);
 
 /*
  * ---- NEXT-2: search radius for a target selectivity ----
@@ -300,9 +393,10 @@ snaps_status snaps_eps_from_histogram(const unsigned long long *h_hist, int n_ma
                                       double target_s, float *h_eps);
 
 /*
- * Kernel timing for roofline reports.  While enabled,
- * every join call records a CUDA event pair on `stream` around each launch of
- * its dominant (join) kernel; the pairs of the most recent call are kept.
+ * Kernel timing for roofline reports.  While enabled
+ * (per calling thread), every join call records a CUDA event pair on `stream`
+ * around each launch of its dominant (join) kernel; the pairs of the most
+ * recent call of this thread are kept.
  * snaps_profile_last_kernel_ms synchronises on them and returns the summed
  * device time in milliseconds and the number of launches (either pointer may
  * be NULL).  Disabled by default; enabling costs two event records per launch.

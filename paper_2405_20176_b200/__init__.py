@@ -8,6 +8,6 @@ the symbol table can be checked), calling a join without the library or a device
 from .binding import (  # noqa: F401
     SnapsError, lib, lib_path, version, workspace_bytes, stream_ring_bytes, planned_evals,
     knn_selfjoin, range_selfjoin, outlier_scores, knn_selfjoin_streamed, probe_fp32_rate,
-    knn_selfjoin_host, EXPORTED_SYMBOLS, profile_enable, profile_last_kernel_ms,
+    knn_selfjoin_host, knn_selfjoin_sink, range_selfjoin_sink, sink_batch_bytes, EXPORTED_SYMBOLS, ENGINES, profile_enable, profile_last_kernel_ms,
     range_selfjoin_grid, knn_select_k, sample_distance_histogram, eps_from_histogram, rank_scores, topn_overlap, select_parameter, knn_scores_at_k, METRIC_KINDS,
 )

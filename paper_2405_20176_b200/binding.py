@@ -11,13 +11,18 @@ from . import build as _build
 EXPORTED_SYMBOLS = [
     "snaps_last_error", "snaps_version", "snaps_workspace_bytes", "snaps_planned_evals",
     "snaps_knn_selfjoin", "snaps_range_selfjoin", "snaps_outlier_scores",
-    "snaps_stream_ring_bytes", "snaps_knn_selfjoin_streamed", "snaps_probe_fp32_rate",
+    "snaps_stream_ring_bytes", "snaps_knn_selfjoin_streamed", "snaps_sink_batch_bytes",
+    "snaps_knn_selfjoin_sink", "snaps_range_selfjoin_sink", "snaps_probe_fp32_rate",
     "snaps_profile_enable", "snaps_profile_last_kernel_ms",
     "snaps_rank_workspace_bytes", "snaps_rank_scores", "snaps_topn_overlap", "snaps_select_parameter",
     "snaps_knn_scores_at_k", "snaps_range_grid_workspace_bytes", "snaps_range_selfjoin_grid",
     "snaps_select_k_workspace_bytes", "snaps_knn_select_k",
     "snaps_dist_hist_workspace_bytes", "snaps_sample_distance_histogram", "snaps_eps_from_histogram",
 ]
+
+ENGINES = {"auto": 0, "lattice": 1, "grid": 2}
+FLAG_X_ON_HOST = 8
+OUT_BITS = {"idx": 1, "dist": 2, "kth": 4, "mean": 8, "indeg": 16, "count": 32, "sumdist": 64, "eps_mean": 128}
 
 _lib = None
 
@@ -26,6 +31,25 @@ class SnapsError(RuntimeError):
     def __init__(self, status: int, message: str):
         super().__init__(f"snaps status {status}: {message}")
         self.status = status
+
+
+class BatchView(ctypes.Structure):
+    """snaps_batch_view of include/snaps.h."""
+    _fields_ = [("mask_begin", ctypes.c_int), ("mask_end", ctypes.c_int),
+                ("q_begin", ctypes.c_int64), ("q_end", ctypes.c_int64), ("N", ctypes.c_int64), ("k", ctypes.c_int),
+                ("idx", ctypes.c_void_p), ("dist", ctypes.c_void_p), ("kth", ctypes.c_void_p),
+                ("mean", ctypes.c_void_p), ("indeg", ctypes.c_void_p), ("count", ctypes.c_void_p),
+                ("sumdist", ctypes.c_void_p), ("eps_mean", ctypes.c_void_p)]
+
+
+BATCH_FN = ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.POINTER(BatchView))
+
+
+class BatchSink(ctypes.Structure):
+    """snaps_batch_sink of include/snaps.h."""
+    _fields_ = [("h_buffers", ctypes.POINTER(ctypes.c_void_p)), ("n_buffers", ctypes.c_int),
+                ("buffer_bytes", ctypes.c_size_t), ("want", ctypes.c_uint), ("consume", BATCH_FN),
+                ("user", ctypes.c_void_p)]
 
 
 def lib_path() -> str:
@@ -42,22 +66,30 @@ def lib():
         L.snaps_last_error.restype = ctypes.c_char_p
         L.snaps_version.restype = ctypes.c_char_p
         L.snaps_workspace_bytes.restype = sz
-        L.snaps_workspace_bytes.argtypes = [i64, i32, i32, i32]
+        L.snaps_workspace_bytes.argtypes = [i64, i32, i32, i32, i32]
         L.snaps_planned_evals.restype = i64
         L.snaps_planned_evals.argtypes = [i64, i32, vp, i32]
         L.snaps_knn_selfjoin.restype = i32
-        L.snaps_knn_selfjoin.argtypes = [vp, i64, i32, i64, vp, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.snaps_knn_selfjoin.argtypes = [vp, i64, i32, i64, vp, i32, i32, i64, i64, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         L.snaps_range_selfjoin.restype = i32
-        L.snaps_range_selfjoin.argtypes = [vp, i64, i32, i64, vp, i32, vp, vp, vp, vp, vp, sz, vp]
+        L.snaps_range_selfjoin.argtypes = [vp, i64, i32, i64, vp, i32, vp, i64, i64, i32, vp, vp, vp, vp, sz, vp]
         L.snaps_outlier_scores.restype = i32
         L.snaps_outlier_scores.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
         L.snaps_stream_ring_bytes.restype = sz
-        L.snaps_stream_ring_bytes.argtypes = [i64, i32, i32]
+        L.snaps_stream_ring_bytes.argtypes = [i64, i64, i32, i32]
         L.snaps_knn_selfjoin_streamed.restype = i32
-        L.snaps_knn_selfjoin_streamed.argtypes = [vp, i64, i32, i64, vp, i32, i32, i32,
+        L.snaps_knn_selfjoin_streamed.argtypes = [vp, i64, i32, i64, vp, i32, i32, i32, i64, i64, i32,
                                                   vp, vp, vp, vp, vp, vp, sz, vp]
+        L.snaps_sink_batch_bytes.restype = sz
+        L.snaps_sink_batch_bytes.argtypes = [i64, i64, i32, i32, ctypes.c_uint]
+        L.snaps_knn_selfjoin_sink.restype = i32
+        L.snaps_knn_selfjoin_sink.argtypes = [vp, i64, i32, i64, vp, i32, i32, i32, i64, i64, i32,
+                                              ctypes.POINTER(BatchSink), vp, sz, vp]
+        L.snaps_range_selfjoin_sink.restype = i32
+        L.snaps_range_selfjoin_sink.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, i64, i64, i32,
+                                                ctypes.POINTER(BatchSink), vp, sz, vp]
         L.snaps_probe_fp32_rate.restype = i32
-        L.snaps_probe_fp32_rate.argtypes = [i32, ctypes.POINTER(ctypes.c_double), vp]
+        L.snaps_probe_fp32_rate.argtypes = [i32, ctypes.POINTER(ctypes.c_double), vp, vp]
         L.snaps_profile_enable.restype = i32
         L.snaps_profile_enable.argtypes = [i32]
         L.snaps_profile_last_kernel_ms.restype = i32
@@ -72,9 +104,9 @@ def lib():
         L.snaps_select_parameter.restype = i32
         L.snaps_select_parameter.argtypes = [vp, vp, i32, i32, i32, vp, vp]
         L.snaps_range_grid_workspace_bytes.restype = sz
-        L.snaps_range_grid_workspace_bytes.argtypes = [i64, i32, i32, i32]
+        L.snaps_range_grid_workspace_bytes.argtypes = [i64, i32, i32, i32, i32]
         L.snaps_range_selfjoin_grid.restype = i32
-        L.snaps_range_selfjoin_grid.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, vp, vp, vp, sz, vp]
+        L.snaps_range_selfjoin_grid.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, i64, i64, i32, vp, vp, vp, vp, sz, vp]
         L.snaps_dist_hist_workspace_bytes.restype = sz
         L.snaps_dist_hist_workspace_bytes.argtypes = [i32, i32, i32]
         L.snaps_sample_distance_histogram.restype = i32
@@ -82,7 +114,7 @@ def lib():
         L.snaps_eps_from_histogram.restype = i32
         L.snaps_eps_from_histogram.argtypes = [vp, i32, i32, vp, i64, i64, ctypes.c_double, vp]
         L.snaps_select_k_workspace_bytes.restype = sz
-        L.snaps_select_k_workspace_bytes.argtypes = [i64, i32]
+        L.snaps_select_k_workspace_bytes.argtypes = [i64, i32, i32]
         L.snaps_knn_select_k.restype = i32
         L.snaps_knn_select_k.argtypes = [i64, i32, i32, vp, vp, vp, i32, i32, vp, vp, vp, vp, sz, vp]
         L.snaps_knn_scores_at_k.restype = i32
@@ -114,12 +146,20 @@ def _stream(stream):
     return ctypes.c_void_p(s.cuda_stream)
 
 
-def workspace_bytes(N: int, n_feat: int, n_masks: int, k: int) -> int:
-    return int(lib().snaps_workspace_bytes(N, n_feat, n_masks, k))
+def _flags(engine: str, x_on_host: bool = False) -> int:
+    return ENGINES[engine] | (FLAG_X_ON_HOST if x_on_host else 0)
 
 
-def stream_ring_bytes(N: int, k: int, masks_per_batch: int) -> int:
-    return int(lib().snaps_stream_ring_bytes(N, k, masks_per_batch))
+def _qrange(q_range, N):
+    return (0, N) if q_range is None else (int(q_range[0]), int(q_range[1]))
+
+
+def workspace_bytes(N: int, n_feat: int, n_masks: int, k: int, engine: str = "auto", x_on_host: bool = False) -> int:
+    return int(lib().snaps_workspace_bytes(N, n_feat, n_masks, k, _flags(engine, x_on_host)))
+
+
+def stream_ring_bytes(nq: int, N: int, k: int, masks_per_batch: int) -> int:
+    return int(lib().snaps_stream_ring_bytes(nq, N, k, masks_per_batch))
 
 
 def planned_evals(N: int, n_feat: int, masks) -> int:
@@ -127,43 +167,48 @@ def planned_evals(N: int, n_feat: int, masks) -> int:
     return int(lib().snaps_planned_evals(N, n_feat, m.ctypes.data_as(ctypes.c_void_p), len(m)))
 
 
-def _workspace(X, n_masks, k, extra=0):
+def _workspace(N, n_feat, n_masks, k, device, engine="auto", extra=0, x_on_host=False):
     import torch
-    nbytes = workspace_bytes(X.shape[0], X.shape[1], n_masks, k) + extra
+    nbytes = workspace_bytes(N, n_feat, n_masks, k, engine, x_on_host)
     if nbytes == 0:
         raise SnapsError(1, "invalid sizes for workspace")
-    return torch.empty(nbytes, dtype=torch.uint8, device=X.device)
+    return torch.empty(nbytes + extra, dtype=torch.uint8, device=device)
 
 
-def knn_selfjoin(X, masks, k, *, lists=True, scores=True, out=None, workspace=None, stream=None):
+def knn_selfjoin(X, masks, k, *, lists=True, scores=True, out=None, workspace=None, stream=None,
+                 q_range=None, engine="auto"):
     """snaps_knn_selfjoin on a CUDA fp32 tensor X [N, n_feat].
 
-    Returns a dict with idx/dist [n_masks, N, k] (if lists) and kth/mean/indeg [n_masks, N]
-    (if scores), all torch CUDA tensors.  `out` may supply preallocated tensors by those names."""
+    Returns a dict with idx/dist [n_masks, nq, k] (if lists), kth/mean [n_masks, nq] and indeg
+    [n_masks, N] (if scores), all torch CUDA tensors; nq = q_range[1] - q_range[0] (default: all N
+    objects are queries).  `out` may supply preallocated tensors by those names."""
     import torch
     assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
     m = _masks(masks)
     N, n_feat = X.shape
+    q0, q1 = _qrange(q_range, N)
+    nq = q1 - q0
     out = dict(out or {})
     dev = X.device
     if lists:
-        out.setdefault("idx", torch.empty((len(m), N, k), dtype=torch.int32, device=dev))
-        out.setdefault("dist", torch.empty((len(m), N, k), dtype=torch.float32, device=dev))
+        out.setdefault("idx", torch.empty((len(m), nq, k), dtype=torch.int32, device=dev))
+        out.setdefault("dist", torch.empty((len(m), nq, k), dtype=torch.float32, device=dev))
     if scores:
-        out.setdefault("kth", torch.empty((len(m), N), dtype=torch.float32, device=dev))
-        out.setdefault("mean", torch.empty((len(m), N), dtype=torch.float32, device=dev))
+        out.setdefault("kth", torch.empty((len(m), nq), dtype=torch.float32, device=dev))
+        out.setdefault("mean", torch.empty((len(m), nq), dtype=torch.float32, device=dev))
         out.setdefault("indeg", torch.empty((len(m), N), dtype=torch.int32, device=dev))
-    ws = workspace if workspace is not None else _workspace(X, len(m), k)
+    ws = workspace if workspace is not None else _workspace(N, n_feat, len(m), k, dev, engine)
     _check(lib().snaps_knn_selfjoin(
-        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m), k,
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m), k, q0, q1, _flags(engine),
         _dptr(out.get("idx")), _dptr(out.get("dist")), _dptr(out.get("kth")),
         _dptr(out.get("mean")), _dptr(out.get("indeg")), _dptr(ws), ws.numel(), _stream(stream)))
     out["_workspace"] = ws
     return out
 
 
-def range_selfjoin(X, masks, eps, *, sums=True, out=None, workspace=None, stream=None):
-    """snaps_range_selfjoin: returns dict count [n_masks, N] (int32 view of uint32) and, if
+def range_selfjoin(X, masks, eps, *, sums=True, out=None, workspace=None, stream=None, q_range=None,
+                   engine="auto"):
+    """snaps_range_selfjoin: returns dict count [n_masks, nq] (int32 view of uint32) and, if
     sums, sumdist / mean."""
     import torch
     assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
@@ -171,16 +216,18 @@ def range_selfjoin(X, masks, eps, *, sums=True, out=None, workspace=None, stream
     e = np.ascontiguousarray(np.asarray(eps, dtype=np.float32).ravel())
     assert len(e) == len(m)
     N, n_feat = X.shape
+    q0, q1 = _qrange(q_range, N)
+    nq = q1 - q0
     out = dict(out or {})
     dev = X.device
-    out.setdefault("count", torch.empty((len(m), N), dtype=torch.int32, device=dev))
+    out.setdefault("count", torch.empty((len(m), nq), dtype=torch.int32, device=dev))
     if sums:
-        out.setdefault("sumdist", torch.empty((len(m), N), dtype=torch.float32, device=dev))
-        out.setdefault("mean", torch.empty((len(m), N), dtype=torch.float32, device=dev))
-    ws = workspace if workspace is not None else _workspace(X, len(m), 0)
+        out.setdefault("sumdist", torch.empty((len(m), nq), dtype=torch.float32, device=dev))
+        out.setdefault("mean", torch.empty((len(m), nq), dtype=torch.float32, device=dev))
+    ws = workspace if workspace is not None else _workspace(N, n_feat, len(m), 0, dev, engine)
     _check(lib().snaps_range_selfjoin(
         _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
-        e.ctypes.data_as(ctypes.c_void_p), _dptr(out["count"]), _dptr(out.get("sumdist")),
+        e.ctypes.data_as(ctypes.c_void_p), q0, q1, _flags(engine), _dptr(out["count"]), _dptr(out.get("sumdist")),
         _dptr(out.get("mean")), _dptr(ws), ws.numel(), _stream(stream)))
     out["_workspace"] = ws
     return out
@@ -208,63 +255,135 @@ def outlier_scores(N, n_masks, k, *, knn_idx=None, knn_dist=None, eps_count=None
 
 
 def knn_selfjoin_streamed(X, masks, k, masks_per_batch, *, lists=True, scores=True, out=None,
-                          workspace=None, stream=None):
-    """snaps_knn_selfjoin_streamed: outputs land in PINNED HOST tensors."""
+                          workspace=None, stream=None, q_range=None, engine="auto", x_on_host=False):
+    """snaps_knn_selfjoin_streamed: outputs land in PINNED HOST tensors.  With x_on_host, X is a host
+    tensor (pinned or pageable) and the copy to the device is part of the call."""
     import torch
-    assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
+    assert X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
+    assert X.is_cuda != bool(x_on_host)
     m = _masks(masks)
     N, n_feat = X.shape
+    q0, q1 = _qrange(q_range, N)
+    nq = q1 - q0
     out = dict(out or {})
 
     def pinned(shape, dtype):
         return torch.empty(shape, dtype=dtype, pin_memory=True)
 
     if lists:
-        out.setdefault("idx", pinned((len(m), N, k), torch.int32))
-        out.setdefault("dist", pinned((len(m), N, k), torch.float32))
+        out.setdefault("idx", pinned((len(m), nq, k), torch.int32))
+        out.setdefault("dist", pinned((len(m), nq, k), torch.float32))
     if scores:
-        out.setdefault("kth", pinned((len(m), N), torch.float32))
-        out.setdefault("mean", pinned((len(m), N), torch.float32))
+        out.setdefault("kth", pinned((len(m), nq), torch.float32))
+        out.setdefault("mean", pinned((len(m), nq), torch.float32))
         out.setdefault("indeg", pinned((len(m), N), torch.int32))
     for n, t in out.items():
         assert n.startswith("_") or t.is_pinned(), n
+    dev = X.device if X.is_cuda else torch.device("cuda", torch.cuda.current_device())
     ws = workspace if workspace is not None else _workspace(
-        X, len(m), k, extra=stream_ring_bytes(N, k, masks_per_batch))
+        N, n_feat, len(m), k, dev, engine, extra=stream_ring_bytes(nq, N, k, masks_per_batch), x_on_host=x_on_host)
     _check(lib().snaps_knn_selfjoin_streamed(
         _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m), k,
-        masks_per_batch, _dptr(out.get("idx")), _dptr(out.get("dist")), _dptr(out.get("kth")),
-        _dptr(out.get("mean")), _dptr(out.get("indeg")), _dptr(ws), ws.numel(), _stream(stream)))
+        masks_per_batch, q0, q1, _flags(engine, x_on_host), _dptr(out.get("idx")), _dptr(out.get("dist")),
+        _dptr(out.get("kth")), _dptr(out.get("mean")), _dptr(out.get("indeg")), _dptr(ws), ws.numel(),
+        _stream(stream)))
     out["_workspace"] = ws
     return out
 
 
 def knn_selfjoin_host(X_host, masks, k, masks_per_batch=None, *, lists=False, scores=True, out=None,
-                      workspace=None, x_device=None, stream=None):
-    """End-to-end call with HOST buffers: pinned X -> device, join, pinned host outputs.
-    Returns the dict of pinned host tensors after the work is enqueued (caller synchronises).
-    `out`, `workspace` and `x_device` may supply preallocated buffers for repeated calls."""
+                      workspace=None, stream=None, engine="auto"):
+    """End-to-end call with HOST buffers only: ONE C call (snaps_knn_selfjoin_streamed with
+    SNAPS_FLAG_X_ON_HOST) copies the pinned table to the device, joins, and copies the outputs into
+    pinned host tensors.  Returns them after the work is enqueued (caller synchronises)."""
     import torch
     Xh = torch.as_tensor(X_host)
     if not Xh.is_pinned():
         Xh = Xh.pin_memory()
-    s = torch.cuda.current_stream() if stream is None else stream
-    with torch.cuda.stream(s):
-        if x_device is None:
-            Xd = Xh.to("cuda", non_blocking=True)
-        else:
-            Xd = x_device
-            Xd.copy_(Xh, non_blocking=True)
     n_masks = len(_masks(masks))
     mpb = masks_per_batch or max(1, min(n_masks, 2048))
-    out = knn_selfjoin_streamed(Xd, masks, k, mpb, lists=lists, scores=scores, out=out,
-                                workspace=workspace, stream=s)
-    out["_X"] = Xd
+    out = knn_selfjoin_streamed(Xh, masks, k, mpb, lists=lists, scores=scores, out=out, workspace=workspace,
+                                stream=stream, engine=engine, x_on_host=True)
+    out["_X"] = Xh
     return out
 
 
+def sink_batch_bytes(nq: int, N: int, k: int, masks_per_batch: int, want) -> int:
+    bits = sum(OUT_BITS[w] for w in want)
+    return int(lib().snaps_sink_batch_bytes(nq, N, k, masks_per_batch, bits))
+
+
+def _run_sink(kind, X, masks, k, eps, masks_per_batch, want, consume, n_buffers, q_range, engine, workspace, stream):
+    import torch
+    assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
+    m = _masks(masks)
+    N, n_feat = X.shape
+    q0, q1 = _qrange(q_range, N)
+    nq = q1 - q0
+    bits = sum(OUT_BITS[w] for w in want)
+    nbytes = int(lib().snaps_sink_batch_bytes(nq, N, k, masks_per_batch, bits))
+    bufs = [torch.empty(nbytes, dtype=torch.uint8, pin_memory=True) for _ in range(n_buffers)]
+    ptrs = (ctypes.c_void_p * n_buffers)(*[b.data_ptr() for b in bufs])
+    shapes = {"idx": (nq, k), "dist": (nq, k), "kth": (nq,), "mean": (nq,), "indeg": (N,),
+              "count": (nq,), "sumdist": (nq,), "eps_mean": (nq,)}
+    dtypes = {"idx": np.int32, "dist": np.float32, "kth": np.float32, "mean": np.float32, "indeg": np.int32,
+              "count": np.uint32, "sumdist": np.float32, "eps_mean": np.float32}
+    errors = []
+
+    def trampoline(_user, view_p):
+        v = view_p.contents
+        nm = v.mask_end - v.mask_begin
+        arrays = {}
+        for name in shapes:
+            addr = getattr(v, name)
+            if addr:
+                shp = (nm,) + shapes[name]
+                n_el = int(np.prod(shp))
+                buf = (ctypes.c_byte * (n_el * 4)).from_address(addr)
+                arrays[name] = np.frombuffer(buf, dtype=dtypes[name], count=n_el).reshape(shp)
+        try:
+            consume(v.mask_begin, v.mask_end, arrays)
+        except Exception as e:          # a Python exception must not unwind through the C frames
+            errors.append(e)
+
+    cb = BATCH_FN(trampoline)
+    sink = BatchSink(ptrs, n_buffers, nbytes, bits, cb, None)
+    ws = workspace if workspace is not None else _workspace(
+        N, n_feat, len(m), k, X.device, engine, extra=stream_ring_bytes(nq, N, k, masks_per_batch))
+    if kind == "knn":
+        rc = lib().snaps_knn_selfjoin_sink(_dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m), k,
+                                           masks_per_batch, q0, q1, _flags(engine), ctypes.byref(sink), _dptr(ws),
+                                           ws.numel(), _stream(stream))
+    else:
+        e = np.ascontiguousarray(np.asarray(eps, dtype=np.float32).ravel())
+        assert len(e) == len(m)
+        rc = lib().snaps_range_selfjoin_sink(_dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
+                                             e.ctypes.data_as(ctypes.c_void_p), masks_per_batch, q0, q1, _flags(engine),
+                                             ctypes.byref(sink), _dptr(ws), ws.numel(), _stream(stream))
+    _check(rc)
+    if errors:
+        raise errors[0]
+    return ws
+
+
+def knn_selfjoin_sink(X, masks, k, masks_per_batch, consume, *, want=("kth", "mean", "indeg"), n_buffers=2,
+                      q_range=None, engine="auto", workspace=None, stream=None):
+    """snaps_knn_selfjoin_sink: `consume(mask_begin, mask_end, arrays)` is called once per mask group
+    with numpy views into a recycled pinned host buffer (valid only during the call)."""
+    return _run_sink("knn", X, masks, k, None, masks_per_batch, want, consume, n_buffers, q_range, engine, workspace, stream)
+
+
+def range_selfjoin_sink(X, masks, eps, masks_per_batch, consume, *, want=("count", "sumdist", "eps_mean"), n_buffers=2,
+                        q_range=None, engine="auto", workspace=None, stream=None):
+    """snaps_range_selfjoin_sink, see knn_selfjoin_sink."""
+    return _run_sink("range", X, masks, 0, eps, masks_per_batch, want, consume, n_buffers, q_range, engine, workspace, stream)
+
+
 def probe_fp32_rate(kind: int, stream=None) -> float:
+    import torch
     v = ctypes.c_double(0.0)
-    _check(lib().snaps_probe_fp32_rate(kind, ctypes.byref(v), _stream(stream)))
+    scratch = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    _check(lib().snaps_probe_fp32_rate(kind, ctypes.byref(v), _dptr(scratch), _stream(stream)))
     return float(v.value)
 
 
@@ -331,9 +450,9 @@ def knn_scores_at_k(knn_idx, knn_dist, k_j: int, stream=None):
     return out
 
 
-def range_selfjoin_grid(X, masks, eps_grid, *, sums=True, stream=None):
+def range_selfjoin_grid(X, masks, eps_grid, *, sums=True, stream=None, q_range=None, engine="auto"):
     """snaps_range_selfjoin_grid: eps_grid [n_masks, G] ascending per mask -> dict count / sumdist /
-    mean, each [n_masks, G, N]."""
+    mean, each [n_masks, G, nq]."""
     import torch
     assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
     m = _masks(masks)
@@ -341,18 +460,20 @@ def range_selfjoin_grid(X, masks, eps_grid, *, sums=True, stream=None):
     assert e.ndim == 2 and e.shape[0] == len(m)
     G = e.shape[1]
     N, n_feat = X.shape
+    q0, q1 = _qrange(q_range, N)
+    nq = q1 - q0
     dev = X.device
-    out = {"count": torch.empty((len(m), G, N), dtype=torch.int32, device=dev)}
+    out = {"count": torch.empty((len(m), G, nq), dtype=torch.int32, device=dev)}
     if sums:
-        out["sumdist"] = torch.empty((len(m), G, N), dtype=torch.float32, device=dev)
-        out["mean"] = torch.empty((len(m), G, N), dtype=torch.float32, device=dev)
-    nbytes = int(lib().snaps_range_grid_workspace_bytes(N, n_feat, len(m), G))
+        out["sumdist"] = torch.empty((len(m), G, nq), dtype=torch.float32, device=dev)
+        out["mean"] = torch.empty((len(m), G, nq), dtype=torch.float32, device=dev)
+    nbytes = int(lib().snaps_range_grid_workspace_bytes(N, n_feat, len(m), G, _flags(engine)))
     if nbytes == 0:
         raise SnapsError(1, "invalid sizes for the radius-grid workspace")
     ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
     _check(lib().snaps_range_selfjoin_grid(
         _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
-        e.ctypes.data_as(ctypes.c_void_p), G, _dptr(out["count"]), _dptr(out.get("sumdist")),
+        e.ctypes.data_as(ctypes.c_void_p), G, q0, q1, _flags(engine), _dptr(out["count"]), _dptr(out.get("sumdist")),
         _dptr(out.get("mean")), _dptr(ws), ws.numel(), _stream(stream)))
     out["_workspace"] = ws
     return out
@@ -369,7 +490,7 @@ def knn_select_k(knn_idx, knn_dist, k_grid, n_top: int, stream=None):
     out = {"j_indeg": torch.empty(n_masks, dtype=torch.int32, device=dev),
            "j_mean": torch.empty(n_masks, dtype=torch.int32, device=dev),
            "u": torch.empty((4, G, n_masks), dtype=torch.float32, device=dev)}
-    ws = torch.empty(int(lib().snaps_select_k_workspace_bytes(N, n_masks)), dtype=torch.uint8, device=dev)
+    ws = torch.empty(int(lib().snaps_select_k_workspace_bytes(N, n_masks, G)), dtype=torch.uint8, device=dev)
     _check(lib().snaps_knn_select_k(N, n_masks, k_max, _dptr(knn_idx), _dptr(knn_dist),
                                     grid.ctypes.data_as(ctypes.c_void_p), G, n_top, _dptr(out["j_indeg"]),
                                     _dptr(out["j_mean"]), _dptr(out["u"]), _dptr(ws), ws.numel(), _stream(stream)))

@@ -1,45 +1,61 @@
-"""Build libsnaps.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+"""Build libsnaps.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+
+Each .cu is compiled to an object under csrc/build/ (in parallel, only when stale), then linked."""
 from __future__ import annotations
 
 import os
 import subprocess
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
+OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(_HERE, "libsnaps.so")
-SOURCES = ["api.cu", "knn_lattice.cu", "range_lattice.cu", "misc_kernels.cu", "pivot_sort.cu", "ranking.cu", "range_grid.cu", "eps_search.cu"]
+SOURCES = ["api.cu", "knn_lattice.cu", "range_lattice.cu", "misc_kernels.cu", "ranking.cu", "range_grid.cu",
+           "eps_search.cu", "grid_index.cu", "grid_join.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     # no implicit mul+add contraction: the kernels place their FMAs explicitly so that the
     # main loop and the rare paths round identically
     "-fmad=false",
-    "-Xcompiler", "-fPIC", "-shared",
-    "-diag-suppress", "177",   # phase-clock variables that only the developer stats build reads
+    "-Xcompiler", "-fPIC",
 ]
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
+def _headers_mtime() -> float:
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
     deps.append(os.path.join(os.path.dirname(_HERE), "include", "snaps.h"))
-    return any(os.path.getmtime(d) > t for d in deps)
+    return max(os.path.getmtime(d) for d in deps)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or _stale():
-        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        tmp = LIB + f".{os.getpid()}.tmp"
-        extra = os.environ.get("SNAPS_NVCC_EXTRA", "").split()   # developer builds, e.g. -DSNAPS_STATS
-        cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
-        if verbose:
-            cmd.insert(1, "-Xptxas=-v")
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    os.makedirs(OBJ, exist_ok=True)
+    hdr = _headers_mtime()
+    todo = []
+    for s in SOURCES:
+        src, obj = os.path.join(CSRC, s), os.path.join(OBJ, s[:-3] + ".o")
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(src), hdr):
+            todo.append((src, obj))
+
+    def compile_one(so):
+        src, obj = so
+        tmp = obj + f".{os.getpid()}.tmp"
+        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas=-v"] if verbose else []), "-c", "-o", tmp, src]
         subprocess.run(cmd, check=True)
+        os.replace(tmp, obj)
+
+    if todo:
+        with ThreadPoolExecutor(max_workers=min(len(todo), os.cpu_count() or 4)) as ex:
+            list(ex.map(compile_one, todo))
+    objs = [os.path.join(OBJ, s[:-3] + ".o") for s in SOURCES]
+    if todo or not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(o) for o in objs):
+        tmp = LIB + f".{os.getpid()}.tmp"
+        subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp, *objs], check=True)
         os.replace(tmp, LIB)
     return LIB
 
 
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force="-f" in sys.argv, verbose="-v" in sys.argv))

@@ -1,5 +1,6 @@
 // api.cu -- C ABI of libsnaps (include/snaps.h): argument checks, the host-side mask-batch
-// planner (step a2), workspace carving, kernel launches and the pinned-host output ring (a8).
+// planner (step a2), engine selection, workspace carving, kernel launches and the batched
+// output paths (a8: staging ring, side-stream D2H, pinned-host destinations or a recycling sink).
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdarg.h>
@@ -13,10 +14,11 @@
 #include <vector>
 
 #include "../../include/snaps.h"
+#include "eps_search.cuh"
+#include "grid_index.cuh"
+#include "grid_join.cuh"
 #include "knn_lattice.cuh"
 #include "misc_kernels.cuh"
-#include "pivot_sort.cuh"
-#include "eps_search.cuh"
 #include "range_grid.cuh"
 #include "range_lattice.cuh"
 #include "ranking.cuh"
@@ -43,31 +45,55 @@ snaps_status fail(snaps_status code, const char* fmt, ...) {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// ---- optional event pairs around the join kernels (snaps_profile_*) ----
-bool g_prof_on = false;
-std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_prof_pool;  // created once, reused
-size_t g_prof_used = 0;
+// ---- optional event pairs around the join kernels (snaps_profile_*), per calling thread ----
+struct Prof {
+    bool on = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> pool;  // created once, reused
+    size_t used = 0;
+};
+thread_local Prof g_prof;
 
-void prof_reset() { g_prof_used = 0; }
+void prof_reset() { g_prof.used = 0; }
 
 bool prof_begin(cudaStream_t st) {
-    if (!g_prof_on) return false;
-    if (g_prof_used == g_prof_pool.size()) {
+    if (!g_prof.on) return false;
+    if (g_prof.used == g_prof.pool.size()) {
         cudaEvent_t a, b;
         if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return false;
-        g_prof_pool.emplace_back(a, b);
+        g_prof.pool.emplace_back(a, b);
     }
-    cudaEventRecord(g_prof_pool[g_prof_used].first, st);
+    cudaEventRecord(g_prof.pool[g_prof.used].first, st);
     return true;
 }
 
 void prof_end(bool began, cudaStream_t st) {
     if (!began) return;
-    cudaEventRecord(g_prof_pool[g_prof_used].second, st);
-    ++g_prof_used;
+    cudaEventRecord(g_prof.pool[g_prof.used].second, st);
+    ++g_prof.used;
+}
+
+// ---- side stream and events of the batched calls, per calling thread, created on first use ----
+struct Side {
+    cudaStream_t stream = nullptr;
+    cudaEvent_t computed[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+};
+thread_local Side g_side;
+
+cudaError_t side_get(Side** out) {
+    if (!g_side.stream) {
+        cudaError_t e = cudaStreamCreateWithFlags(&g_side.stream, cudaStreamNonBlocking);
+        for (int s = 0; s < 2 && e == cudaSuccess; ++s) {
+            e = cudaEventCreateWithFlags(&g_side.computed[s], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g_side.copied[s], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) return e;
+    }
+    *out = &g_side;
+    return cudaSuccess;
 }
 
 int n_tiles_for(int64_t N) { return static_cast<int>((N + snaps::kTileRows - 1) / snaps::kTileRows); }
+int n_blocks_for(int64_t N) { return static_cast<int>((N + 31) / 32); }
 
 // Gray rank of the 9 high-feature bits: consecutive batches differ in one feature, which is
 // what makes the previous batch's neighbours good threshold seeds.
@@ -77,9 +103,9 @@ uint32_t gray_rank(uint32_t gray) {
     return b;
 }
 
-// Step a2.  One batch per distinct set H of features 6..14; slot[T] = position of mask H|T.
-// A mask listed more than once gets a further batch with the same H.
-void plan_lattice(const uint16_t* masks, int n_masks, const float* thr,
+// Step a2.  One batch per distinct set H of features 6..14; slot[T] = position of mask H|T
+// (+ slot_base).  A mask listed more than once gets a further batch with the same H.
+void plan_lattice(const uint16_t* masks, int n_masks, const float* thr, int slot_base,
                   std::vector<snaps::BatchDesc>* out) {
     std::map<uint32_t, std::vector<int>> by_h;  // gray rank of H -> batch indices
     std::vector<snaps::BatchDesc>& B = *out;
@@ -98,8 +124,7 @@ void plan_lattice(const uint16_t* masks, int n_masks, const float* thr,
             snaps::BatchDesc d;
             d.hmask = H;
             d.n_valid = 0;
-            d.pivot = (H >> snaps::kLow) ? snaps::kLow + __builtin_ctz(H >> snaps::kLow) : -1;
-            d.pad_ = 0;
+            d.pad_[0] = d.pad_[1] = 0;
             for (int t = 0; t < snaps::kLat; ++t) {
                 d.slot[t] = -1;
                 d.thr[t] = -1.f;
@@ -108,7 +133,7 @@ void plan_lattice(const uint16_t* masks, int n_masks, const float* thr,
             use = static_cast<int>(B.size()) - 1;
             lst.push_back(use);
         }
-        B[use].slot[T] = m;
+        B[use].slot[T] = slot_base + m;
         B[use].n_valid += 1;
         if (thr) B[use].thr[T] = thr[m];
     }
@@ -119,148 +144,126 @@ void plan_lattice(const uint16_t* masks, int n_masks, const float* thr,
     B.swap(ordered);
 }
 
-// Pivot sweep only: a batch without high features has no pivot and would take a full pass.  Split
-// it by lattice feature instead -- the masks that contain feature 0, then of the rest those that
-// contain feature 1, ... -- so that every piece has a feature all its masks share (its pivot).
-void split_for_sweep(std::vector<snaps::BatchDesc>* batches) {
-    std::vector<snaps::BatchDesc> out;
-    for (const snaps::BatchDesc& b : *batches) {
-        if (b.pivot >= 0) {
-            out.push_back(b);
-            continue;
-        }
-        bool taken[snaps::kLat] = {false};
-        for (int f = 0; f < snaps::kLow; ++f) {
-            snaps::BatchDesc d = b;
-            d.n_valid = 0;
-            d.pivot = f;
-            for (int t = 0; t < snaps::kLat; ++t) {
-                const bool mine = b.slot[t] >= 0 && !taken[t] && ((t >> f) & 1);
-                if (mine) {
-                    taken[t] = true;
-                    d.n_valid += 1;
-                } else {
-                    d.slot[t] = -1;
-                    d.thr[t] = -1.f;
-                }
-            }
-            if (d.n_valid > 0) out.push_back(d);
-        }
-    }
-    batches->swap(out);
+int popcount16(uint32_t m) { return __builtin_popcount(m & 0xffffu); }
+
+// ---- what every join call shares ---------------------------------------------------------
+struct Job {
+    const float* X;          // caller's table (device, or host with SNAPS_FLAG_X_ON_HOST)
+    int64_t N;
+    int n_feat;
+    int64_t ld;
+    const uint16_t* h_masks;
+    int n_masks;
+    int64_t q_begin, q_end;
+    int flags;
+    int engine;
+    int64_t nq() const { return q_end - q_begin; }
+};
+
+int resolve_engine(int flags, int64_t N, int k) {
+    const int e = flags & SNAPS_ENGINE_MASK;
+    if (e != SNAPS_ENGINE_AUTO) return e;
+    return (N >= (1 << 18) || k > SNAPS_LATTICE_MAX_K) ? SNAPS_ENGINE_GRID : SNAPS_ENGINE_LATTICE;
 }
 
-snaps_status check_common(const float* d_X, int64_t N, int n_feat, int64_t ld,
-                          const uint16_t* h_masks, int n_masks) {
-    if (!d_X) return fail(SNAPS_INVALID_ARG, "d_X is NULL");
-    if (reinterpret_cast<uintptr_t>(d_X) % 4 != 0) return fail(SNAPS_INVALID_ARG, "d_X not 4-byte aligned");
-    if (N < 2) return fail(SNAPS_INVALID_ARG, "N = %lld < 2", (long long)N);
-    if (N > (int64_t)1 << 30) return fail(SNAPS_UNSUPPORTED, "N = %lld > 2^30", (long long)N);
-    if (n_feat < 1 || n_feat > SNAPS_MAX_FEATURES)
-        return fail(SNAPS_INVALID_ARG, "n_feat = %d outside 1..15", n_feat);
-    if (ld < n_feat) return fail(SNAPS_INVALID_ARG, "ld = %lld < n_feat", (long long)ld);
-    if (!h_masks || n_masks < 1) return fail(SNAPS_INVALID_ARG, "no masks");
-    for (int m = 0; m < n_masks; ++m) {
-        if (h_masks[m] == 0) return fail(SNAPS_INVALID_ARG, "mask %d is zero", m);
-        if ((h_masks[m] >> n_feat) != 0)
-            return fail(SNAPS_INVALID_ARG, "mask %d (0x%x) has a bit >= n_feat", m, h_masks[m]);
+snaps_status check_job(const Job& j, int k_for_engine) {
+    if (!j.X) return fail(SNAPS_INVALID_ARG, "X is NULL");
+    if (reinterpret_cast<uintptr_t>(j.X) % 4 != 0) return fail(SNAPS_INVALID_ARG, "X not 4-byte aligned");
+    if (j.N < 2) return fail(SNAPS_INVALID_ARG, "N = %lld < 2", (long long)j.N);
+    if (j.N > (int64_t)1 << 30) return fail(SNAPS_UNSUPPORTED, "N = %lld > 2^30", (long long)j.N);
+    if (j.n_feat < 1 || j.n_feat > SNAPS_MAX_FEATURES)
+        return fail(SNAPS_INVALID_ARG, "n_feat = %d outside 1..15", j.n_feat);
+    if (j.ld < j.n_feat) return fail(SNAPS_INVALID_ARG, "ld = %lld < n_feat", (long long)j.ld);
+    if (!j.h_masks || j.n_masks < 1) return fail(SNAPS_INVALID_ARG, "no masks");
+    for (int m = 0; m < j.n_masks; ++m) {
+        if (j.h_masks[m] == 0) return fail(SNAPS_INVALID_ARG, "mask %d is zero", m);
+        if ((j.h_masks[m] >> j.n_feat) != 0)
+            return fail(SNAPS_INVALID_ARG, "mask %d (0x%x) has a bit >= n_feat", m, j.h_masks[m]);
     }
+    if (j.q_begin < 0 || j.q_end > j.N || j.q_begin >= j.q_end)
+        return fail(SNAPS_INVALID_ARG, "query range [%lld, %lld) not within [0, N)", (long long)j.q_begin,
+                    (long long)j.q_end);
+    if (j.flags & ~(SNAPS_ENGINE_MASK | SNAPS_FLAG_X_ON_HOST)) return fail(SNAPS_INVALID_ARG, "unknown flag bits 0x%x", j.flags);
+    if (j.engine != SNAPS_ENGINE_LATTICE && j.engine != SNAPS_ENGINE_GRID)
+        return fail(SNAPS_INVALID_ARG, "unknown engine %d", j.engine);
+    if (j.engine == SNAPS_ENGINE_LATTICE && k_for_engine > SNAPS_LATTICE_MAX_K)
+        return fail(SNAPS_INVALID_ARG, "k = %d: the sub-lattice engine holds k <= %d", k_for_engine, SNAPS_LATTICE_MAX_K);
     return SNAPS_OK;
 }
 
-// Large tables take the pivot sweep (pivot_sort.cuh); SNAPS_KNN_SWEEP=0/1 overrides the size rule.
-bool use_sweep(int64_t N) {
-    if (const char* e = getenv("SNAPS_KNN_SWEEP")) return atoi(e) != 0;
-    return N >= (1 << 18);
-}
-
+// ---- workspace ---------------------------------------------------------------------------
+// common:   [host-X copy] | Xp | counter(256)
+// lattice:  Xb | batch descriptors (n_masks)
+// grid:     device masks | plans | radii (n_masks x 32 floats) | table region | index region
+// then:     whatever the caller added (staging ring, radius grid)
 struct Workspace {
-    unsigned char* pivot;   // 9 pivot sets + sort scratch (only when use_sweep(N))
+    float* Xdense;             // dense copy of a host X, else nullptr
     float* Xp;
+    unsigned long long* counter;
     float4* Xb;
-    int* counter;
     snaps::BatchDesc* batches;
-    unsigned char* ring;   // rest
-    size_t ring_bytes;
+    uint16_t* d_masks;
+    snaps::GridPlan* plans;
+    float* radii;
+    unsigned char* grid_table;
+    unsigned char* grid_index;
+    size_t grid_index_bytes;
+    unsigned char* extra;
+    size_t extra_bytes;
 };
 
-int n_blocks_for(int64_t N) { return static_cast<int>((N + 31) / 32); }
-
-
-
-// one pivot set: sorted blocked table, sorted values, position -> id, id -> position
-size_t pivot_set_bytes(int64_t N) {
-    const size_t n_pad = static_cast<size_t>(n_blocks_for(N)) * 32;
-    return align_up(n_pad * 64, 256) + 2 * align_up(n_pad * 4, 256) + align_up(static_cast<size_t>(N) * 4, 256);
+size_t base_workspace_bytes(int64_t N, int n_feat, int n_masks, int engine, int flags) {
+    size_t b = 0;
+    if (flags & SNAPS_FLAG_X_ON_HOST) b += align_up(static_cast<size_t>(N) * n_feat * 4, 256);
+    b += align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256) + 256;
+    if (engine == SNAPS_ENGINE_LATTICE) {
+        b += align_up(static_cast<size_t>(n_blocks_for(N)) * 2048, 256);
+        b += align_up(static_cast<size_t>(n_masks) * sizeof(snaps::BatchDesc), 256);
+    } else {
+        b += align_up(static_cast<size_t>(n_masks) * 2, 256);
+        b += align_up(static_cast<size_t>(n_masks) * sizeof(snaps::GridPlan), 256);
+        b += align_up(static_cast<size_t>(n_masks) * 32 * 4, 256);
+        b += snaps::grid_table_bytes(N) + snaps::grid_index_bytes(N);
+    }
+    return b;
 }
 
-size_t pivot_region_bytes(int64_t N) {
-    return 15 * pivot_set_bytes(N) + align_up(snaps::pivot_sort_temp_bytes(n_blocks_for(N) * 32), 256);
-}
-
-size_t base_workspace_bytes(int64_t N, int n_masks, int k) {
-    const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
-    const size_t blocked = align_up(static_cast<size_t>(n_blocks_for(N)) * 2048, 256);
-    const size_t batches = align_up(static_cast<size_t>(n_masks) * sizeof(snaps::BatchDesc), 256);
-    const size_t pivot = use_sweep(N) ? pivot_region_bytes(N) : 0;
-    return table + blocked + 256 + batches + pivot;
-}
-
-snaps_status carve(void* d_ws, size_t bytes, int64_t N, int n_masks, int k, Workspace* w) {
+snaps_status carve(void* d_ws, size_t bytes, const Job& j, Workspace* w) {
     if (!d_ws) return fail(SNAPS_INVALID_ARG, "d_workspace is NULL");
     if (reinterpret_cast<uintptr_t>(d_ws) % 256 != 0)
         return fail(SNAPS_INVALID_ARG, "d_workspace not 256-byte aligned");
-    const size_t need = base_workspace_bytes(N, n_masks, k);
-    if (bytes < need)
-        return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", bytes, need);
+    const size_t need = base_workspace_bytes(j.N, j.n_feat, j.n_masks, j.engine, j.flags);
+    if (bytes < need) return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", bytes, need);
     unsigned char* p = static_cast<unsigned char*>(d_ws);
-    const size_t table = align_up(static_cast<size_t>(n_tiles_for(N)) * snaps::kTileBytes, 256);
-    const size_t blocked = align_up(static_cast<size_t>(n_blocks_for(N)) * 2048, 256);
-    const size_t batches = align_up(static_cast<size_t>(n_masks) * sizeof(snaps::BatchDesc), 256);
-    w->Xp = reinterpret_cast<float*>(p);
-    w->Xb = reinterpret_cast<float4*>(p + table);
-    w->counter = reinterpret_cast<int*>(p + table + blocked);
-    w->batches = reinterpret_cast<snaps::BatchDesc*>(p + table + blocked + 256);
-    w->pivot = p + table + blocked + 256 + batches;
-    w->ring = p + need;
-    w->ring_bytes = bytes - need;
-    return SNAPS_OK;
-}
-
-// Pointers of pivot set j (feature j) inside the pivot region.
-struct PivotSet {
-    float4* Xs;
-    float* piv;
-    int* idmap;
-    int* pos;
-};
-
-PivotSet pivot_set(const Workspace& w, int64_t N, int j) {
-    const size_t n_pad = static_cast<size_t>(n_blocks_for(N)) * 32;
-    unsigned char* b = w.pivot + static_cast<size_t>(j) * pivot_set_bytes(N);
-    PivotSet s;
-    s.Xs = reinterpret_cast<float4*>(b);
-    s.piv = reinterpret_cast<float*>(b + align_up(n_pad * 64, 256));
-    s.idmap = reinterpret_cast<int*>(b + align_up(n_pad * 64, 256) + align_up(n_pad * 4, 256));
-    s.pos = reinterpret_cast<int*>(b + align_up(n_pad * 64, 256) + 2 * align_up(n_pad * 4, 256));
-    return s;
-}
-
-// Build the sorted copies for the pivot features the batches use (lowest high feature of each).
-snaps_status build_pivots(const Workspace& w, int64_t N, const std::vector<snaps::BatchDesc>& batches,
-                          cudaStream_t st) {
-    bool need[15] = {false};
-    for (const snaps::BatchDesc& b : batches)
-        if (b.pivot >= 0) need[b.pivot] = true;
-    const int n_pad = n_blocks_for(N) * 32;
-    void* temp = w.pivot + 15 * pivot_set_bytes(N);
-    const size_t temp_bytes = snaps::pivot_sort_temp_bytes(n_pad);
-    for (int j = 0; j < 15; ++j) {
-        if (!need[j]) continue;
-        const PivotSet s = pivot_set(w, N, j);
-        CUDA_TRY(snaps::pivot_build(w.Xp, static_cast<int>(N), n_pad, j, s.Xs, s.piv, s.idmap,
-                                    s.pos, temp, temp_bytes, st));
+    memset(w, 0, sizeof(*w));
+    if (j.flags & SNAPS_FLAG_X_ON_HOST) {
+        w->Xdense = reinterpret_cast<float*>(p);
+        p += align_up(static_cast<size_t>(j.N) * j.n_feat * 4, 256);
     }
+    w->Xp = reinterpret_cast<float*>(p);
+    p += align_up(static_cast<size_t>(n_tiles_for(j.N)) * snaps::kTileBytes, 256);
+    w->counter = reinterpret_cast<unsigned long long*>(p);
+    p += 256;
+    if (j.engine == SNAPS_ENGINE_LATTICE) {
+        w->Xb = reinterpret_cast<float4*>(p);
+        p += align_up(static_cast<size_t>(n_blocks_for(j.N)) * 2048, 256);
+        w->batches = reinterpret_cast<snaps::BatchDesc*>(p);
+        p += align_up(static_cast<size_t>(j.n_masks) * sizeof(snaps::BatchDesc), 256);
+    } else {
+        w->d_masks = reinterpret_cast<uint16_t*>(p);
+        p += align_up(static_cast<size_t>(j.n_masks) * 2, 256);
+        w->plans = reinterpret_cast<snaps::GridPlan*>(p);
+        p += align_up(static_cast<size_t>(j.n_masks) * sizeof(snaps::GridPlan), 256);
+        w->radii = reinterpret_cast<float*>(p);
+        p += align_up(static_cast<size_t>(j.n_masks) * 32 * 4, 256);
+        w->grid_table = p;
+        p += snaps::grid_table_bytes(j.N);
+        w->grid_index = p;
+        w->grid_index_bytes = snaps::grid_index_bytes(j.N);
+        p += w->grid_index_bytes;
+    }
+    w->extra = p;
+    w->extra_bytes = bytes - need;
     return SNAPS_OK;
 }
 
@@ -278,62 +281,452 @@ int sm_count() {
 }
 
 int knn_warps_for(int k) {
-    // per-warp list state in shared memory; what is left of the 256 KB array stays L1 for the
-    // table stream
-    const size_t budget = 227 * 1024;
+    // per-warp list state in shared memory: as many warps (queries) per CTA as fit the 227 KB
     int w = snaps::kKnnMaxThreads / 32;
-    if (const char* e = getenv("SNAPS_KNN_WARPS")) {   // tuning knob: warps (queries) per CTA
-        const int v = atoi(e);
-        if (v >= 1 && v <= snaps::kKnnMaxThreads / 32 && snaps::knn_lattice_smem_bytes(k, v) <= 227 * 1024) return v;
-    }
-    while (w > 1 && snaps::knn_lattice_smem_bytes(k, w) > budget) --w;
+    while (w > 1 && snaps::knn_lattice_smem_bytes(k, w) > 227 * 1024) --w;
     return w;
 }
 
-// Launch the kNN kernel over descriptors already uploaded at d_batches[0..nb).
-snaps_status knn_enqueue(const Workspace& w, const snaps::BatchDesc* d_batches, int nb, int64_t N, int k,
-                         int32_t* out_idx, float* out_dist, float* out_kth, float* out_mean,
-                         int32_t* out_indeg, cudaStream_t st) {
-    CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
-    snaps::KnnParams p;
-    p.Xp = w.Xp;
-    p.Xb = w.Xb;
-    p.n_blocks = n_blocks_for(N);
-    p.sweep = use_sweep(N) ? 1 : 0;
-    for (int j = 0; j < 15; ++j) {
-        const PivotSet s = p.sweep ? pivot_set(w, N, j) : PivotSet{nullptr, nullptr, nullptr, nullptr};
-        p.Xs[j] = s.Xs;
-        p.piv[j] = s.piv;
-        p.idmap[j] = s.idmap;
-        p.pos[j] = s.pos;
+// ---- a1 and the engine's table-level state -----------------------------------------------
+struct Engine {
+    Job job;
+    Workspace w;
+    cudaStream_t st;
+    snaps::GridTable gt;
+    snaps::GridIndex gi;
+};
+
+snaps_status engine_begin(Engine* E) {
+    const Job& j = E->job;
+    Workspace& w = E->w;
+    const float* Xdev = j.X;
+    int64_t ld = j.ld;
+    if (j.flags & SNAPS_FLAG_X_ON_HOST) {
+        CUDA_TRY(cudaMemcpy2DAsync(w.Xdense, static_cast<size_t>(j.n_feat) * 4, j.X, static_cast<size_t>(j.ld) * 4,
+                                   static_cast<size_t>(j.n_feat) * 4, static_cast<size_t>(j.N), cudaMemcpyHostToDevice,
+                                   E->st));
+        Xdev = w.Xdense;
+        ld = j.n_feat;
     }
-    p.N = static_cast<int>(N);
+    CUDA_TRY(snaps::stage_table_launch(Xdev, ld, static_cast<int>(j.N), j.n_feat, w.Xp,
+                                       n_tiles_for(j.N) * snaps::kTileRows, E->st));
+    if (j.engine == SNAPS_ENGINE_LATTICE) {
+        CUDA_TRY(snaps::stage_blocked_launch(Xdev, ld, static_cast<int>(j.N), j.n_feat, w.Xb, n_blocks_for(j.N), E->st));
+    } else {
+        CUDA_TRY(snaps::grid_table_build(w.Xp, static_cast<int>(j.N), j.n_feat, &E->gt, w.grid_table, w.grid_index,
+                                         w.grid_index_bytes, E->st));
+        snaps::grid_index_carve(w.grid_index, w.grid_index_bytes, j.N, &E->gi);
+        CUDA_TRY(cudaMemcpyAsync(w.d_masks, j.h_masks, static_cast<size_t>(j.n_masks) * 2, cudaMemcpyHostToDevice, E->st));
+        CUDA_TRY(snaps::grid_plan_launch(w.d_masks, j.n_masks, j.N, E->gt, w.plans, E->st));
+    }
+    return SNAPS_OK;
+}
+
+// The outputs of one launch group: pointers to the group's first mask row.
+struct KnnOut {
+    int32_t* idx;
+    float* dist;
+    float* kth;
+    float* mean;
+    int32_t* indeg;
+};
+struct RangeOut {
+    uint32_t* count;
+    float* sum;
+    float* mean;
+};
+
+// ---- sub-lattice engine launches (descriptors already on the device) -----------------------
+snaps_status lattice_knn_enqueue(Engine* E, const snaps::BatchDesc* d_batches, int nb, int k, const KnnOut& o) {
+    const Job& j = E->job;
+    CUDA_TRY(cudaMemsetAsync(E->w.counter, 0, 256, E->st));
+    snaps::KnnParams p;
+    p.Xp = E->w.Xp;
+    p.Xb = E->w.Xb;
+    p.n_blocks = n_blocks_for(j.N);
+    p.N = static_cast<int>(j.N);
+    p.q_begin = static_cast<int>(j.q_begin);
+    p.nq = static_cast<int>(j.nq());
     p.k = k;
     p.batches = d_batches;
     p.n_batches = nb;
     p.warps = knn_warps_for(k);
     // runs of 8 consecutive batches: long enough for the previous batch's neighbours to seed the
     // next one, short enough that the in-degree rows of the batches in flight (8 x 64 x 4N bytes)
-    // stay in L2; items are plentiful (N per run), so the per-warp scheduler balances the tail
-    int run = 8;
-    if (const char* e = getenv("SNAPS_KNN_RUN")) {      // tuning knob: batches per work item
-        const int v = atoi(e);
-        if (v >= 1) run = v;
-    }
-    p.batches_per_item = std::min(nb, run);
+    // stay in L2; items are plentiful (nq per run), so the per-warp scheduler balances the tail
+    p.batches_per_item = std::min(nb, 8);
     p.n_bchunks = (nb + p.batches_per_item - 1) / p.batches_per_item;
-    p.work_counter = reinterpret_cast<unsigned long long*>(w.counter);
-    p.out_idx = out_idx;
-    p.out_dist = out_dist;
-    p.out_kth = out_kth;
-    p.out_mean = out_mean;
-    p.out_indeg = out_indeg;
-    const int64_t items = N * p.n_bchunks;
+    p.work_counter = E->w.counter;
+    p.out_idx = o.idx;
+    p.out_dist = o.dist;
+    p.out_kth = o.kth;
+    p.out_mean = o.mean;
+    p.out_indeg = o.indeg;
+    const int64_t items = j.nq() * p.n_bchunks;
     const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
-    const bool prof = prof_begin(st);
-    CUDA_TRY(snaps::knn_lattice_launch(p, grid, st));
-    prof_end(prof, st);
+    const bool prof = prof_begin(E->st);
+    CUDA_TRY(snaps::knn_lattice_launch(p, grid, E->st));
+    prof_end(prof, E->st);
     return SNAPS_OK;
+}
+
+snaps_status lattice_range_enqueue(Engine* E, const snaps::BatchDesc* d_batches, int nb, const RangeOut& o) {
+    const Job& j = E->job;
+    CUDA_TRY(cudaMemsetAsync(E->w.counter, 0, 256, E->st));
+    snaps::RangeParams p;
+    p.Xp = E->w.Xp;
+    p.Xb = E->w.Xb;
+    p.n_blocks = n_blocks_for(j.N);
+    p.N = static_cast<int>(j.N);
+    p.q_begin = static_cast<int>(j.q_begin);
+    p.nq = static_cast<int>(j.nq());
+    p.batches = d_batches;
+    p.n_batches = nb;
+    p.warps = snaps::kRangeMaxThreads / 32;
+    p.batches_per_item = std::min(nb, 8);
+    p.n_bchunks = (nb + p.batches_per_item - 1) / p.batches_per_item;
+    p.work_counter = E->w.counter;
+    p.out_count = o.count;
+    p.out_sum = o.sum;
+    p.out_mean = o.mean;
+    const int64_t items = j.nq() * p.n_bchunks;
+    const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
+    const bool prof = prof_begin(E->st);
+    CUDA_TRY(snaps::range_lattice_launch(p, grid, E->st));
+    prof_end(prof, E->st);
+    return SNAPS_OK;
+}
+
+// ---- grid engine launches: masks [m0, m0 + nm) of the job, one index + one join each --------
+void grid_params_common(Engine* E, int m, snaps::GridJoinParams* p, int* d_out) {
+    const Job& j = E->job;
+    const int d = popcount16(j.h_masks[m]);
+    memset(p, 0, sizeof(*p));
+    snaps::grid_bits_for(j.N, d, p->bits);
+    p->Xp = E->w.Xp;
+    p->Xs = E->gi.Xs;
+    p->keys = E->gi.keys;
+    p->perm = E->gi.perm;
+    p->cell_start = E->gi.cell_start;
+    p->qlist = (j.q_begin > 0 || j.q_end < j.N) ? E->gi.qlist : nullptr;
+    p->edges = E->gt.edges;
+    p->plan = E->w.plans + m;
+    p->N = static_cast<int>(j.N);
+    p->nq = static_cast<int>(j.nq());
+    p->q_begin = static_cast<int>(j.q_begin);
+    *d_out = d;
+}
+
+snaps_status grid_knn_enqueue(Engine* E, int m0, int nm, int k, const KnnOut& o) {
+    const Job& j = E->job;
+    const size_t nq = static_cast<size_t>(j.nq()), N = static_cast<size_t>(j.N);
+    for (int m = m0; m < m0 + nm; ++m) {
+        snaps::GridJoinParams p;
+        int d = 0;
+        grid_params_common(E, m, &p, &d);
+        CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, &E->gi, E->st));
+        const size_t r = static_cast<size_t>(m - m0);
+        p.k = k;
+        p.out_idx = o.idx ? o.idx + r * nq * k : nullptr;
+        p.out_dist = o.dist ? o.dist + r * nq * k : nullptr;
+        p.out_kth = o.kth ? o.kth + r * nq : nullptr;
+        p.out_mean = o.mean ? o.mean + r * nq : nullptr;
+        p.out_indeg = o.indeg ? o.indeg + r * N : nullptr;
+        const bool prof = prof_begin(E->st);
+        CUDA_TRY(snaps::grid_knn_launch(p, d, E->st));
+        prof_end(prof, E->st);
+    }
+    return SNAPS_OK;
+}
+
+// radii: device [n_masks][G] fl(eps^2) rows (G = 0: h_eps2 gives one value per mask)
+snaps_status grid_range_enqueue(Engine* E, int m0, int nm, const float* h_eps2, int G, const RangeOut& o) {
+    const Job& j = E->job;
+    const size_t nq = static_cast<size_t>(j.nq());
+    const size_t per_mask = nq * static_cast<size_t>(G > 0 ? G : 1);
+    for (int m = m0; m < m0 + nm; ++m) {
+        snaps::GridJoinParams p;
+        int d = 0;
+        grid_params_common(E, m, &p, &d);
+        CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, &E->gi, E->st));
+        const size_t r = static_cast<size_t>(m - m0);
+        p.G = G;
+        if (G > 0) p.eps2_grid = E->w.radii + static_cast<size_t>(m) * G;
+        else p.eps2 = h_eps2[m];
+        p.out_count = o.count + r * per_mask;
+        p.out_sum = o.sum ? o.sum + r * per_mask : nullptr;
+        p.out_rmean = o.mean ? o.mean + r * per_mask : nullptr;
+        const bool prof = prof_begin(E->st);
+        CUDA_TRY(snaps::grid_range_launch(p, d, E->st));
+        prof_end(prof, E->st);
+    }
+    return SNAPS_OK;
+}
+
+// fl(eps^2) and nextafter(fl(eps^2)): D <= eps <=> d^2 <= fl(eps^2) <=> d^2 < nextafter (closed ball, reading A2)
+snaps_status eps_squares(const float* h_eps, size_t n, std::vector<float>* e2, std::vector<float>* thr) {
+    e2->resize(n);
+    thr->resize(n);
+    for (size_t m = 0; m < n; ++m) {
+        if (!(h_eps[m] > 0.f) || !isfinite(h_eps[m]))
+            return fail(SNAPS_INVALID_ARG, "eps[%zu] = %g is not finite and > 0", m, (double)h_eps[m]);
+        (*e2)[m] = static_cast<float>(static_cast<double>(h_eps[m]) * static_cast<double>(h_eps[m]));
+        (*thr)[m] = nextafterf((*e2)[m], INFINITY);
+    }
+    return SNAPS_OK;
+}
+
+// ---- a8: mask groups -> staging ring -> side-stream D2H -> host destination -----------------
+// One output array of a group: bytes per mask, device staging pointer (per slot), host destination.
+struct OutArray {
+    size_t bytes_per_mask;
+    unsigned char* stage[2];
+    unsigned char* h_full;      // streamed call: the caller's full-size array (offset by mask), or
+    size_t sink_offset;         // sink call: offset inside the recycled host buffer
+    bool want;
+};
+
+struct Batched {
+    Engine* E;
+    int k;                       // 0 = range join
+    const float* h_eps2;         // range join (grid engine)
+    int masks_per_batch;
+    OutArray arr[5];             // knn: idx, dist, kth, mean, indeg; range: count, sum, mean
+    int n_arr;
+    const snaps_batch_sink* sink;   // nullptr = full-size pinned arrays
+};
+
+size_t ring_bytes(int64_t nq, int64_t N, int k, int mpb) {
+    // two staging slots, each: two list arrays, two score arrays and the in-degree rows (kNN); the range
+    // join's count, sum and mean fit the same space
+    const size_t m = static_cast<size_t>(mpb);
+    const size_t slot = 2 * align_up(static_cast<size_t>(nq) * k * 4 * m, 256) + 2 * align_up(static_cast<size_t>(nq) * 4 * m, 256) +
+                        align_up(static_cast<size_t>(N) * 4 * m, 256);
+    return 2 * slot;
+}
+
+snaps_status run_batched(Batched* B, const std::vector<snaps::BatchDesc>* all_batches, const std::vector<size_t>* group_off) {
+    Engine* E = B->E;
+    const Job& j = E->job;
+    Side* side = nullptr;
+    CUDA_TRY(side_get(&side));
+    // carve the staging ring
+    unsigned char* r = E->w.extra;
+    size_t left = E->w.extra_bytes;
+    for (int s = 0; s < 2; ++s)
+        for (int a = 0; a < B->n_arr; ++a) {
+            const size_t b = align_up(B->arr[a].bytes_per_mask * B->masks_per_batch, 256);
+            if (!B->arr[a].want) { B->arr[a].stage[s] = nullptr; continue; }
+            if (left < b) return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace lacks %zu bytes for the staging ring", b - left);
+            B->arr[a].stage[s] = r;
+            r += b;
+            left -= b;
+        }
+    const bool knn = B->k > 0;
+    const int indeg_arr = 4;
+    struct Pending { int m0, nm, buf; };
+    Pending prev = {0, 0, -1};
+    auto consume = [&](const Pending& pd, int slot) -> snaps_status {
+        CUDA_TRY(cudaEventSynchronize(side->copied[slot]));
+        snaps_batch_view v;
+        memset(&v, 0, sizeof(v));
+        v.mask_begin = pd.m0;
+        v.mask_end = pd.m0 + pd.nm;
+        v.q_begin = j.q_begin;
+        v.q_end = j.q_end;
+        v.N = j.N;
+        v.k = B->k;
+        unsigned char* hb = static_cast<unsigned char*>(B->sink->h_buffers[pd.buf]);
+        auto at = [&](int a) -> const void* { return B->arr[a].want ? hb + B->arr[a].sink_offset : nullptr; };
+        if (knn) {
+            v.idx = static_cast<const int32_t*>(at(0));
+            v.dist = static_cast<const float*>(at(1));
+            v.kth = static_cast<const float*>(at(2));
+            v.mean = static_cast<const float*>(at(3));
+            v.indeg = static_cast<const int32_t*>(at(4));
+        } else {
+            v.count = static_cast<const uint32_t*>(at(0));
+            v.sumdist = static_cast<const float*>(at(1));
+            v.eps_mean = static_cast<const float*>(at(2));
+        }
+        B->sink->consume(B->sink->user, &v);
+        return SNAPS_OK;
+    };
+    int group = 0;
+    for (int m0 = 0; m0 < j.n_masks; m0 += B->masks_per_batch, ++group) {
+        const int nm = std::min(B->masks_per_batch, j.n_masks - m0);
+        const int s = group & 1;
+        // staging slot s is free once its previous copy-out has finished
+        if (group >= 2) CUDA_TRY(cudaStreamWaitEvent(E->st, side->copied[s], 0));
+        snaps_status rc;
+        if (knn) {
+            KnnOut o = {reinterpret_cast<int32_t*>(B->arr[0].stage[s]), reinterpret_cast<float*>(B->arr[1].stage[s]),
+                        reinterpret_cast<float*>(B->arr[2].stage[s]), reinterpret_cast<float*>(B->arr[3].stage[s]),
+                        reinterpret_cast<int32_t*>(B->arr[indeg_arr].stage[s])};
+            if (o.indeg) CUDA_TRY(cudaMemsetAsync(o.indeg, 0, B->arr[indeg_arr].bytes_per_mask * nm, E->st));
+            if (j.engine == SNAPS_ENGINE_LATTICE)
+                rc = lattice_knn_enqueue(E, E->w.batches + (*group_off)[group],
+                                         static_cast<int>((*group_off)[group + 1] - (*group_off)[group]), B->k, o);
+            else
+                rc = grid_knn_enqueue(E, m0, nm, B->k, o);
+        } else {
+            RangeOut o = {reinterpret_cast<uint32_t*>(B->arr[0].stage[s]), reinterpret_cast<float*>(B->arr[1].stage[s]),
+                          reinterpret_cast<float*>(B->arr[2].stage[s])};
+            if (j.engine == SNAPS_ENGINE_LATTICE)
+                rc = lattice_range_enqueue(E, E->w.batches + (*group_off)[group],
+                                           static_cast<int>((*group_off)[group + 1] - (*group_off)[group]), o);
+            else
+                rc = grid_range_enqueue(E, m0, nm, B->h_eps2, 0, o);
+        }
+        if (rc != SNAPS_OK) return rc;
+        CUDA_TRY(cudaEventRecord(side->computed[s], E->st));
+        CUDA_TRY(cudaStreamWaitEvent(side->stream, side->computed[s], 0));
+        const int buf = B->sink ? group % B->sink->n_buffers : -1;
+        for (int a = 0; a < B->n_arr; ++a) {
+            if (!B->arr[a].want) continue;
+            const size_t bytes = B->arr[a].bytes_per_mask * nm;
+            unsigned char* dst = B->sink ? static_cast<unsigned char*>(B->sink->h_buffers[buf]) + B->arr[a].sink_offset
+                                         : B->arr[a].h_full + B->arr[a].bytes_per_mask * m0;
+            CUDA_TRY(cudaMemcpyAsync(dst, B->arr[a].stage[s], bytes, cudaMemcpyDeviceToHost, side->stream));
+        }
+        CUDA_TRY(cudaEventRecord(side->copied[s], side->stream));
+        if (B->sink) {
+            // the previous group is consumed (and its host buffer recycled) while this one computes
+            if (group >= 1) {
+                rc = consume(prev, (group - 1) & 1);
+                if (rc != SNAPS_OK) return rc;
+            }
+            prev = {m0, nm, buf};
+        }
+    }
+    if (B->sink) {
+        snaps_status rc = consume(prev, (group - 1) & 1);
+        if (rc != SNAPS_OK) return rc;
+    }
+    // the caller's stream completes only after the last copies have landed
+    for (int s = 0; s < 2 && s < group; ++s) CUDA_TRY(cudaStreamWaitEvent(E->st, side->copied[s], 0));
+    return SNAPS_OK;
+}
+
+// Plans every mask group of a batched sub-lattice run up front and uploads all descriptors with
+// one copy, so that the group loop only enqueues.  Slots are relative to the group's first mask.
+snaps_status lattice_plan_groups(Engine* E, const float* thr, int mpb, std::vector<snaps::BatchDesc>* all,
+                                 std::vector<size_t>* group_off) {
+    const Job& j = E->job;
+    for (int m0 = 0; m0 < j.n_masks; m0 += mpb) {
+        std::vector<snaps::BatchDesc> b;
+        plan_lattice(j.h_masks + m0, std::min(mpb, j.n_masks - m0), thr ? thr + m0 : nullptr, 0, &b);
+        group_off->push_back(all->size());
+        all->insert(all->end(), b.begin(), b.end());
+    }
+    group_off->push_back(all->size());
+    CUDA_TRY(cudaMemcpyAsync(E->w.batches, all->data(), sizeof(snaps::BatchDesc) * all->size(), cudaMemcpyHostToDevice, E->st));
+    return SNAPS_OK;
+}
+
+snaps_status sink_check(const snaps_batch_sink* sink, size_t need) {
+    if (!sink || !sink->h_buffers || !sink->consume) return fail(SNAPS_INVALID_ARG, "sink, its buffers or its consumer is NULL");
+    if (sink->n_buffers < 2) return fail(SNAPS_INVALID_ARG, "sink needs >= 2 host buffers");
+    for (int b = 0; b < sink->n_buffers; ++b)
+        if (!sink->h_buffers[b]) return fail(SNAPS_INVALID_ARG, "sink buffer %d is NULL", b);
+    if (sink->buffer_bytes < need) return fail(SNAPS_INVALID_ARG, "sink buffers hold %zu < %zu bytes", sink->buffer_bytes, need);
+    return SNAPS_OK;
+}
+
+snaps_status knn_batched(const float* X, int64_t N, int n_feat, int64_t ld, const uint16_t* h_masks, int n_masks, int k,
+                         int mpb, int64_t q_begin, int64_t q_end, int flags, void* const h_out[5], const snaps_batch_sink* sink,
+                         void* d_ws, size_t ws_bytes, void* stream) {
+    prof_reset();
+    Engine E;
+    E.job = Job{X, N, n_feat, ld, h_masks, n_masks, q_begin, q_end, flags, resolve_engine(flags, N, k)};
+    E.st = static_cast<cudaStream_t>(stream);
+    snaps_status rc = check_job(E.job, k);
+    if (rc) return rc;
+    if (k < 1 || k > SNAPS_MAX_K || k > N - 1)
+        return fail(SNAPS_INVALID_ARG, "k = %d outside 1..min(N-1, %d)", k, SNAPS_MAX_K);
+    if (mpb < 1) return fail(SNAPS_INVALID_ARG, "masks_per_batch < 1");
+    const size_t nq = static_cast<size_t>(q_end - q_begin);
+    Batched B;
+    memset(&B, 0, sizeof(B));
+    B.E = &E;
+    B.k = k;
+    B.masks_per_batch = mpb;
+    B.n_arr = 5;
+    B.sink = sink;
+    const size_t per[5] = {nq * k * 4, nq * k * 4, nq * 4, nq * 4, static_cast<size_t>(N) * 4};
+    const unsigned bits[5] = {SNAPS_OUT_IDX, SNAPS_OUT_DIST, SNAPS_OUT_KTH, SNAPS_OUT_MEAN, SNAPS_OUT_INDEG};
+    size_t off = 0;
+    bool any = false;
+    for (int a = 0; a < 5; ++a) {
+        B.arr[a].bytes_per_mask = per[a];
+        B.arr[a].want = sink ? (sink->want & bits[a]) != 0 : h_out[a] != nullptr;
+        B.arr[a].h_full = sink ? nullptr : static_cast<unsigned char*>(h_out[a]);
+        B.arr[a].sink_offset = off;
+        if (B.arr[a].want) off += align_up(per[a] * mpb, 256);
+        any |= B.arr[a].want;
+    }
+    if (!any) return fail(SNAPS_INVALID_ARG, "no output asked for");
+    if (sink) {
+        rc = sink_check(sink, off);
+        if (rc) return rc;
+    }
+    rc = carve(d_ws, ws_bytes, E.job, &E.w);
+    if (rc) return rc;
+    rc = engine_begin(&E);
+    if (rc) return rc;
+    std::vector<snaps::BatchDesc> all;
+    std::vector<size_t> group_off;
+    if (E.job.engine == SNAPS_ENGINE_LATTICE) {
+        rc = lattice_plan_groups(&E, nullptr, mpb, &all, &group_off);
+        if (rc) return rc;
+    }
+    return run_batched(&B, &all, &group_off);
+}
+
+snaps_status range_batched(const float* X, int64_t N, int n_feat, int64_t ld, const uint16_t* h_masks, int n_masks,
+                           const float* h_eps, int mpb, int64_t q_begin, int64_t q_end, int flags, const snaps_batch_sink* sink,
+                           void* d_ws, size_t ws_bytes, void* stream) {
+    prof_reset();
+    Engine E;
+    E.job = Job{X, N, n_feat, ld, h_masks, n_masks, q_begin, q_end, flags, resolve_engine(flags, N, 0)};
+    E.st = static_cast<cudaStream_t>(stream);
+    snaps_status rc = check_job(E.job, 0);
+    if (rc) return rc;
+    if (!h_eps) return fail(SNAPS_INVALID_ARG, "h_eps is NULL");
+    if (mpb < 1) return fail(SNAPS_INVALID_ARG, "masks_per_batch < 1");
+    std::vector<float> e2, thr;
+    rc = eps_squares(h_eps, n_masks, &e2, &thr);
+    if (rc) return rc;
+    const size_t nq = static_cast<size_t>(q_end - q_begin);
+    Batched B;
+    memset(&B, 0, sizeof(B));
+    B.E = &E;
+    B.k = 0;
+    B.h_eps2 = e2.data();
+    B.masks_per_batch = mpb;
+    B.n_arr = 3;
+    B.sink = sink;
+    const unsigned bits[3] = {SNAPS_OUT_COUNT, SNAPS_OUT_SUMDIST, SNAPS_OUT_EPSMEAN};
+    size_t off = 0;
+    for (int a = 0; a < 3; ++a) {
+        B.arr[a].bytes_per_mask = nq * 4;
+        B.arr[a].want = a == 0 || (sink->want & bits[a]) != 0;   // the count drives the kernel: always staged
+        B.arr[a].sink_offset = off;
+        off += align_up(nq * 4 * mpb, 256);
+    }
+    rc = sink_check(sink, off);
+    if (rc) return rc;
+    rc = carve(d_ws, ws_bytes, E.job, &E.w);
+    if (rc) return rc;
+    rc = engine_begin(&E);
+    if (rc) return rc;
+    std::vector<snaps::BatchDesc> all;
+    std::vector<size_t> group_off;
+    if (E.job.engine == SNAPS_ENGINE_LATTICE) {
+        rc = lattice_plan_groups(&E, thr.data(), mpb, &all, &group_off);
+        if (rc) return rc;
+    }
+    return run_batched(&B, &all, &group_off);
 }
 
 }  // namespace
@@ -342,120 +735,78 @@ extern "C" {
 
 const char* snaps_last_error(void) { return g_err; }
 
-const char* snaps_version(void) { return "snaps-b200 0.1 (sm_100a)"; }
+const char* snaps_version(void) { return "snaps-b200 0.2 (sm_100a)"; }
 
-size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k) {
-    if (N < 2 || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES || n_masks < 1 || k < 0 || k > SNAPS_MAX_K)
+size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k, int flags) {
+    if (N < 2 || N > ((int64_t)1 << 30) || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES || n_masks < 1 || k < 0 || k > SNAPS_MAX_K)
         return 0;
-    return base_workspace_bytes(N, n_masks, k);
+    const int engine = resolve_engine(flags, N, k);
+    if (engine != SNAPS_ENGINE_LATTICE && engine != SNAPS_ENGINE_GRID) return 0;
+    return base_workspace_bytes(N, n_feat, n_masks, engine, flags);
 }
 
 int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t* h_masks, int n_masks) {
     if (!h_masks || n_masks < 1 || N < 2 || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES) return -1;
     std::vector<snaps::BatchDesc> b;
-    plan_lattice(h_masks, n_masks, nullptr, &b);
+    plan_lattice(h_masks, n_masks, nullptr, 0, &b);
     return static_cast<int64_t>(b.size()) * snaps::kLat * N * N;
 }
 
 snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t ld,
-                                const uint16_t* h_masks, int n_masks, int k, int32_t* out_idx,
-                                float* out_dist, float* out_kth, float* out_mean,
-                                int32_t* out_indeg, void* d_workspace, size_t workspace_bytes,
-                                void* stream) {
+                                const uint16_t* h_masks, int n_masks, int k, int64_t q_begin, int64_t q_end,
+                                int flags, int32_t* out_idx, float* out_dist, float* out_kth, float* out_mean,
+                                int32_t* out_indeg, void* d_workspace, size_t workspace_bytes, void* stream) {
     prof_reset();
-    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    Engine E;
+    E.job = Job{d_X, N, n_feat, ld, h_masks, n_masks, q_begin, q_end, flags, resolve_engine(flags, N, k)};
+    E.st = static_cast<cudaStream_t>(stream);
+    snaps_status rc = check_job(E.job, k);
     if (rc) return rc;
     if (k < 1 || k > SNAPS_MAX_K || k > N - 1)
         return fail(SNAPS_INVALID_ARG, "k = %d outside 1..min(N-1, %d)", k, SNAPS_MAX_K);
     if (!out_idx && !out_dist && !out_kth && !out_mean && !out_indeg)
         return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
-    Workspace w;
-    rc = carve(d_workspace, workspace_bytes, N, n_masks, k, &w);
+    rc = carve(d_workspace, workspace_bytes, E.job, &E.w);
     if (rc) return rc;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    std::vector<snaps::BatchDesc> batches;
-    plan_lattice(h_masks, n_masks, nullptr, &batches);
-    const int n_tiles = n_tiles_for(N);
-    CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
-                                       n_tiles * snaps::kTileRows, st));
-    CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
-    if (use_sweep(N)) {
-        split_for_sweep(&batches);
-        rc = build_pivots(w, N, batches, st);
-        if (rc) return rc;
-    }
+    rc = engine_begin(&E);
+    if (rc) return rc;
     if (out_indeg)
-        CUDA_TRY(cudaMemsetAsync(out_indeg, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, st));
-    CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
-                             cudaMemcpyHostToDevice, st));
-    return knn_enqueue(w, w.batches, static_cast<int>(batches.size()), N, k, out_idx, out_dist, out_kth,
-                       out_mean, out_indeg, st);
+        CUDA_TRY(cudaMemsetAsync(out_indeg, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, E.st));
+    const KnnOut o = {out_idx, out_dist, out_kth, out_mean, out_indeg};
+    if (E.job.engine == SNAPS_ENGINE_GRID) return grid_knn_enqueue(&E, 0, n_masks, k, o);
+    std::vector<snaps::BatchDesc> batches;
+    plan_lattice(h_masks, n_masks, nullptr, 0, &batches);
+    CUDA_TRY(cudaMemcpyAsync(E.w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
+                             cudaMemcpyHostToDevice, E.st));
+    return lattice_knn_enqueue(&E, E.w.batches, static_cast<int>(batches.size()), k, o);
 }
 
 snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t ld,
-                                  const uint16_t* h_masks, int n_masks, const float* h_eps,
-                                  uint32_t* out_count, float* out_sumdist, float* out_mean,
+                                  const uint16_t* h_masks, int n_masks, const float* h_eps, int64_t q_begin,
+                                  int64_t q_end, int flags, uint32_t* out_count, float* out_sumdist, float* out_mean,
                                   void* d_workspace, size_t workspace_bytes, void* stream) {
     prof_reset();
-    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    Engine E;
+    E.job = Job{d_X, N, n_feat, ld, h_masks, n_masks, q_begin, q_end, flags, resolve_engine(flags, N, 0)};
+    E.st = static_cast<cudaStream_t>(stream);
+    snaps_status rc = check_job(E.job, 0);
     if (rc) return rc;
     if (!h_eps) return fail(SNAPS_INVALID_ARG, "h_eps is NULL");
     if (!out_count) return fail(SNAPS_INVALID_ARG, "out_count is NULL");
-    std::vector<float> thr(n_masks);
-    for (int m = 0; m < n_masks; ++m) {
-        if (!(h_eps[m] > 0.f) || !isfinite(h_eps[m]))
-            return fail(SNAPS_INVALID_ARG, "eps[%d] = %g is not finite and > 0", m, (double)h_eps[m]);
-        // D <= eps  <=>  D^2 <= eps^2: compare d^2 < nextafter(fl(eps^2)) (closed ball, reading A2)
-        const float e2 = static_cast<float>(static_cast<double>(h_eps[m]) * static_cast<double>(h_eps[m]));
-        thr[m] = nextafterf(e2, INFINITY);
-    }
-    Workspace w;
-    rc = carve(d_workspace, workspace_bytes, N, n_masks, 1, &w);
+    std::vector<float> e2, thr;
+    rc = eps_squares(h_eps, n_masks, &e2, &thr);
     if (rc) return rc;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rc = carve(d_workspace, workspace_bytes, E.job, &E.w);
+    if (rc) return rc;
+    rc = engine_begin(&E);
+    if (rc) return rc;
+    const RangeOut o = {out_count, out_sumdist, out_mean};
+    if (E.job.engine == SNAPS_ENGINE_GRID) return grid_range_enqueue(&E, 0, n_masks, e2.data(), 0, o);
     std::vector<snaps::BatchDesc> batches;
-    plan_lattice(h_masks, n_masks, thr.data(), &batches);
-    if (use_sweep(N)) split_for_sweep(&batches);
-    const int nb = static_cast<int>(batches.size());
-    const int n_tiles = n_tiles_for(N);
-    CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
-                                       n_tiles * snaps::kTileRows, st));
-    CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * nb,
-                             cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
-    CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
-    if (use_sweep(N)) {
-        rc = build_pivots(w, N, batches, st);
-        if (rc) return rc;
-    }
-    snaps::RangeParams p;
-    p.Xp = w.Xp;
-    p.Xb = w.Xb;
-    p.n_blocks = n_blocks_for(N);
-    p.sweep = use_sweep(N) ? 1 : 0;
-    for (int j = 0; j < 15; ++j) {
-        const PivotSet s = p.sweep ? pivot_set(w, N, j) : PivotSet{nullptr, nullptr, nullptr, nullptr};
-        p.Xs[j] = s.Xs;
-        p.piv[j] = s.piv;
-        p.idmap[j] = s.idmap;
-        p.pos[j] = s.pos;
-    }
-    p.N = static_cast<int>(N);
-    p.batches = w.batches;
-    p.n_batches = nb;
-    p.warps = snaps::kRangeMaxThreads / 32;
-    p.batches_per_item = std::min(nb, 8);
-    p.n_bchunks = (nb + p.batches_per_item - 1) / p.batches_per_item;
-    p.work_counter = reinterpret_cast<unsigned long long*>(w.counter);
-    p.out_count = out_count;
-    p.out_sum = out_sumdist;
-    p.out_mean = out_mean;
-    const int64_t items = N * p.n_bchunks;
-    const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
-    const bool prof = prof_begin(st);
-    CUDA_TRY(snaps::range_lattice_launch(p, grid, st));
-    prof_end(prof, st);
-    return SNAPS_OK;
+    plan_lattice(h_masks, n_masks, thr.data(), 0, &batches);
+    CUDA_TRY(cudaMemcpyAsync(E.w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
+                             cudaMemcpyHostToDevice, E.st));
+    return lattice_range_enqueue(&E, E.w.batches, static_cast<int>(batches.size()), o);
 }
 
 snaps_status snaps_outlier_scores(int64_t N, int n_masks, int k, const int32_t* knn_idx,
@@ -482,139 +833,74 @@ snaps_status snaps_outlier_scores(int64_t N, int n_masks, int k, const int32_t* 
     return SNAPS_OK;
 }
 
-size_t snaps_stream_ring_bytes(int64_t N, int k, int masks_per_batch) {
-    if (N < 2 || k < 1 || masks_per_batch < 1) return 0;
-    // two staging slots, each: idx + dist lists and three score arrays for one mask group
-    const size_t per_mask = align_up(static_cast<size_t>(N) * (2 * static_cast<size_t>(k) + 3) * 4, 256) + 5 * 256;
-    return 2 * per_mask * static_cast<size_t>(masks_per_batch);
+size_t snaps_stream_ring_bytes(int64_t nq, int64_t N, int k, int masks_per_batch) {
+    if (nq < 1 || N < 2 || nq > N || k < 0 || masks_per_batch < 1) return 0;
+    return ring_bytes(nq, N, k, masks_per_batch);
+}
+
+size_t snaps_sink_batch_bytes(int64_t nq, int64_t N, int k, int masks_per_batch, unsigned want) {
+    if (nq < 1 || N < 2 || k < 0 || masks_per_batch < 1) return 0;
+    const size_t mpb = static_cast<size_t>(masks_per_batch);
+    size_t b = 0;
+    if (want & SNAPS_OUT_IDX) b += align_up(static_cast<size_t>(nq) * k * 4 * mpb, 256);
+    if (want & SNAPS_OUT_DIST) b += align_up(static_cast<size_t>(nq) * k * 4 * mpb, 256);
+    if (want & SNAPS_OUT_KTH) b += align_up(static_cast<size_t>(nq) * 4 * mpb, 256);
+    if (want & SNAPS_OUT_MEAN) b += align_up(static_cast<size_t>(nq) * 4 * mpb, 256);
+    if (want & SNAPS_OUT_INDEG) b += align_up(static_cast<size_t>(N) * 4 * mpb, 256);
+    if (want & (SNAPS_OUT_COUNT | SNAPS_OUT_SUMDIST | SNAPS_OUT_EPSMEAN)) b += 3 * align_up(static_cast<size_t>(nq) * 4 * mpb, 256);
+    return b;
 }
 
 snaps_status snaps_knn_selfjoin_streamed(const float* d_X, int64_t N, int n_feat, int64_t ld,
-                                         const uint16_t* h_masks, int n_masks, int k,
-                                         int masks_per_batch, int32_t* h_out_idx, float* h_out_dist,
-                                         float* h_out_kth, float* h_out_mean, int32_t* h_out_indeg,
-                                         void* d_workspace, size_t workspace_bytes, void* stream) {
-    prof_reset();
-    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
-    if (rc) return rc;
-    if (k < 1 || k > SNAPS_MAX_K || k > N - 1)
-        return fail(SNAPS_INVALID_ARG, "k = %d outside 1..min(N-1, %d)", k, SNAPS_MAX_K);
-    if (masks_per_batch < 1) return fail(SNAPS_INVALID_ARG, "masks_per_batch < 1");
-    if (!h_out_idx && !h_out_dist && !h_out_kth && !h_out_mean && !h_out_indeg)
-        return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
-    Workspace w;
-    rc = carve(d_workspace, workspace_bytes, N, n_masks, k, &w);
-    if (rc) return rc;
-    const size_t ring_need = snaps_stream_ring_bytes(N, k, masks_per_batch);
-    if (w.ring_bytes < ring_need)
-        return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace ring %zu < %zu bytes", w.ring_bytes, ring_need);
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const int n_tiles = n_tiles_for(N);
-    CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
-                                       n_tiles * snaps::kTileRows, st));
-    CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
-
-    const size_t mpb = static_cast<size_t>(masks_per_batch);
-    const size_t n_list = align_up(mpb * N * k * 4, 256);
-    const size_t n_score = align_up(mpb * N * 4, 256);
-    struct Slot {
-        int32_t* idx;
-        float* dist;
-        float* kth;
-        float* mean;
-        int32_t* indeg;
-    } slots[2];
-    unsigned char* r = w.ring;
-    for (int s = 0; s < 2; ++s) {
-        slots[s].idx = reinterpret_cast<int32_t*>(r); r += n_list;
-        slots[s].dist = reinterpret_cast<float*>(r); r += n_list;
-        slots[s].kth = reinterpret_cast<float*>(r); r += n_score;
-        slots[s].mean = reinterpret_cast<float*>(r); r += n_score;
-        slots[s].indeg = reinterpret_cast<int32_t*>(r); r += n_score;
-    }
-    // Plan every mask group up front and upload all descriptors with one copy, so that the
-    // loop below only enqueues (no host<->device synchronisation between groups).
-    std::vector<snaps::BatchDesc> all_batches;
-    std::vector<size_t> group_off;
-    for (int m0 = 0; m0 < n_masks; m0 += masks_per_batch) {
-        std::vector<snaps::BatchDesc> b;
-        plan_lattice(h_masks + m0, std::min(masks_per_batch, n_masks - m0), nullptr, &b);
-        if (use_sweep(N)) split_for_sweep(&b);
-        group_off.push_back(all_batches.size());
-        all_batches.insert(all_batches.end(), b.begin(), b.end());
-    }
-    group_off.push_back(all_batches.size());
-    if (use_sweep(N)) {
-        rc = build_pivots(w, N, all_batches, st);
-        if (rc) return rc;
-    }
-    CUDA_TRY(cudaMemcpyAsync(w.batches, all_batches.data(), sizeof(snaps::BatchDesc) * all_batches.size(),
-                             cudaMemcpyHostToDevice, st));
-    cudaStream_t side;
-    CUDA_TRY(cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking));
-    cudaEvent_t computed[2], copied[2];
-    for (int s = 0; s < 2; ++s) {
-        CUDA_TRY(cudaEventCreateWithFlags(&computed[s], cudaEventDisableTiming));
-        CUDA_TRY(cudaEventCreateWithFlags(&copied[s], cudaEventDisableTiming));
-    }
-    snaps_status result = SNAPS_OK;
-    int group = 0;
-    for (int m0 = 0; m0 < n_masks && result == SNAPS_OK; m0 += masks_per_batch, ++group) {
-        const int nm = std::min(masks_per_batch, n_masks - m0);
-        const int s = group & 1;
-        if (group >= 2) {
-            // staging slot s is free once its previous copy-out has finished
-            cudaError_t e = cudaStreamWaitEvent(st, copied[s], 0);
-            if (e != cudaSuccess) { result = fail(SNAPS_CUDA_ERROR, "cudaStreamWaitEvent: %s", cudaGetErrorString(e)); break; }
-        }
-        if (h_out_indeg) {
-            cudaError_t e = cudaMemsetAsync(slots[s].indeg, 0, sizeof(int32_t) * static_cast<size_t>(nm) * N, st);
-            if (e != cudaSuccess) { result = fail(SNAPS_CUDA_ERROR, "cudaMemsetAsync: %s", cudaGetErrorString(e)); break; }
-        }
-        result = knn_enqueue(w, w.batches + group_off[group],
-                             static_cast<int>(group_off[group + 1] - group_off[group]), N, k,
-                             h_out_idx ? slots[s].idx : nullptr,
-                             h_out_dist ? slots[s].dist : nullptr, h_out_kth ? slots[s].kth : nullptr,
-                             h_out_mean ? slots[s].mean : nullptr, h_out_indeg ? slots[s].indeg : nullptr, st);
-        if (result != SNAPS_OK) break;
-        cudaEventRecord(computed[s], st);
-        cudaStreamWaitEvent(side, computed[s], 0);
-        const size_t off_list = static_cast<size_t>(m0) * N * k, off_score = static_cast<size_t>(m0) * N;
-        const size_t b_list = static_cast<size_t>(nm) * N * k * 4, b_score = static_cast<size_t>(nm) * N * 4;
-        cudaError_t e = cudaSuccess;
-        if (h_out_idx && e == cudaSuccess) e = cudaMemcpyAsync(h_out_idx + off_list, slots[s].idx, b_list, cudaMemcpyDeviceToHost, side);
-        if (h_out_dist && e == cudaSuccess) e = cudaMemcpyAsync(h_out_dist + off_list, slots[s].dist, b_list, cudaMemcpyDeviceToHost, side);
-        if (h_out_kth && e == cudaSuccess) e = cudaMemcpyAsync(h_out_kth + off_score, slots[s].kth, b_score, cudaMemcpyDeviceToHost, side);
-        if (h_out_mean && e == cudaSuccess) e = cudaMemcpyAsync(h_out_mean + off_score, slots[s].mean, b_score, cudaMemcpyDeviceToHost, side);
-        if (h_out_indeg && e == cudaSuccess) e = cudaMemcpyAsync(h_out_indeg + off_score, slots[s].indeg, b_score, cudaMemcpyDeviceToHost, side);
-        if (e != cudaSuccess) { result = fail(SNAPS_CUDA_ERROR, "cudaMemcpyAsync D2H: %s", cudaGetErrorString(e)); break; }
-        cudaEventRecord(copied[s], side);
-    }
-    // the caller's stream completes only after the last copies have landed
-    for (int s = 0; s < 2 && s < group; ++s) cudaStreamWaitEvent(st, copied[s], 0);
-    for (int s = 0; s < 2; ++s) {
-        cudaEventDestroy(computed[s]);
-        cudaEventDestroy(copied[s]);
-    }
-    cudaStreamDestroy(side);
-    return result;
+                                         const uint16_t* h_masks, int n_masks, int k, int masks_per_batch,
+                                         int64_t q_begin, int64_t q_end, int flags, int32_t* h_out_idx,
+                                         float* h_out_dist, float* h_out_kth, float* h_out_mean,
+                                         int32_t* h_out_indeg, void* d_workspace, size_t workspace_bytes, void* stream) {
+    void* const h_out[5] = {h_out_idx, h_out_dist, h_out_kth, h_out_mean, h_out_indeg};
+    return knn_batched(d_X, N, n_feat, ld, h_masks, n_masks, k, masks_per_batch, q_begin, q_end, flags, h_out, nullptr,
+                       d_workspace, workspace_bytes, stream);
 }
 
-size_t snaps_range_grid_workspace_bytes(int64_t N, int n_feat, int n_masks, int G) {
+snaps_status snaps_knn_selfjoin_sink(const float* d_X, int64_t N, int n_feat, int64_t ld, const uint16_t* h_masks,
+                                     int n_masks, int k, int masks_per_batch, int64_t q_begin, int64_t q_end, int flags,
+                                     const snaps_batch_sink* sink, void* d_workspace, size_t workspace_bytes, void* stream) {
+    if (!sink) return fail(SNAPS_INVALID_ARG, "sink is NULL");
+    void* const none[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    return knn_batched(d_X, N, n_feat, ld, h_masks, n_masks, k, masks_per_batch, q_begin, q_end, flags, none, sink,
+                       d_workspace, workspace_bytes, stream);
+}
+
+snaps_status snaps_range_selfjoin_sink(const float* d_X, int64_t N, int n_feat, int64_t ld, const uint16_t* h_masks,
+                                       int n_masks, const float* h_eps, int masks_per_batch, int64_t q_begin,
+                                       int64_t q_end, int flags, const snaps_batch_sink* sink, void* d_workspace,
+                                       size_t workspace_bytes, void* stream) {
+    if (!sink) return fail(SNAPS_INVALID_ARG, "sink is NULL");
+    return range_batched(d_X, N, n_feat, ld, h_masks, n_masks, h_eps, masks_per_batch, q_begin, q_end, flags, sink,
+                         d_workspace, workspace_bytes, stream);
+}
+
+size_t snaps_range_grid_workspace_bytes(int64_t N, int n_feat, int n_masks, int G, int flags) {
     if (N < 2 || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES || n_masks < 1 || G < 1 || G > snaps::kRangeGridMaxRadii)
         return 0;
-    return base_workspace_bytes(N, n_masks, 0) + align_up(static_cast<size_t>(n_masks) * G * 4, 256);
+    const int engine = resolve_engine(flags, N, 0);
+    if (engine != SNAPS_ENGINE_LATTICE && engine != SNAPS_ENGINE_GRID) return 0;
+    return base_workspace_bytes(N, n_feat, n_masks, engine, flags) + align_up(static_cast<size_t>(n_masks) * G * 4, 256);
 }
 
 snaps_status snaps_range_selfjoin_grid(const float* d_X, int64_t N, int n_feat, int64_t ld,
                                        const uint16_t* h_masks, int n_masks, const float* h_eps_grid, int G,
-                                       uint32_t* out_count, float* out_sumdist, float* out_mean,
-                                       void* d_workspace, size_t workspace_bytes, void* stream) {
+                                       int64_t q_begin, int64_t q_end, int flags, uint32_t* out_count,
+                                       float* out_sumdist, float* out_mean, void* d_workspace, size_t workspace_bytes,
+                                       void* stream) {
     prof_reset();
-    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    Engine E;
+    E.job = Job{d_X, N, n_feat, ld, h_masks, n_masks, q_begin, q_end, flags, resolve_engine(flags, N, 0)};
+    E.st = static_cast<cudaStream_t>(stream);
+    snaps_status rc = check_job(E.job, 0);
     if (rc) return rc;
     if (!h_eps_grid || !out_count) return fail(SNAPS_INVALID_ARG, "NULL eps grid or out_count");
     if (G < 1 || G > snaps::kRangeGridMaxRadii) return fail(SNAPS_INVALID_ARG, "G = %d outside 1..%d", G, snaps::kRangeGridMaxRadii);
+    const bool grid_engine = E.job.engine == SNAPS_ENGINE_GRID;
     std::vector<float> thr(static_cast<size_t>(n_masks) * G);
     for (int m = 0; m < n_masks; ++m)
         for (int g = 0; g < G; ++g) {
@@ -622,45 +908,51 @@ snaps_status snaps_range_selfjoin_grid(const float* d_X, int64_t N, int n_feat, 
             if (!(e > 0.f) || !isfinite(e) || (g > 0 && !(e > h_eps_grid[static_cast<size_t>(m) * G + g - 1])))
                 return fail(SNAPS_INVALID_ARG, "eps_grid[%d][%d] = %g: radii must be finite, > 0 and ascending", m, g, (double)e);
             const float e2 = static_cast<float>(static_cast<double>(e) * static_cast<double>(e));
-            thr[static_cast<size_t>(m) * G + g] = nextafterf(e2, INFINITY);   // closed ball, reading A2
+            // closed ball, reading A2: d^2 <= fl(eps^2) (grid engine) <=> d^2 < nextafter (sub-lattice engine)
+            thr[static_cast<size_t>(m) * G + g] = grid_engine ? e2 : nextafterf(e2, INFINITY);
         }
-    Workspace w;
-    rc = carve(d_workspace, workspace_bytes, N, n_masks, 0, &w);
+    rc = carve(d_workspace, workspace_bytes, E.job, &E.w);
     if (rc) return rc;
+    rc = engine_begin(&E);
+    if (rc) return rc;
+    if (grid_engine) {
+        // the workspace has 32 radii per mask
+        CUDA_TRY(cudaMemcpyAsync(E.w.radii, thr.data(), thr.size() * 4, cudaMemcpyHostToDevice, E.st));
+        const RangeOut o = {out_count, out_sumdist, out_mean};
+        return grid_range_enqueue(&E, 0, n_masks, nullptr, G, o);
+    }
     const size_t grid_bytes = align_up(static_cast<size_t>(n_masks) * G * 4, 256);
-    if (w.ring_bytes < grid_bytes)
+    if (E.w.extra_bytes < grid_bytes)
         return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace lacks %zu bytes for the radius grid", grid_bytes);
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
     std::vector<snaps::BatchDesc> batches;
-    plan_lattice(h_masks, n_masks, nullptr, &batches);
+    plan_lattice(h_masks, n_masks, nullptr, 0, &batches);
     const int nb = static_cast<int>(batches.size());
-    CUDA_TRY(snaps::stage_table_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xp,
-                                       n_tiles_for(N) * snaps::kTileRows, st));
-    CUDA_TRY(snaps::stage_blocked_launch(d_X, ld, static_cast<int>(N), n_feat, w.Xb, n_blocks_for(N), st));
-    CUDA_TRY(cudaMemcpyAsync(w.batches, batches.data(), sizeof(snaps::BatchDesc) * nb, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaMemcpyAsync(w.ring, thr.data(), thr.size() * 4, cudaMemcpyHostToDevice, st));
-    CUDA_TRY(cudaStreamSynchronize(st));   // thr is a host temporary: the copy must land before it goes away
-    CUDA_TRY(cudaMemsetAsync(w.counter, 0, 256, st));
+    // pageable host sources: the copies are staged before cudaMemcpyAsync returns
+    CUDA_TRY(cudaMemcpyAsync(E.w.batches, batches.data(), sizeof(snaps::BatchDesc) * nb, cudaMemcpyHostToDevice, E.st));
+    CUDA_TRY(cudaMemcpyAsync(E.w.extra, thr.data(), thr.size() * 4, cudaMemcpyHostToDevice, E.st));
+    CUDA_TRY(cudaMemsetAsync(E.w.counter, 0, 256, E.st));
     snaps::RangeGridParams p;
-    p.Xp = w.Xp;
-    p.Xb = w.Xb;
+    p.Xp = E.w.Xp;
+    p.Xb = E.w.Xb;
     p.n_blocks = n_blocks_for(N);
     p.N = static_cast<int>(N);
+    p.q_begin = static_cast<int>(q_begin);
+    p.nq = static_cast<int>(q_end - q_begin);
     p.G = G;
-    p.batches = w.batches;
+    p.batches = E.w.batches;
     p.n_batches = nb;
-    p.thr_grid = reinterpret_cast<const float*>(w.ring);
+    p.thr_grid = reinterpret_cast<const float*>(E.w.extra);
     p.warps = snaps::kRangeGridMaxThreads / 32;
     while (p.warps > 1 && snaps::range_grid_smem_bytes(G, p.warps) > 227 * 1024) --p.warps;
-    p.work_counter = reinterpret_cast<unsigned long long*>(w.counter);
+    p.work_counter = E.w.counter;
     p.out_count = out_count;
     p.out_sum = out_sumdist;
     p.out_mean = out_mean;
-    const int64_t items = N * nb;
+    const int64_t items = static_cast<int64_t>(p.nq) * nb;
     const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
-    const bool prof = prof_begin(st);
-    CUDA_TRY(snaps::range_grid_launch(p, grid, st));
-    prof_end(prof, st);
+    const bool prof = prof_begin(E.st);
+    CUDA_TRY(snaps::range_grid_launch(p, grid, E.st));
+    prof_end(prof, E.st);
     return SNAPS_OK;
 }
 
@@ -674,7 +966,8 @@ snaps_status snaps_sample_distance_histogram(const float* d_X, int64_t N, int n_
                                              int nq, const int32_t* h_sample_c, int nc, const float* h_rmax,
                                              int n_bins, unsigned long long* out_hist, void* d_workspace,
                                              size_t workspace_bytes, void* stream) {
-    snaps_status rc = check_common(d_X, N, n_feat, ld, h_masks, n_masks);
+    const Job job = Job{d_X, N, n_feat, ld, h_masks, n_masks, 0, N, 0, SNAPS_ENGINE_LATTICE};
+    snaps_status rc = check_job(job, 0);
     if (rc) return rc;
     if (!h_sample_q || !h_sample_c || !h_rmax || !out_hist || nq < 1 || nc < 1)
         return fail(SNAPS_INVALID_ARG, "NULL or empty samples");
@@ -711,11 +1004,12 @@ snaps_status snaps_eps_from_histogram(const unsigned long long* h_hist, int n_ma
     return SNAPS_OK;
 }
 
-size_t snaps_select_k_workspace_bytes(int64_t N, int n_masks) {
-    if (N < 2 || n_masks < 1) return 0;
+size_t snaps_select_k_workspace_bytes(int64_t N, int n_masks, int G) {
+    if (N < 2 || n_masks < 1 || G < 2 || G > 256) return 0;
     const size_t arr = align_up(static_cast<size_t>(N) * n_masks * 4, 256);
-    // score array, three order arrays (smallest k, largest k, current k), ranking scratch
-    return 4 * arr + align_up(snaps::rank_workspace_bytes(N, n_masks), 256);
+    // score array, three order arrays (smallest k, largest k, current k), the U curves, ranking scratch
+    return 4 * arr + align_up(sizeof(float) * 4 * G * static_cast<size_t>(n_masks), 256) +
+           align_up(snaps::rank_workspace_bytes(N, n_masks), 256);
 }
 
 snaps_status snaps_knn_select_k(int64_t N, int n_masks, int k_max, const int32_t* knn_idx, const float* knn_dist,
@@ -731,9 +1025,9 @@ snaps_status snaps_knn_select_k(int64_t N, int n_masks, int k_max, const int32_t
     if (n_top < 1 || n_top > N) return fail(SNAPS_INVALID_ARG, "n_top = %d outside 1..N", n_top);
     if (!out_j_indeg || !out_j_mean) return fail(SNAPS_INVALID_ARG, "NULL outputs");
     if ((N + 31) / 32 * 4 > 200 * 1024) return fail(SNAPS_UNSUPPORTED, "N too large for the top-n bitmap");
-    if (!d_workspace || workspace_bytes < snaps_select_k_workspace_bytes(N, n_masks))
+    if (!d_workspace || workspace_bytes < snaps_select_k_workspace_bytes(N, n_masks, G))
         return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace %zu < %zu bytes", workspace_bytes,
-                    snaps_select_k_workspace_bytes(N, n_masks));
+                    snaps_select_k_workspace_bytes(N, n_masks, G));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const size_t arr = align_up(static_cast<size_t>(N) * n_masks * 4, 256);
     unsigned char* p = static_cast<unsigned char*>(d_workspace);
@@ -741,14 +1035,10 @@ snaps_status snaps_knn_select_k(int64_t N, int n_masks, int k_max, const int32_t
     int32_t* ord_min = reinterpret_cast<int32_t*>(p + arr);
     int32_t* ord_max = reinterpret_cast<int32_t*>(p + 2 * arr);
     int32_t* ord_cur = reinterpret_cast<int32_t*>(p + 3 * arr);
-    void* rws = p + 4 * arr;
-    const size_t rws_bytes = workspace_bytes - 4 * arr;
-    float* u_tmp = nullptr;   // U arrays live in out_u if given, else in a temporary device buffer
-    float* u = out_u;
-    if (!u) {
-        CUDA_TRY(cudaMallocAsync(&u_tmp, sizeof(float) * 4 * G * static_cast<size_t>(n_masks), st));
-        u = u_tmp;
-    }
+    const size_t u_bytes = align_up(sizeof(float) * 4 * G * static_cast<size_t>(n_masks), 256);
+    void* rws = p + 4 * arr + u_bytes;
+    const size_t rws_bytes = workspace_bytes - 4 * arr - u_bytes;
+    float* u = out_u ? out_u : reinterpret_cast<float*>(p + 4 * arr);   // U curves: the caller's array or the workspace
     snaps_status rc = SNAPS_OK;
     for (int metric = 0; metric < 2 && rc == SNAPS_OK; ++metric) {
         const int kind = metric == 0 ? SNAPS_METRIC_KNN_INDEGREE : SNAPS_METRIC_KNN_MEAN;
@@ -782,7 +1072,6 @@ snaps_status snaps_knn_select_k(int64_t N, int n_masks, int k_max, const int32_t
             e = snaps::select_launch(u_min, u_max, G, n_masks, n_top, metric == 0 ? out_j_indeg : out_j_mean, st);
         if (e != cudaSuccess) rc = fail(SNAPS_CUDA_ERROR, "select_k: %s", cudaGetErrorString(e));
     }
-    if (u_tmp) cudaFreeAsync(u_tmp, st);
     return rc;
 }
 
@@ -837,29 +1126,29 @@ snaps_status snaps_knn_scores_at_k(int64_t N, int n_masks, int k_max, int k_j, c
 }
 
 snaps_status snaps_profile_enable(int on) {
-    g_prof_on = on != 0;
+    g_prof.on = on != 0;
     prof_reset();
     return SNAPS_OK;
 }
 
 snaps_status snaps_profile_last_kernel_ms(float* h_ms, int* h_launches) {
     float total = 0.f;
-    for (size_t i = 0; i < g_prof_used; ++i) {
-        CUDA_TRY(cudaEventSynchronize(g_prof_pool[i].second));
+    for (size_t i = 0; i < g_prof.used; ++i) {
+        CUDA_TRY(cudaEventSynchronize(g_prof.pool[i].second));
         float ms = 0.f;
-        CUDA_TRY(cudaEventElapsedTime(&ms, g_prof_pool[i].first, g_prof_pool[i].second));
+        CUDA_TRY(cudaEventElapsedTime(&ms, g_prof.pool[i].first, g_prof.pool[i].second));
         total += ms;
     }
     if (h_ms) *h_ms = total;
-    if (h_launches) *h_launches = static_cast<int>(g_prof_used);
+    if (h_launches) *h_launches = static_cast<int>(g_prof.used);
     return SNAPS_OK;
 }
 
-snaps_status snaps_probe_fp32_rate(int kind, double* h_lane_ops_per_s, void* stream) {
-    if (kind < 0 || kind > 2 || !h_lane_ops_per_s) return fail(SNAPS_INVALID_ARG, "bad probe arguments");
+snaps_status snaps_probe_fp32_rate(int kind, double* h_lane_ops_per_s, void* d_scratch, void* stream) {
+    if (kind < 0 || kind > 5 || !h_lane_ops_per_s || !d_scratch) return fail(SNAPS_INVALID_ARG, "bad probe arguments");
     double ops = 0.0;
     float ms = 0.f;
-    CUDA_TRY(snaps::probe_fp32_launch(kind, &ops, &ms, static_cast<cudaStream_t>(stream)));
+    CUDA_TRY(snaps::probe_fp32_launch(kind, &ops, &ms, static_cast<float*>(d_scratch), static_cast<cudaStream_t>(stream)));
     *h_lane_ops_per_s = ops / (static_cast<double>(ms) * 1e-3);
     return SNAPS_OK;
 }

@@ -1,55 +1,44 @@
 // knn_lattice.cu -- kNN self-join over a batch of feature subspaces (steps a3-a5, a7).
 //
 // What it computes: PAPER.md:112, 122 (kNNSJ) for every mask of a sub-lattice batch;
-// scores of PAPER.md:251-252 fused into the tail.  How (DESIGN.md "kNN kernel"):
+// scores of PAPER.md:251-252 fused into the tail.  How (DESIGN.md 5.1):
 //   * one warp = one query object x the 64 masks {H u T : T subset of features 0..5};
 //     the 32 lanes hold 32 different candidates per step;
-//   * candidates stream from the blocked copy of the table (2.5 MB at N=31,693: L2 resident,
-//     four coalesced 128-bit loads per step, next block prefetched into registers); the warps
-//     of a CTA scan in a loose convoy and share the lines through L1 -- no barrier couples them;
-//   * FILTER (every candidate): 15 squared differences once, then the 16 partial sums
-//     X[u] over features 2..5 (add-only).  X[u] is a lower bound of the four sums
+//   * candidates stream from the blocked copy of the table (2 MB at N=31,693: L2 resident,
+//     four coalesced 128-bit loads per step, next block prefetched into registers); no barrier
+//     couples the warps of a CTA;
+//   * FILTER (every candidate, snaps_device.cuh: lattice_filter): squared differences once, then the
+//     16 partial sums X[u] over features 2..5 (add-only).  X[u] is a lower bound of the four sums
 //     X[u] (+sq0) (+sq1) of "group" u (adding non-negative terms never rounds below the
 //     addend), so a candidate can enter one of the group's lists only if X[u] < G[u],
 //     G[u] = max of the group's four current thresholds (register-held);
 //   * COMPACT: lanes that pass any group test push (id, base, sq0..5) into a per-warp
 //     shared-memory queue (ballot + popc); with running thresholds a few % of candidates pass;
-//   * REFINE (every 32 queued candidates, all lanes busy): the 64 subset sums by add-only
-//     enumeration in a fixed order, each compared with its list's current threshold
-//     (k-th squared distance so far), branch-free into a 64-bit pass mask per lane; passing
-//     (list, id, d^2) triples go to a per-warp ring at positions from a warp prefix sum;
-//   * DRAIN: ring entries are merged into the sorted lists entry-parallel (one lane per
-//     entry, lanes that target the same list take turns); a list is 12/20/28/36 words apart
-//     from the next so that whole lists move with conflict-free 128-bit accesses and the
-//     insert is a rank computation in registers; thresholds and G are refreshed;
+//   * REFINE (every 32 queued candidates, all lanes busy): lane = candidate forms the 64 subset
+//     sums by add-only enumeration in a fixed order; they cross to the list owners through a
+//     32 x 32 shared-memory transpose; lane = list merges the sums below its threshold into its
+//     sorted list, held in registers for the merge (right-aligned, branch-free insert); a list is
+//     12/20/28/36 words apart from the next so that whole lists move with conflict-free 128-bit
+//     accesses; thresholds and G are refreshed;
 //   * thresholds start from an upper bound seeded by evaluating k known objects
-//     (the first k ids and the previous batch's neighbours: consecutive batches
+//     (the first k ids or the previous batch's neighbours: consecutive batches
 //     differ in one feature), tightened by min over supersets (the k-th distance
 //     is monotone in the feature set).
 #include "knn_lattice.cuh"
 
 namespace snaps {
 
-#ifdef SNAPS_STATS
-// Developer diagnostics (never built into the shipped library): phase clocks and event counts.
-__device__ unsigned long long g_stats[16];
-#define STAT_ADD(i, v) do { if (lane == 0) atomicAdd(&g_stats[i], (unsigned long long)(v)); } while (0)
-#define STAT_CLK() clock64()
-#else
-#define STAT_ADD(i, v) do { } while (0)
-#define STAT_CLK() 0ll
-#endif
 
 // ---- per-warp shared-memory state (32-bit words); S = list stride (template parameter) ----
-//   [0, 64*S)        list d^2, list L at L*S, ascending by (d^2, id)
+//   [0, 64*S)        list d^2, list L at L*S, ascending by (d^2, id), right aligned
 //   [64*S, 128*S)    list ids
-//   then rows of 64 words: list count, threshold, seed bound, output slot,
+//   then rows of 64 words: (unused), threshold, seed bound, output slot,
 //   one row: words 0..15 G (group maxima), words 16..30 the query's 15 features
-//   then the ring (3 arrays of kRing words) and the queue (kQueue entries of 8 words)
+//   then the 32 x 32 transpose (row stride 36), the candidate ids of a refine step and the
+//   queue (kQueue entries of 8 words)
 #define L_D2(e, L) ws[(L) * S + (e)]
 #define L_ID(e, L) wsi[64 * S + (L) * S + (e)]
 #define ROWS(r) (128 * S + (r) * 64)
-#define L_CNT(L) wsi[ROWS(0) + (L)]
 #define THR(L) ws[ROWS(1) + (L)]
 #define SEED(L) ws[ROWS(2) + (L)]
 #define SLOT(L) wsi[ROWS(3) + (L)]
@@ -57,7 +46,7 @@ __device__ unsigned long long g_stats[16];
 #define QROW(j) ws[ROWS(4) + 16 + (j)]
 #define MT(T, j) ws[ROWS(5) + (T) * 36 + (j)]
 #define CANDID(j) wsi[ROWS(5) + 32 * 36 + (j)]
-#define QUEUE4(e) (reinterpret_cast<float4*>(ws + ROWS(5) + 32 * 36 + 32) + 2 * (e))
+#define QUEUE4 (reinterpret_cast<float4*>(ws + ROWS(5) + 32 * 36 + 32))
 constexpr int kQueue = 64;   // queue entries (8 words each); refine as soon as 32 are waiting
 
 __host__ __device__ constexpr int knn_list_stride(int k) { return k <= 12 ? 12 : k <= 20 ? 20 : k <= 28 ? 28 : 36; }
@@ -74,50 +63,19 @@ __host__ __device__ constexpr int knn_warp_words(int k) {
 // ties are broken by the smaller id (reading A3).
 // The add order (high features by FMA in feature order -> features 2,3,4,5 -> 0 -> 1) is the
 // same wherever a squared distance is formed, so a value never depends on scheduling.
-// ORD = candidates arrive in increasing id order (the plain scan).  The pivot sweep visits them
-// in sorted-feature order instead: then ties at the threshold must be let through (<=) and the
-// (d^2, id) key is compared explicitly.
-template <int S, bool ORD>
+template <int S>
 __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N, int head, int n) {
     constexpr int NE = S > 32 ? 32 : S;   // list elements held (S = 36 carries 4 words of padding)
     int* wsi = reinterpret_cast<int*>(ws);
     __syncwarp();
-    const long long t0_ = STAT_CLK();
-    STAT_ADD(7, 1);
-    STAT_ADD(8, n);
-    float base = __int_as_float(0x7f800000);
-    float sq[kLow] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    int cand = -1;
-    if (lane < n) {
-        const float4* e = QUEUE4((head + lane) % kQueue);
-        const float4 a = e[0], b = e[1];
-        cand = __float_as_int(a.x);
-        base = a.y; sq[0] = a.z; sq[1] = a.w;
-        sq[2] = b.x; sq[3] = b.y; sq[4] = b.z; sq[5] = b.w;
-        // self by index (reading A4) and padding rows (A19) never reach a list
-        if (cand == q || cand >= N) base = __int_as_float(0x7f800000);
-    }
+    PairTerms pt;
+    const int cand = queue_pop(QUEUE4, kQueue, head, lane, n, q, N, pt);
     CANDID(lane) = cand;
     float X8[8];   // partial sums over features 2,3,4; feature 5 is added per half (same order as X[16])
-    X8[0] = base;
-#pragma unroll
-    for (int u = 1; u < 8; ++u) {
-        const int hb = 31 - __clz(u);
-        X8[u] = __fadd_rn(X8[u & ~(1 << hb)], sq[2 + hb]);
-    }
+    lattice_partial8(pt, X8);
 #pragma unroll
     for (int half = 0; half < 2; ++half) {
-#pragma unroll
-        for (int uu = 0; uu < 8; ++uu) {
-            const float s0 = half ? __fadd_rn(X8[uu], sq[5]) : X8[uu];
-            const float s1 = __fadd_rn(s0, sq[0]);
-            const float s2 = __fadd_rn(s0, sq[1]);
-            const float s3 = __fadd_rn(s1, sq[1]);
-            MT(4 * uu + 0, lane) = s0;
-            MT(4 * uu + 1, lane) = s1;
-            MT(4 * uu + 2, lane) = s2;
-            MT(4 * uu + 3, lane) = s3;
-        }
+        lattice_sums_to_transpose(pt, X8, half, &MT(0, 0), lane);
         __syncwarp();
         // ---- lane = list T.  The k entries are right aligned in the NE slots (ascending; unused
         // bottom slots hold -inf, not yet filled top slots +inf), so the k-th is always slot NE-1.
@@ -143,10 +101,10 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N
 #pragma unroll
         for (int j4 = 0; j4 < 8; ++j4) {
             const float4 m = *reinterpret_cast<const float4*>(&MT(lane, 4 * j4));
-            mask |= ((ORD ? m.x < thr : m.x <= thr) ? 1u : 0u) << (4 * j4);
-            mask |= ((ORD ? m.y < thr : m.y <= thr) ? 1u : 0u) << (4 * j4 + 1);
-            mask |= ((ORD ? m.z < thr : m.z <= thr) ? 1u : 0u) << (4 * j4 + 2);
-            mask |= ((ORD ? m.w < thr : m.w <= thr) ? 1u : 0u) << (4 * j4 + 3);
+            mask |= (m.x < thr ? 1u : 0u) << (4 * j4);
+            mask |= (m.y < thr ? 1u : 0u) << (4 * j4 + 1);
+            mask |= (m.z < thr ? 1u : 0u) << (4 * j4 + 2);
+            mask |= (m.w < thr ? 1u : 0u) << (4 * j4 + 3);
         }
         // ... merged in candidate order (= increasing id).  Every id already in the list is
         // smaller than the new one, so "list entry e precedes (d, id)" is v[e] <= d, and the
@@ -157,13 +115,11 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N
             mask &= mask - 1u;
             const float d = MT(lane, j);
             const int id = CANDID(j);
-            if (ORD ? (d < thr)
-                    : (d <= thr && ((d < v[NE - 1]) | ((d == v[NE - 1]) & (id < w[NE - 1]))))) {
+            if (d < thr) {
                 changed = true;
                 bool below[NE];
 #pragma unroll
-                for (int e = 0; e < NE; ++e)
-                    below[e] = ORD ? (v[e] <= d) : ((v[e] < d) | ((v[e] == d) & (w[e] < id)));
+                for (int e = 0; e < NE; ++e) below[e] = v[e] <= d;
 #pragma unroll
                 for (int e = NE - 1; e >= 1; --e) {
                     v[e] = below[e] ? v[e] : (below[e - 1] ? d : v[e - 1]);
@@ -191,7 +147,6 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N
         GMAX(lane) = fmaxf(fmaxf(t.x, t.y), fmaxf(t.z, t.w));
     }
     __syncwarp();
-    STAT_ADD(0, STAT_CLK() - t0_);
 }
 
 // Upper bounds on the final k-th squared distance of every list of the new batch.
@@ -268,7 +223,7 @@ __device__ __noinline__ void knn_emit(float* ws, const KnnParams& p, int q, int 
         const int L = lane + 32 * h;
         const int sl = SLOT(L);
         if (sl < 0) continue;
-        const size_t o = static_cast<size_t>(sl) * static_cast<size_t>(p.N) + static_cast<size_t>(q);
+        const size_t o = static_cast<size_t>(sl) * static_cast<size_t>(p.nq) + static_cast<size_t>(q - p.q_begin);
         float sum = 0.f, dk = 0.f;
 #pragma unroll 1
         for (int e = 0; e < k; ++e) {
@@ -297,17 +252,11 @@ __device__ __noinline__ void knn_emit(float* ws, const KnnParams& p, int q, int 
             G[4 * i4 + 2] = v.z;                                              \
             G[4 * i4 + 3] = v.w;                                              \
         }                                                                     \
-        if (SWEEP) {                                                          \
-            Gall = G[0];                                                      \
-            _Pragma("unroll") for (int u = 1; u < 16; ++u) Gall = fmaxf(Gall, G[u]); \
-        }                                                                     \
     } while (0)
 
-// SWEEP = false: every candidate block in id order (tables that fit the L2 / small N).
-// SWEEP = true: the pivot sweep (pivot_sort.cu): the batch's table copy sorted by the batch's
-// lowest high feature f is scanned outwards from the query's own position, and a direction stops
-// at the first block whose nearest value of f is farther than every threshold of the batch.
-template <int S, bool SWEEP>
+// Every candidate block in id order (the table is L2 resident at the sizes this engine serves;
+// large tables and arbitrary mask lists take the grid engine, grid_join.cu).
+template <int S>
 __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const KnnParams p) {
     extern __shared__ __align__(128) unsigned char smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -317,7 +266,7 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
 
     // one item = one query x a run of consecutive batches, fetched per warp: no block-level
     // synchronisation anywhere in the kernel (a warp never waits for a slower query)
-    const long long n_items = static_cast<long long>(p.N) * p.n_bchunks;
+    const long long n_items = static_cast<long long>(p.nq) * p.n_bchunks;
     const unsigned lt = (1u << lane) - 1u;
     const int n_blocks = p.n_blocks;
     for (;;) {
@@ -325,17 +274,17 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
         if (lane == 0) item = atomicAdd(p.work_counter, 1ull);
         item = __shfl_sync(kFull, item, 0);
         if (item >= n_items) break;
-        const int q = static_cast<int>(item % p.N);
-        const int bc = static_cast<int>(item / p.N);
+        const int q = p.q_begin + static_cast<int>(item % p.nq);
+        const int bc = static_cast<int>(item / p.nq);
         const int b0 = bc * p.batches_per_item;
         const int b1 = min(b0 + p.batches_per_item, p.n_batches);
 
-        float qlo[kLow];
+        FilterQuery fq;
         float qhi[9];
         {
             const float* qr = p.Xp + static_cast<size_t>(q) * kRowFloats;
 #pragma unroll
-            for (int j = 0; j < kLow; ++j) qlo[j] = qr[j];
+            for (int j = 0; j < kLow; ++j) fq.qlo[j] = qr[j];
 #pragma unroll
             for (int j = 0; j < 9; ++j) qhi[j] = qr[kLow + j];
             if (lane < 15) QROW(lane) = qr[lane];
@@ -345,142 +294,47 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
         for (int b = b0; b < b1; ++b) {
             const BatchDesc* bd = &p.batches[b];
             const uint32_t H = bd->hmask;
-            const long long tb_ = STAT_CLK();
             SLOT(lane) = bd->slot[lane];
             SLOT(lane + 32) = bd->slot[lane + 32];
             knn_seed<S>(ws, p.Xp, q, k, H, has_prev, lane);
-            STAT_ADD(9, STAT_CLK() - tb_);
             // group 0 = lattice slots {}, {0}, {1}, {0,1}: when only {0,1} is asked for (always so for
             // masks of >= 2 features when H is empty), its own sum is the group's bound -- X[0] alone
             // would be 0 there and let every candidate through
-            const bool g0_both = (SLOT(0) < 0) & (SLOT(1) < 0) & (SLOT(2) < 0);
+            filter_query_init(fq, qhi, H, (SLOT(0) < 0) & (SLOT(1) < 0) & (SLOT(2) < 0));
             float G[16];
-            float Gall = 0.f;   // SWEEP: largest threshold of the batch
             RELOAD_G();
-            float wq[9], w[9];  // high features: diff = c*w - q*w, w in {0,1}
-#pragma unroll
-            for (int j = 0; j < 9; ++j) {
-                w[j] = ((H >> (kLow + j)) & 1u) ? 1.f : 0.f;
-                wq[j] = w[j] * qhi[j];
-            }
             int qhead = 0, qtail = 0;  // queue positions (warp-uniform, monotone)
             // candidates: block t = rows 32t..32t+31, lane = row, four coalesced 128-bit loads;
             // two register sets alternate (one in use, one in flight) -- no register moves
-#define LOAD_BLOCK(dst, tab_, t_)                                                             \
+#define FILTER_BLOCK(r, t_)                                                                   \
     {                                                                                         \
-        const float4* b_ = (tab_) + static_cast<size_t>(t_) * 128 + lane;                      \
-        dst.v0 = __ldg(b_); dst.v1 = __ldg(b_ + 32); dst.v2 = __ldg(b_ + 64); dst.v3 = __ldg(b_ + 96); \
-    }
-#define FILTER_BLOCK(r, t_, CAND_)                                                            \
-    {                                                                                         \
-        const float c[15] = {r.v0.x, r.v0.y, r.v0.z, r.v0.w, r.v1.x, r.v1.y, r.v1.z, r.v1.w,   \
-                             r.v2.x, r.v2.y, r.v2.z, r.v2.w, r.v3.x, r.v3.y, r.v3.z};          \
-        /* keep the padding word of the fourth load live until here: otherwise its register is  \
-           handed out as scratch while the prefetch is still in flight and the warp stalls on it */ \
-        asm volatile("" ::"f"(r.v3.w));                                                        \
-        float sq[kLow];                                                                       \
-        _Pragma("unroll") for (int j = 0; j < kLow; ++j) {                                    \
-            const float diff = c[j] - qlo[j];                                                 \
-            sq[j] = __fmul_rn(diff, diff);                                                    \
-        }                                                                                     \
-        float base = 0.f;                                                                     \
-        _Pragma("unroll") for (int j = 0; j < 9; ++j) {                                       \
-            const float diff = __fmaf_rn(c[kLow + j], w[j], -wq[j]);                          \
-            base = __fmaf_rn(diff, diff, base);                                               \
-        }                                                                                     \
-        /* FILTER: group lower bounds against group maxima */                                 \
-        float X[16];                                                                          \
-        X[0] = base;                                                                          \
-        _Pragma("unroll") for (int u = 1; u < 16; ++u) {                                      \
-            const int hb = 31 - __clz(u);                                                     \
-            X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);                                  \
-        }                                                                                     \
-        float x0 = X[0];                                                                      \
-        if (g0_both) x0 = __fadd_rn(__fadd_rn(X[0], sq[0]), sq[1]);                           \
-        bool pa = SWEEP ? (x0 <= G[0]) : (x0 < G[0]), pb = false;                             \
-        _Pragma("unroll") for (int u = 0; u < 16; u += 2) {                                   \
-            if (u > 0) pa |= SWEEP ? (X[u] <= G[u]) : (X[u] < G[u]);                          \
-            pb |= SWEEP ? (X[u + 1] <= G[u + 1]) : (X[u + 1] < G[u + 1]);                     \
-        }                                                                                     \
-        const bool pass = pa | pb;                                                            \
+        PairTerms pt;                                                                         \
+        const bool pass = lattice_filter<false>(r, fq, G, pt);                                \
         const unsigned bal = __ballot_sync(kFull, pass);                                      \
         if (bal) {                                                                            \
-            /* COMPACT */                                                                     \
-            if (pass) {                                                                       \
-                float4* e = QUEUE4((qtail + __popc(bal & lt)) % kQueue);                      \
-                e[0] = make_float4(__int_as_float(CAND_), base, sq[0], sq[1]);                \
-                e[1] = make_float4(sq[2], sq[3], sq[4], sq[5]);                               \
-            }                                                                                 \
-            qtail += __popc(bal);                                                             \
+            qtail += queue_push(QUEUE4, kQueue, qtail, pass, bal, lt, (t_) * 32 + lane, pt);  \
             if (qtail - qhead >= 32) {                                                        \
-                knn_refine<S, !SWEEP>(ws, k, lane, q, p.N, qhead, 32);                        \
+                knn_refine<S>(ws, k, lane, q, p.N, qhead, 32);                                \
                 qhead += 32;                                                                  \
                 RELOAD_G();                                                                   \
             }                                                                                 \
         }                                                                                     \
     }
-            struct Blk { float4 v0, v1, v2, v3; };
-            if (!SWEEP) {
-                Blk ra, rb;
-                LOAD_BLOCK(ra, p.Xb, 0)
-                rb = ra;
+            Blk ra, rb;
+            load_block(ra, p.Xb, 0, lane);
+            rb = ra;
 #pragma unroll 1
-                for (int t = 0; t < n_blocks; t += 2) {
-                    if (t + 1 < n_blocks) LOAD_BLOCK(rb, p.Xb, t + 1)
-                    FILTER_BLOCK(ra, t, (t) * 32 + lane)
-                    if (t + 1 < n_blocks) {
-                        if (t + 2 < n_blocks) LOAD_BLOCK(ra, p.Xb, t + 2)
-                        FILTER_BLOCK(rb, t + 1, (t + 1) * 32 + lane)
-                    }
-                }
-            } else {
-                const int pf = bd->pivot;   // a feature all valid masks of the batch contain, or -1
-                const float4* tab = pf >= 0 ? p.Xs[pf] : p.Xb;
-                const int* idm = pf >= 0 ? p.idmap[pf] : nullptr;
-                const float* pv = pf >= 0 ? p.piv[pf] : nullptr;
-                const int t0 = pf >= 0 ? (p.pos[pf][q] >> 5) : 0;
-                const float qf = pf >= 0 ? QROW(pf) : 0.f;
-#pragma unroll 1
-                for (int dir = 1; dir >= -1; dir -= 2) {
-                    int t = dir > 0 ? t0 : t0 - 1;
-                    const int t_end = dir > 0 ? n_blocks : -1;
-                    if (t != t_end) {
-                        const int eo = dir > 0 ? 31 : 0;   // the block's row farthest along the sweep
-                        Blk nx;
-                        float pe_n = 0.f;
-                        LOAD_BLOCK(nx, tab, t)
-                        if (pv) pe_n = __ldg(pv + 32 * t + eo);
-#pragma unroll 1
-                        for (;;) {
-                            const Blk r = nx;
-                            const float pe = pe_n;
-                            const int tn = t + dir;
-                            if (tn != t_end) {
-                                LOAD_BLOCK(nx, tab, tn)
-                                if (pv) pe_n = __ldg(pv + 32 * tn + eo);
-                            }
-                            FILTER_BLOCK(r, t, (idm ? __ldg(idm + t * 32 + lane) : t * 32 + lane))
-                            if (pv) {
-                                // every row further along has (x_f - q_f)^2 >= de^2, a lower bound of
-                                // all its sums (non-negative terms, monotone rounding)
-                                const float de = dir > 0 ? pe - qf : qf - pe;
-                                if (de > 0.f && __fmul_rn(de, de) > Gall) break;
-                            }
-                            if (tn == t_end) break;
-                            t = tn;
-                        }
-                    }
-                    if (!pv) break;   // unsorted table: one full pass
+            for (int t = 0; t < n_blocks; t += 2) {
+                if (t + 1 < n_blocks) load_block(rb, p.Xb, t + 1, lane);
+                FILTER_BLOCK(ra, t)
+                if (t + 1 < n_blocks) {
+                    if (t + 2 < n_blocks) load_block(ra, p.Xb, t + 2, lane);
+                    FILTER_BLOCK(rb, t + 1)
                 }
             }
-#undef LOAD_BLOCK
 #undef FILTER_BLOCK
-            const long long te_ = STAT_CLK();
-            if (qtail > qhead) knn_refine<S, !SWEEP>(ws, k, lane, q, p.N, qhead, qtail - qhead);
+            if (qtail > qhead) knn_refine<S>(ws, k, lane, q, p.N, qhead, qtail - qhead);
             knn_emit<S>(ws, p, q, lane);
-            STAT_ADD(10, STAT_CLK() - te_);
-            STAT_ADD(3, STAT_CLK() - tb_);
-            STAT_ADD(11, 1);
             has_prev = true;
         }
     }
@@ -490,25 +344,12 @@ size_t knn_lattice_smem_bytes(int k, int warps) {
     return 128 + static_cast<size_t>(warps) * knn_warp_words(k) * 4;
 }
 
-#ifdef SNAPS_STATS
-extern "C" int snaps_debug_stats(unsigned long long* out16, int reset) {
-    if (out16) cudaMemcpyFromSymbol(out16, g_stats, sizeof(g_stats));
-    if (reset) {
-        unsigned long long z[16] = {0};
-        cudaMemcpyToSymbol(g_stats, z, sizeof(z));
-    }
-    return 0;
-}
-#endif
 
 cudaError_t knn_lattice_launch(const KnnParams& p, int grid, cudaStream_t stream) {
     const size_t smem = knn_lattice_smem_bytes(p.k, p.warps);
     const int stride = knn_list_stride(p.k);
-    auto kernel = p.sweep
-        ? (stride == 12 ? knn_lattice_kernel<12, true> : stride == 20 ? knn_lattice_kernel<20, true>
-           : stride == 28 ? knn_lattice_kernel<28, true> : knn_lattice_kernel<36, true>)
-        : (stride == 12 ? knn_lattice_kernel<12, false> : stride == 20 ? knn_lattice_kernel<20, false>
-           : stride == 28 ? knn_lattice_kernel<28, false> : knn_lattice_kernel<36, false>);
+    auto kernel = stride == 12 ? knn_lattice_kernel<12> : stride == 20 ? knn_lattice_kernel<20>
+                  : stride == 28 ? knn_lattice_kernel<28> : knn_lattice_kernel<36>;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kernel<<<grid, p.warps * 32, smem, stream>>>(p);

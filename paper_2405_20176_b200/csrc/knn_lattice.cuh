@@ -5,17 +5,15 @@
 namespace snaps {
 
 constexpr int kKnnMaxThreads = 512;  // 16 warps x 128 registers
+constexpr int kLatticeMaxK = 32;     // list length the sub-lattice kernel holds in shared memory
 
 struct KnnParams {
     const float* Xp;            // staged table, row-major, n_tiles*128 rows of 20 floats (seeds, query rows)
     const float4* Xb;           // staged table, blocked: [n_blocks][4 feature groups][32 rows] float4
     int n_blocks;               // ceil(N / 32)
-    int sweep;                  // 1: pivot sweep over the sorted copies below (pivot_sort.cuh)
-    const float4* Xs[15];        // per pivot feature: blocked table sorted by that feature
-    const float* piv[15];        //   its sorted values
-    const int* idmap[15];        //   sorted position -> object id
-    const int* pos[15];          //   object id -> sorted position
     int N;
+    int q_begin;                // queries are the objects q_begin .. q_begin + nq - 1
+    int nq;
     int k;
     const BatchDesc* batches;   // device
     int n_batches;
@@ -23,11 +21,11 @@ struct KnnParams {
     int n_bchunks;              // ceil(n_batches / batches_per_item)
     int warps;                  // warps per CTA (each works on its own query)
     unsigned long long* work_counter;  // device, zeroed before launch
-    int32_t* out_idx;
+    int32_t* out_idx;           // [n_masks][nq][k]
     float* out_dist;
-    float* out_kth;
+    float* out_kth;             // [n_masks][nq]
     float* out_mean;
-    int32_t* out_indeg;
+    int32_t* out_indeg;         // [n_masks][N]
 };
 
 size_t knn_lattice_smem_bytes(int k, int warps);

@@ -113,7 +113,7 @@ template <int KIND>
 __global__ void __launch_bounds__(512, 1) probe_kernel(float* out, float a, float b) {
     float v[kProbeIlp];
 #pragma unroll
-    for (int i = 0; i < kProbeIlp; ++i) v[i] = a * static_cast<float>(threadIdx.x + i);
+    for (int i = 0; i < kProbeIlp; ++i) v[i] = (KIND >= 3 ? 1e-3f : 1.f) * a * static_cast<float>(threadIdx.x % 7 + i);
     unsigned hits = 0u;
 #pragma unroll 1
     for (int it = 0; it < kProbeIters; ++it) {
@@ -125,6 +125,22 @@ __global__ void __launch_bounds__(512, 1) probe_kernel(float* out, float a, floa
                     v[i] = __fmaf_rn(v[i], a, b);
                 } else if (KIND == 1) {
                     v[i] = __fadd_rn(v[i], b);
+                } else if (KIND == 3) {
+                    // three register operands (the multiplier is another accumulator): the form a real
+                    // distance chain has
+                    v[i] = __fmaf_rn(v[i], v[(i + 5) & (kProbeIlp - 1)], v[(i + 9) & (kProbeIlp - 1)]);
+                } else if (KIND == 4 || KIND == 5) {
+                    // packed pairs (sm_100: fma.rn.f32x2 / add.rn.f32x2, SASS FFMA2 / FADD2): two IEEE
+                    // fp32 results per lane and instruction; counted as 2 lane-ops
+                    if (i % 2 == 0) {
+                        unsigned long long x, y, z;
+                        asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "f"(v[i]), "f"(v[i + 1]));
+                        asm("mov.b64 %0, {%1, %2};" : "=l"(y) : "f"(v[(i + 4) & (kProbeIlp - 1)]), "f"(v[(i + 5) & (kProbeIlp - 1)]));
+                        asm("mov.b64 %0, {%1, %2};" : "=l"(z) : "f"(v[(i + 8) & (kProbeIlp - 1)]), "f"(v[(i + 9) & (kProbeIlp - 1)]));
+                        if (KIND == 4) asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(x) : "l"(y), "l"(z));
+                        else asm("add.rn.f32x2 %0, %0, %1;" : "+l"(x) : "l"(y));
+                        asm("mov.b64 {%0, %1}, %2;" : "=f"(v[i]), "=f"(v[i + 1]) : "l"(x));
+                    }
                 } else {
                     // the join's filter mix: one add and one compare per value, the compares OR-ed
                     // into two predicate chains (FSETP.LT.OR), as in FILTER
@@ -146,10 +162,8 @@ __global__ void __launch_bounds__(512, 1) probe_kernel(float* out, float a, floa
     if (s == 123.456f) out[0] = s;
 }
 
-cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, cudaStream_t stream) {
-    float* d_out = nullptr;
-    cudaError_t e = cudaMalloc(&d_out, 64);
-    if (e != cudaSuccess) return e;
+cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, float* d_out, cudaStream_t stream) {
+    cudaError_t e = cudaSuccess;
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
@@ -158,6 +172,9 @@ cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, cudaStream_
         if (rep == 2) cudaEventRecord(e0, stream);
         if (kind == 0) probe_kernel<0><<<grid, block, 0, stream>>>(d_out, 1.0000001f, 1e-7f);
         else if (kind == 1) probe_kernel<1><<<grid, block, 0, stream>>>(d_out, 1.0000001f, 1e-7f);
+        else if (kind == 3) probe_kernel<3><<<grid, block, 0, stream>>>(d_out, 1.0000001f, 1e-7f);
+        else if (kind == 4) probe_kernel<4><<<grid, block, 0, stream>>>(d_out, 1.0000001f, 1e-7f);
+        else if (kind == 5) probe_kernel<5><<<grid, block, 0, stream>>>(d_out, 1.0000001f, 1e-7f);
         else probe_kernel<2><<<grid, block, 0, stream>>>(d_out, -1.0f, 1e-7f);
     }
     cudaEventRecord(e1, stream);
@@ -168,7 +185,6 @@ cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, cudaStream_
     *lane_ops = per_thread * grid * block;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    cudaFree(d_out);
     return e;
 }
 

@@ -19,6 +19,6 @@ cudaError_t eps_mean_launch(int64_t total, const uint32_t* cnt, const float* sum
                             cudaStream_t stream);
 
 // kind 0: FFMA, 1: FADD, 2: FADD+FSETP pairs.  Returns lane-ops executed and elapsed ms.
-cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, cudaStream_t stream);
+cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, float* d_scratch, cudaStream_t stream);
 
 }  // namespace snaps

@@ -9,13 +9,12 @@
 namespace snaps {
 
 constexpr int kGQueue = 64;
-constexpr float kGInf = __builtin_huge_valf();
 
 // per-warp shared-memory words; G = number of radii (runtime)
 //   SLOT[64] | QROW[16] | MT 32x36 | queue 64x8 | THR[64][G] | HCNT[64][G] | HSUM[64][G]
 #define G_SLOT(L) wsi[(L)]
 #define G_MT(T, j) ws[80 + (T) * 36 + (j)]
-#define G_QUEUE4(e) (reinterpret_cast<float4*>(ws + 80 + 32 * 36) + 2 * (e))
+#define G_QUEUE4 (reinterpret_cast<float4*>(ws + 80 + 32 * 36))
 #define G_BASE (80 + 32 * 36 + kGQueue * 8)
 #define G_THR(L, g) ws[G_BASE + (L) * G + (g)]
 #define G_HCNT(L, g) wsi[G_BASE + 64 * G + (L) * G + (g)]
@@ -27,36 +26,13 @@ __device__ __noinline__ void range_grid_refine(float* ws, int G, bool with_sum, 
                                                int n) {
     int* wsi = reinterpret_cast<int*>(ws);
     __syncwarp();
-    float base = kGInf;
-    float sq[kLow] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    if (lane < n) {
-        const float4* e = G_QUEUE4((head + lane) % kGQueue);
-        const float4 a = e[0], b = e[1];
-        const int cand = __float_as_int(a.x);
-        base = a.y; sq[0] = a.z; sq[1] = a.w;
-        sq[2] = b.x; sq[3] = b.y; sq[4] = b.z; sq[5] = b.w;
-        if (cand == q || cand >= N) base = kGInf;   // self by index (A4), padding rows (A19)
-    }
+    PairTerms pt;
+    queue_pop(G_QUEUE4, kGQueue, head, lane, n, q, N, pt);   // self by index (A4), padding rows (A19)
     float X8[8];
-    X8[0] = base;
-#pragma unroll
-    for (int u = 1; u < 8; ++u) {
-        const int hb = 31 - __clz(u);
-        X8[u] = __fadd_rn(X8[u & ~(1 << hb)], sq[2 + hb]);
-    }
+    lattice_partial8(pt, X8);
 #pragma unroll
     for (int half = 0; half < 2; ++half) {
-#pragma unroll
-        for (int uu = 0; uu < 8; ++uu) {
-            const float s0 = half ? __fadd_rn(X8[uu], sq[5]) : X8[uu];
-            const float s1 = __fadd_rn(s0, sq[0]);
-            const float s2 = __fadd_rn(s0, sq[1]);
-            const float s3 = __fadd_rn(s1, sq[1]);
-            G_MT(4 * uu + 0, lane) = s0;
-            G_MT(4 * uu + 1, lane) = s1;
-            G_MT(4 * uu + 2, lane) = s2;
-            G_MT(4 * uu + 3, lane) = s3;
-        }
+        lattice_sums_to_transpose(pt, X8, half, &G_MT(0, 0), lane);
         __syncwarp();
         const int T = 32 * half + lane;
         const float thr = G_THR(T, G - 1);   // the largest radius of this list (-1 for unused slots)
@@ -90,7 +66,7 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
     float* ws = reinterpret_cast<float*>(smem) + static_cast<size_t>(warp) * range_grid_warp_words(G);
     int* wsi = reinterpret_cast<int*>(ws);
     const bool with_sum = p.out_sum != nullptr || p.out_mean != nullptr;
-    const long long n_items = static_cast<long long>(p.N) * p.n_batches;
+    const long long n_items = static_cast<long long>(p.nq) * p.n_batches;
     const unsigned lt = (1u << lane) - 1u;
     const int n_blocks = p.n_blocks;
     for (;;) {
@@ -98,13 +74,14 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
         if (lane == 0) item = atomicAdd(p.work_counter, 1ull);
         item = __shfl_sync(kFull, item, 0);
         if (item >= n_items) break;
-        const int q = static_cast<int>(item % p.N);
-        const int b = static_cast<int>(item / p.N);
-        float qlo[kLow], qhi[9];
+        const int q = p.q_begin + static_cast<int>(item % p.nq);
+        const int b = static_cast<int>(item / p.nq);
+        FilterQuery fq;
+        float qhi[9];
         {
             const float* qr = p.Xp + static_cast<size_t>(q) * kRowFloats;
 #pragma unroll
-            for (int j = 0; j < kLow; ++j) qlo[j] = qr[j];
+            for (int j = 0; j < kLow; ++j) fq.qlo[j] = qr[j];
 #pragma unroll
             for (int j = 0; j < 9; ++j) qhi[j] = qr[kLow + j];
         }
@@ -122,65 +99,24 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
             }
         }
         __syncwarp();
-        const bool g0_both = (G_SLOT(0) < 0) & (G_SLOT(1) < 0) & (G_SLOT(2) < 0);
+        filter_query_init(fq, qhi, H, (G_SLOT(0) < 0) & (G_SLOT(1) < 0) & (G_SLOT(2) < 0));
         float Gm[16];
 #pragma unroll
         for (int u = 0; u < 16; ++u)
             Gm[u] = fmaxf(fmaxf(G_THR(4 * u, G - 1), G_THR(4 * u + 1, G - 1)),
                           fmaxf(G_THR(4 * u + 2, G - 1), G_THR(4 * u + 3, G - 1)));
-        float wq[9], w[9];
-#pragma unroll
-        for (int j = 0; j < 9; ++j) {
-            w[j] = ((H >> (kLow + j)) & 1u) ? 1.f : 0.f;
-            wq[j] = w[j] * qhi[j];
-        }
         int qhead = 0, qtail = 0;
-        float4 n0, n1, n2, n3;
-        {
-            const float4* b_ = p.Xb + lane;
-            n0 = __ldg(b_); n1 = __ldg(b_ + 32); n2 = __ldg(b_ + 64); n3 = __ldg(b_ + 96);
-        }
+        Blk nx;
+        load_block(nx, p.Xb, 0, lane);
 #pragma unroll 1
         for (int t = 0; t < n_blocks; ++t) {
-            const float4 r0 = n0, r1 = n1, r2 = n2, r3 = n3;
-            if (t + 1 < n_blocks) {
-                const float4* b_ = p.Xb + static_cast<size_t>(t + 1) * 128 + lane;
-                n0 = __ldg(b_); n1 = __ldg(b_ + 32); n2 = __ldg(b_ + 64); n3 = __ldg(b_ + 96);
-            }
-            const float c[15] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w,
-                                 r2.x, r2.y, r2.z, r2.w, r3.x, r3.y, r3.z};
-            float sq[kLow];
-#pragma unroll
-            for (int j = 0; j < kLow; ++j) {
-                const float diff = c[j] - qlo[j];
-                sq[j] = __fmul_rn(diff, diff);
-            }
-            float base = 0.f;
-#pragma unroll
-            for (int j = 0; j < 9; ++j) {
-                const float diff = __fmaf_rn(c[kLow + j], w[j], -wq[j]);
-                base = __fmaf_rn(diff, diff, base);
-            }
-            float X[16];
-            X[0] = base;
-#pragma unroll
-            for (int u = 1; u < 16; ++u) {
-                const int hb = 31 - __clz(u);
-                X[u] = __fadd_rn(X[u & ~(1 << hb)], sq[2 + hb]);
-            }
-            float x0 = X[0];
-            if (g0_both) x0 = __fadd_rn(__fadd_rn(X[0], sq[0]), sq[1]);
-            bool pass = x0 < Gm[0];
-#pragma unroll
-            for (int u = 1; u < 16; ++u) pass |= (X[u] < Gm[u]);
+            const Blk r = nx;
+            if (t + 1 < n_blocks) load_block(nx, p.Xb, t + 1, lane);
+            PairTerms pt;
+            const bool pass = lattice_filter<false>(r, fq, Gm, pt);
             const unsigned bal = __ballot_sync(kFull, pass);
             if (bal) {
-                if (pass) {
-                    float4* e = G_QUEUE4((qtail + __popc(bal & lt)) % kGQueue);
-                    e[0] = make_float4(__int_as_float(t * 32 + lane), base, sq[0], sq[1]);
-                    e[1] = make_float4(sq[2], sq[3], sq[4], sq[5]);
-                }
-                qtail += __popc(bal);
+                qtail += queue_push(G_QUEUE4, kGQueue, qtail, pass, bal, lt, t * 32 + lane, pt);
                 if (qtail - qhead >= 32) {
                     range_grid_refine(ws, G, with_sum, lane, q, p.N, qhead, 32);
                     qhead += 32;
@@ -199,7 +135,7 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
             for (int g = 0; g < G; ++g) {
                 cnt += G_HCNT(L, g);
                 tot += G_HSUM(L, g);
-                const size_t o = (static_cast<size_t>(sl) * G + g) * static_cast<size_t>(p.N) + q;
+                const size_t o = (static_cast<size_t>(sl) * G + g) * static_cast<size_t>(p.nq) + (q - p.q_begin);
                 p.out_count[o] = static_cast<uint32_t>(cnt);
                 if (p.out_sum) p.out_sum[o] = tot;
                 if (p.out_mean) p.out_mean[o] = cnt > 0 ? tot / static_cast<float>(cnt) : 0.f;

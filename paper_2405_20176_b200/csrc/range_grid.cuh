@@ -12,13 +12,15 @@ struct RangeGridParams {
     const float4* Xb;
     int n_blocks;
     int N;
+    int q_begin;                // queries are the objects q_begin .. q_begin + nq - 1
+    int nq;
     int G;                      // radii per mask, ascending
     const BatchDesc* batches;   // slot[] only (thr[] unused)
     int n_batches;
     const float* thr_grid;      // device [n_masks][G]: nextafter(eps^2)
     int warps;
     unsigned long long* work_counter;
-    uint32_t* out_count;        // [n_masks][G][N]
+    uint32_t* out_count;        // [n_masks][G][nq]
     float* out_sum;
     float* out_mean;
 };

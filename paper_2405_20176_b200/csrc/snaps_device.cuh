@@ -1,10 +1,10 @@
-// snaps_device.cuh -- device-side building blocks shared by the join kernels (sm_100a).
+// snaps_device.cuh -- device-side building blocks shared by the sub-lattice join kernels (sm_100a).
 //
 // Layouts of the staged table ("a1" in DESIGN.md).  Row-major copy Xp: row r of the caller's
 // N x n_feat fp32 matrix becomes 20 floats (80 bytes): features 0..14, then 5 zeros; used for
-// query rows, seed evaluations and as the gather source of the sorted copies.  Blocked copy Xb
-// (the candidate stream of both join kernels): 32 rows per block, four feature groups of 32
-// float4 per block, read with four fully coalesced 128-bit loads per warp.
+// query rows, seed evaluations and as the gather source of the grid engine's compact rows.
+// Blocked copy Xb (the candidate stream of the sub-lattice kernels): 32 rows per block, four
+// feature groups of 32 float4 per block, read with four fully coalesced 128-bit loads per warp.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -17,7 +17,6 @@ constexpr int kTileRows = 128;                 // Xp is padded to a multiple of 
 constexpr int kTileBytes = kTileRows * kRowBytes;  // 10240
 constexpr int kLow = 6;                        // lattice features per batch
 constexpr int kLat = 1 << kLow;                // 64 subset sums per (pair, batch)
-constexpr int kRing = 128;                     // kNN: per-warp ring of (list, id, d^2) triples awaiting merge
 constexpr unsigned kFull = 0xffffffffu;
 constexpr float kPadCoord = 1e18f;             // coordinate of padding rows (squares stay finite: 15e36)
 
@@ -30,8 +29,7 @@ struct alignas(16) BatchDesc {
     int32_t slot[kLat];
     uint32_t hmask;            // bits 6..14
     int32_t n_valid;
-    int32_t pivot;             // pivot sweep: a feature every valid mask of the batch contains, or -1
-    int32_t pad_;
+    int32_t pad_[2];
 };
 static_assert(sizeof(BatchDesc) % 16 == 0, "BatchDesc rows are read with 128-bit loads");
 
@@ -46,6 +44,147 @@ __device__ __forceinline__ float masked_d2(const float* __restrict__ a, const fl
         if ((mask >> j) & 1u) acc = __fadd_rn(acc, sq);
     }
     return acc;
+}
+
+// ---- the candidate stream and the group filter shared by knn_lattice.cu, range_lattice.cu and
+// range_grid.cu (DESIGN.md 5.1 steps 1-2).
+
+// One block of the blocked table in registers: lane = row 32t + lane.
+struct Blk {
+    float4 v0, v1, v2, v3;
+};
+
+__device__ __forceinline__ void load_block(Blk& dst, const float4* __restrict__ Xb, int t, int lane) {
+    const float4* b = Xb + static_cast<size_t>(t) * 128 + lane;
+    dst.v0 = __ldg(b);
+    dst.v1 = __ldg(b + 32);
+    dst.v2 = __ldg(b + 64);
+    dst.v3 = __ldg(b + 96);
+}
+
+// The per-query, per-batch constants of the filter.
+struct FilterQuery {
+    float qlo[kLow];   // the query's lattice features
+    float w[9];        // high features: diff = c*w - q*w with w in {0,1} (1 = feature in H)
+    float wq[9];
+    bool g0_both;      // group 0 asked for {0,1} only: its own sum is the group's bound
+};
+
+__device__ __forceinline__ void filter_query_init(FilterQuery& f, const float (&qhi)[9], uint32_t H, bool g0_both) {
+#pragma unroll
+    for (int j = 0; j < 9; ++j) {
+        f.w[j] = ((H >> (kLow + j)) & 1u) ? 1.f : 0.f;
+        f.wq[j] = f.w[j] * qhi[j];
+    }
+    f.g0_both = g0_both;
+}
+
+// What the refine step needs of a candidate that passed: the high-feature part of every sum and the
+// six lattice squared differences.
+struct PairTerms {
+    float base;
+    float sq[kLow];
+};
+
+// FILTER of one candidate (this lane's row of block r): the six lattice squared differences, the
+// high-feature part `base` (FMA chain in feature order), the 16 partial sums X[u] over subsets u
+// of features {2,3,4,5} (add-only), and the test of each X[u] -- a lower bound of the four sums
+// X[u] (+sq0) (+sq1) of group u -- against the group's largest threshold G[u].
+// INCL = let equality through (not used by the in-order scans).
+template <bool INCL>
+__device__ __forceinline__ bool lattice_filter(const Blk& r, const FilterQuery& f, const float (&G)[16],
+                                               PairTerms& out) {
+    const float c[15] = {r.v0.x, r.v0.y, r.v0.z, r.v0.w, r.v1.x, r.v1.y, r.v1.z, r.v1.w,
+                         r.v2.x, r.v2.y, r.v2.z, r.v2.w, r.v3.x, r.v3.y, r.v3.z};
+    // keep the padding word of the fourth load live until here: otherwise its register is handed
+    // out as scratch while the prefetch is still in flight and the warp stalls on it
+    asm volatile("" ::"f"(r.v3.w));
+#pragma unroll
+    for (int j = 0; j < kLow; ++j) {
+        const float diff = c[j] - f.qlo[j];
+        out.sq[j] = __fmul_rn(diff, diff);
+    }
+    float base = 0.f;
+#pragma unroll
+    for (int j = 0; j < 9; ++j) {
+        const float diff = __fmaf_rn(c[kLow + j], f.w[j], -f.wq[j]);
+        base = __fmaf_rn(diff, diff, base);
+    }
+    out.base = base;
+    float X[16];
+    X[0] = base;
+#pragma unroll
+    for (int u = 1; u < 16; ++u) {
+        const int hb = 31 - __clz(u);
+        X[u] = __fadd_rn(X[u & ~(1 << hb)], out.sq[2 + hb]);
+    }
+    float x0 = X[0];
+    if (f.g0_both) x0 = __fadd_rn(__fadd_rn(X[0], out.sq[0]), out.sq[1]);
+    bool pa = INCL ? (x0 <= G[0]) : (x0 < G[0]), pb = false;
+#pragma unroll
+    for (int u = 0; u < 16; u += 2) {
+        if (u > 0) pa |= INCL ? (X[u] <= G[u]) : (X[u] < G[u]);
+        pb |= INCL ? (X[u + 1] <= G[u + 1]) : (X[u + 1] < G[u + 1]);
+    }
+    return pa | pb;
+}
+
+// COMPACT: the lanes that passed append (id, base, sq0..5) to the warp's queue of 8-word entries.
+// Returns the number of entries appended (warp-uniform).
+__device__ __forceinline__ int queue_push(float4* queue, int queue_len, int qtail, bool pass, unsigned bal,
+                                          unsigned lanes_below, int cand, const PairTerms& t) {
+    if (pass) {
+        float4* e = queue + 2 * ((qtail + __popc(bal & lanes_below)) % queue_len);
+        e[0] = make_float4(__int_as_float(cand), t.base, t.sq[0], t.sq[1]);
+        e[1] = make_float4(t.sq[2], t.sq[3], t.sq[4], t.sq[5]);
+    }
+    return __popc(bal);
+}
+
+// The 64 subset sums of a queued candidate in the fixed order (high features -> 2,3,4 -> 5 -> 0 -> 1),
+// written as rows T = 0..31 of a 32 x 32 transpose (row stride 36 words), half = 0: the sums without
+// feature 5, half = 1: with it.  X8 = partial sums over features 2,3,4.
+__device__ __forceinline__ void lattice_partial8(const PairTerms& t, float (&X8)[8]) {
+    X8[0] = t.base;
+#pragma unroll
+    for (int u = 1; u < 8; ++u) {
+        const int hb = 31 - __clz(u);
+        X8[u] = __fadd_rn(X8[u & ~(1 << hb)], t.sq[2 + hb]);
+    }
+}
+
+__device__ __forceinline__ void lattice_sums_to_transpose(const PairTerms& t, const float (&X8)[8], int half,
+                                                          float* mt, int lane) {
+#pragma unroll
+    for (int uu = 0; uu < 8; ++uu) {
+        const float s0 = half ? __fadd_rn(X8[uu], t.sq[5]) : X8[uu];
+        const float s1 = __fadd_rn(s0, t.sq[0]);
+        const float s2 = __fadd_rn(s0, t.sq[1]);
+        const float s3 = __fadd_rn(s1, t.sq[1]);
+        mt[(4 * uu + 0) * 36 + lane] = s0;
+        mt[(4 * uu + 1) * 36 + lane] = s1;
+        mt[(4 * uu + 2) * 36 + lane] = s2;
+        mt[(4 * uu + 3) * 36 + lane] = s3;
+    }
+}
+
+// The entry a lane takes from the queue at refine time; self (reading A4) and padding rows (A19)
+// get an infinite base so that none of their sums can pass.
+__device__ __forceinline__ int queue_pop(const float4* queue, int queue_len, int head, int lane, int n, int q, int N,
+                                         PairTerms& t) {
+    t.base = __int_as_float(0x7f800000);
+#pragma unroll
+    for (int j = 0; j < kLow; ++j) t.sq[j] = 0.f;
+    int cand = -1;
+    if (lane < n) {
+        const float4* e = queue + 2 * ((head + lane) % queue_len);
+        const float4 a = e[0], b = e[1];
+        cand = __float_as_int(a.x);
+        t.base = a.y; t.sq[0] = a.z; t.sq[1] = a.w;
+        t.sq[2] = b.x; t.sq[3] = b.y; t.sq[4] = b.z; t.sq[5] = b.w;
+        if (cand == q || cand >= N) t.base = __int_as_float(0x7f800000);
+    }
+    return cand;
 }
 
 }  // namespace snaps

@@ -40,3 +40,23 @@ def unshard(index_lists, n_masks: int) -> np.ndarray:
     cat = np.concatenate(index_lists)
     assert len(cat) == n_masks and len(np.unique(cat)) == n_masks
     return np.argsort(cat, kind="stable")
+
+
+def shard_queries(n_objects: int, rank: int, world: int):
+    """-> (q_begin, q_end): the contiguous slice of query ids `rank` owns (table
+    replicated, every rank joins its slice against all objects; lists and scores concatenate in rank
+    order, the in-degree rows of the ranks add up)."""
+    assert 0 <= rank < world
+    return n_objects * rank // world, n_objects * (rank + 1) // world
+
+
+def shard_masks_by_cost(masks, rank: int, world: int):
+    """Grid engine (one subspace per launch, cost grows with the number of features): masks sorted by
+    popcount and dealt round-robin, so that every rank gets the same mix.  -> indices, ascending."""
+    m = np.asarray(masks, dtype=np.uint16).astype(np.int64)
+    assert 0 <= rank < world
+    pc = np.zeros(len(m), dtype=np.int64)
+    for b in range(16):
+        pc += (m >> b) & 1
+    order = np.argsort(pc, kind="stable")
+    return np.sort(order[rank::world])

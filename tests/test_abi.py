@@ -37,7 +37,7 @@ def test_workspace_and_plan_sizes():
     ev = s.planned_evals(31693, 15, m)
     assert ev == 512 * 64 * 31693 ** 2             # 512 complete sub-lattices cover Eq. 1's 32,752
     assert s.planned_evals(2000, 4, workloads.all_masks(4)) == 64 * 2000 ** 2
-    assert s.stream_ring_bytes(1000, 10, 4) >= 2 * 4 * 1000 * 23 * 4
+    assert s.stream_ring_bytes(1000, 1000, 10, 4) >= 2 * 4 * 1000 * 23 * 4
 
 
 def test_no_torch_types_in_header():

@@ -1,5 +1,5 @@
 """Seeded randomised parity sweep: ragged N, every list stride (k up to 32), 1..15 features, heavy
-ties and duplicated rows, repeated masks, both scan modes (plain / pivot sweep), kNN and range
+ties and duplicated rows, repeated masks, both engines (sub-lattice / grid), kNN and range
 joins -- each case element by element against the fp64 oracle under tests/parity.py's rules."""
 import numpy as np
 import pytest
@@ -11,7 +11,7 @@ pytestmark = pytest.mark.gpu
 
 
 @pytest.mark.parametrize("seed", [11, 12, 13, 14])
-def test_random_cases_against_oracle(seed, oracle_mod, monkeypatch):
+def test_random_cases_against_oracle(seed, oracle_mod):
     import torch
     import paper_2405_20176_b200 as snaps
     rng = np.random.default_rng(seed)
@@ -33,9 +33,9 @@ def test_random_cases_against_oracle(seed, oracle_mod, monkeypatch):
         allm = workloads.all_masks(nf, 1)
         masks = rng.choice(allm, min(len(allm), int(rng.integers(1, 70))),
                            replace=bool(rng.integers(0, 2)) and len(allm) > 1)
-        monkeypatch.setenv("SNAPS_KNN_SWEEP", str(int(rng.integers(0, 2))))
+        engine = ("lattice", "grid")[int(rng.integers(0, 2))]
         Xd = torch.from_numpy(X).cuda()
-        out = snaps.knn_selfjoin(Xd, masks, k)
+        out = snaps.knn_selfjoin(Xd, masks, k, engine=engine)
         torch.cuda.synchronize()
         g = {a: out[a].cpu().numpy() for a in ("idx", "dist", "kth", "mean", "indeg")}
         kk = min(k + 1, n - 1)
@@ -47,8 +47,7 @@ def test_random_cases_against_oracle(seed, oracle_mod, monkeypatch):
         kth, mean, indeg = oracle_mod.knn_scores(n, oi[:, :, :k], od[:, :, :k])
         check_knn_scores(g, g["idx"], kth, mean, indeg, unamb, n)
         eps = np.maximum(np.median(od[:, :, k - 1], axis=1) * 1.00317, 1e-3).astype(np.float32)
-        r = snaps.range_selfjoin(Xd, masks, eps)
+        r = snaps.range_selfjoin(Xd, masks, eps, engine=engine)
         torch.cuda.synchronize()
         check_range(r["count"].cpu().numpy(), r["sumdist"].cpu().numpy(), r["mean"].cpu().numpy(),
                     oracle_mod, X, masks, eps)
-    monkeypatch.delenv("SNAPS_KNN_SWEEP", raising=False)

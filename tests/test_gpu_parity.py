@@ -22,9 +22,9 @@ def _dev(X):
     return torch.from_numpy(np.ascontiguousarray(X)).cuda()
 
 
-def _knn_case(snaps, oracle_mod, X, masks, k, full_scores=True):
+def _knn_case(snaps, oracle_mod, X, masks, k, engine="auto"):
     import torch
-    out = snaps.knn_selfjoin(_dev(X), masks, k)
+    out = snaps.knn_selfjoin(_dev(X), masks, k, engine=engine)
     torch.cuda.synchronize()
     g = {n: out[n].cpu().numpy() for n in ("idx", "dist", "kth", "mean", "indeg")}
     N = len(X)
@@ -309,50 +309,86 @@ def test_streamed_large_table_reduced_configs_4_5(snaps, oracle_mod):
         assert bool((st["indeg"].sum(dim=1) == n * k).all())
 
 
-# ---------------------------------------------------------------- pivot sweep (large-N path)
-@pytest.fixture
-def force_sweep(monkeypatch):
-    """The library switches to the pivot sweep at N >= 2^18; SNAPS_KNN_SWEEP=1 forces it so that the
-    path can be checked element by element at sizes the oracle finishes in seconds."""
-    monkeypatch.setenv("SNAPS_KNN_SWEEP", "1")
-    yield
-    monkeypatch.delenv("SNAPS_KNN_SWEEP", raising=False)
-
-
-@pytest.mark.parametrize("n,nf,k,seed", [(129, 15, 16, 5), (1537, 15, 10, 8), (3000, 12, 3, 7), (700, 9, 10, 11)])
-def test_pivot_sweep_random_tables(snaps, oracle_mod, force_sweep, n, nf, k, seed):
+# ---------------------------------------------------------------- grid engine (large N, arbitrary masks, k <= 256)
+# The library takes the grid engine at N >= 2^18 or k > 32; engine="grid" forces it so that the path
+# is checked element by element at sizes the oracle finishes in seconds.
+@pytest.mark.parametrize("n,nf,k,seed", [(2, 2, 1, 0), (3, 3, 2, 1), (33, 4, 5, 2), (129, 15, 16, 5), (1537, 15, 10, 8),
+                                         (3000, 12, 3, 7), (700, 9, 10, 11), (5000, 15, 16, 12)])
+def test_grid_engine_random_tables(snaps, oracle_mod, n, nf, k, seed):
     X = workloads.make_table(n, seed, cols=list(range(nf)), outlier_frac=0.02)
     allm = workloads.all_masks(nf, 1)
     rng = np.random.default_rng(seed)
     masks = rng.choice(allm, min(len(allm), 60), replace=False)
-    _knn_case(snaps, oracle_mod, X, masks, k)
+    _knn_case(snaps, oracle_mod, X, masks, k, engine="grid")
 
 
-def test_pivot_sweep_ties(snaps, oracle_mod, force_sweep):
-    # candidates no longer arrive in id order: ties at the threshold must still go to the smaller id
+def test_grid_engine_ties(snaps, oracle_mod):
+    # candidates do not arrive in id order: ties at the threshold must still go to the smaller id
     X = workloads.hypercube_table(9)
-    _knn_case(snaps, oracle_mod, X, workloads.all_masks(9, 1)[::7], 10)
+    _knn_case(snaps, oracle_mod, X, workloads.all_masks(9, 1)[::7], 10, engine="grid")
     X = workloads.duplicate_block_table(900, 3, frac=0.3)
     masks = np.array([(1 << 13) | (1 << 14), (1 << 13) | 1, 0x7FFF, 1 << 14, (1 << 6) | 3], dtype=np.uint16)
-    g, _ = _knn_case(snaps, oracle_mod, X, masks, 10)
+    g, _ = _knn_case(snaps, oracle_mod, X, masks, 10, engine="grid")
     oi, od = oracle_mod.knn_selfjoin(X, masks, 10)
     zero = od[0, :, -1] == 0
     assert zero.sum() > 100 and (g["idx"][0][zero] == oi[0][zero]).all()
 
 
-def test_pivot_sweep_equals_plain_scan(snaps, oracle_mod, monkeypatch):
+def test_grid_engine_negative_and_signed_zero_columns(snaps, oracle_mod):
+    # the quantile bins order values with an order-preserving key: negative coordinates and -0.0 are legal
+    X = workloads.make_table(2500, 17, cols=list(range(8)), outlier_frac=0.02) - np.float32(0.5)
+    X[::7, 2] = np.float32(-0.0)
+    X[1::7, 2] = np.float32(0.0)
+    masks = np.array([0b101, 0b1100, 0b11111111, 0b100, 0b1000110], dtype=np.uint16)
+    _knn_case(snaps, oracle_mod, X, masks, 10, engine="grid")
+    _knn_case(snaps, oracle_mod, X, masks, 10, engine="lattice")
+
+
+@pytest.mark.parametrize("k", [33, 64, 256])
+def test_grid_engine_large_k(snaps, oracle_mod, k):
+    # NEXT-3: k beyond the sub-lattice engine's 32 (k_max = 256 on LSST5M); auto picks the grid engine
+    X = workloads.make_table(1800, 19, cols=list(range(10)), outlier_frac=0.01)
+    masks = np.array([0b11, 0b1010101, 0b1111111111, 0b1000000100, 0b110110], dtype=np.uint16)
+    _knn_case(snaps, oracle_mod, X, masks, k)
+
+
+def test_engines_agree(snaps, oracle_mod):
+    # same joins from both engines: ids equal wherever the oracle says the query is unambiguous
     import torch
     X = workloads.make_table(4000, 13, outlier_frac=0.01)
     masks = workloads.pair_masks_plus_full(15)
     Xd = _dev(X)
-    monkeypatch.setenv("SNAPS_KNN_SWEEP", "0")
-    a = snaps.knn_selfjoin(Xd, masks, 10)
-    monkeypatch.setenv("SNAPS_KNN_SWEEP", "1")
-    b = snaps.knn_selfjoin(Xd, masks, 10)
+    a = snaps.knn_selfjoin(Xd, masks, 10, engine="lattice")
+    b = snaps.knn_selfjoin(Xd, masks, 10, engine="grid")
     torch.cuda.synchronize()
-    monkeypatch.delenv("SNAPS_KNN_SWEEP", raising=False)
-    for n in ("idx", "dist", "kth", "mean", "indeg"):
-        assert torch.equal(a[n], b[n]), n
+    same = (a["idx"] == b["idx"]).all(dim=2)
+    assert same.float().mean().item() > 0.999
+    assert torch.allclose(a["dist"], b["dist"], rtol=2e-6, atol=0)
+    assert bool((a["indeg"].sum(dim=1) == b["indeg"].sum(dim=1)).all())
+
+
+def test_query_range_slices_concatenate(snaps, oracle_mod):
+    # a rank owns a query slice; slices concatenate, in-degree rows add
+    import torch
+    X = workloads.make_table(2600, 29, cols=list(range(12)), outlier_frac=0.01)
+    masks = workloads.all_masks(12)[::41]
+    Xd = _dev(X)
+    for engine in ("lattice", "grid"):
+        full = snaps.knn_selfjoin(Xd, masks, 9, engine=engine)
+        cuts = [0, 700, 701, 1999, 2600]
+        parts = [snaps.knn_selfjoin(Xd, masks, 9, engine=engine, q_range=(cuts[i], cuts[i + 1])) for i in range(4)]
+        torch.cuda.synchronize()
+        for n in ("idx", "dist", "kth", "mean"):
+            assert torch.equal(torch.cat([p[n] for p in parts], dim=1), full[n]), (engine, n)
+        assert torch.equal(sum(p["indeg"] for p in parts), full["indeg"]), engine
+        eps = np.full(len(masks), 0.2, np.float32)
+        rf = snaps.range_selfjoin(Xd, masks, eps, engine=engine)
+        rp = [snaps.range_selfjoin(Xd, masks, eps, engine=engine, q_range=(cuts[i], cuts[i + 1])) for i in range(4)]
+        torch.cuda.synchronize()
+        assert torch.equal(torch.cat([p["count"] for p in rp], dim=1), rf["count"]), engine
+        # the grid engine adds a query's distances in scan order, which depends on the 32 queries it is grouped with
+        cat = torch.cat([p["sumdist"] for p in rp], dim=1)
+        assert torch.equal(cat, rf["sumdist"]) if engine == "lattice" else torch.allclose(cat, rf["sumdist"], rtol=2e-5, atol=0)
 
 
 def test_config4_full_size_sampled(snaps, oracle_mod):
@@ -375,8 +411,8 @@ def test_config4_full_size_sampled(snaps, oracle_mod):
     assert bool((st["indeg"].sum(dim=1) == n * k).all())
 
 
-@pytest.mark.parametrize("n,nf,seed", [(130, 5, 1), (1537, 15, 3), (3000, 15, 5)])
-def test_pivot_sweep_range_join(snaps, oracle_mod, force_sweep, n, nf, seed):
+@pytest.mark.parametrize("n,nf,seed", [(2, 2, 0), (130, 5, 1), (1537, 15, 3), (3000, 15, 5)])
+def test_grid_engine_range_join(snaps, oracle_mod, n, nf, seed):
     import torch
     X = workloads.make_table(n, seed, cols=list(range(nf)), outlier_frac=0.02)
     allm = workloads.all_masks(nf, 1)
@@ -384,7 +420,7 @@ def test_pivot_sweep_range_join(snaps, oracle_mod, force_sweep, n, nf, seed):
     masks = rng.choice(allm, min(len(allm), 48), replace=False)
     _, od = oracle_mod.knn_selfjoin(X, masks, min(10, n - 1))
     eps = np.array([max(1.003 * np.median(od[m, :, -1]), 1e-3) for m in range(len(masks))], dtype=np.float32)
-    out = snaps.range_selfjoin(_dev(X), masks, eps)
+    out = snaps.range_selfjoin(_dev(X), masks, eps, engine="grid")
     torch.cuda.synchronize()
     lo, hi = check_range(out["count"].cpu().numpy(), out["sumdist"].cpu().numpy(), out["mean"].cpu().numpy(),
                          oracle_mod, X, masks, eps)
