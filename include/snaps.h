@@ -382,6 +382,28 @@ snaps_status snaps_sample_distance_histogram(const float *d_X, int64_t N, int n_
                                              void *d_workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * The whole search of PAPER.md:229-237 in one call, on the device: (1) eps_mean[mask] = the mean
+ * distance over the sampled (query, candidate) pairs, c != q by index -- "the upper bound on a
+ * practical search radius"; (2) the histogram of those distances in n_bins equal bins
+ * over [0, eps_mean); (3) for every target selectivity s_t (mean neighbours per point, PAPER.md:221;
+ * the paper's eps_min / eps_max are s = 0.001 |D| and 0.15 |D|) the upper edge of the first bin whose
+ * cumulative mean cum * (N-1) / pairs reaches s_t, or eps_mean if none does.
+ *   h_sample_q [nq], h_sample_c [nc]  host, distinct object ids each
+ *   h_target_s [n_targets]            host, > 0
+ *   out_eps_mean  device [n_masks] fp32;  out_eps  device [n_masks][n_targets] fp32
+ *   out_hist      device [n_masks][n_bins] uint64 or NULL (the histogram, for inspection)
+ * Workspace: snaps_eps_search_workspace_bytes(nq, nc, n_masks, n_bins, n_targets).
+ */
+size_t snaps_eps_search_workspace_bytes(int nq, int nc, int n_masks, int n_bins, int n_targets);
+
+snaps_status snaps_eps_search(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                              const uint16_t *h_masks, int n_masks,
+                              const int32_t *h_sample_q, int nq, const int32_t *h_sample_c, int nc,
+                              int n_bins, const double *h_target_s, int n_targets,
+                              float *out_eps_mean, float *out_eps, unsigned long long *out_hist,
+                              void *d_workspace, size_t workspace_bytes, void *stream);
+
+/*
  * Host arithmetic on a histogram copied back from the device: the cumulative histogram gives the
  * mean number of neighbours per point at each bin edge, mean(r_b) = cum[b] * (N-1) / (nq * nc')
  * with nc' = candidates per query (nc, minus one where the query is in the candidate sample --

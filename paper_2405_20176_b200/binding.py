@@ -18,6 +18,7 @@ EXPORTED_SYMBOLS = [
     "snaps_knn_scores_at_k", "snaps_range_grid_workspace_bytes", "snaps_range_selfjoin_grid",
     "snaps_select_k_workspace_bytes", "snaps_knn_select_k",
     "snaps_dist_hist_workspace_bytes", "snaps_sample_distance_histogram", "snaps_eps_from_histogram",
+    "snaps_eps_search_workspace_bytes", "snaps_eps_search",
 ]
 
 ENGINES = {"auto": 0, "lattice": 1, "grid": 2}
@@ -113,6 +114,10 @@ def lib():
         L.snaps_sample_distance_histogram.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, i32, vp, i32, vp, vp, sz, vp]
         L.snaps_eps_from_histogram.restype = i32
         L.snaps_eps_from_histogram.argtypes = [vp, i32, i32, vp, i64, i64, ctypes.c_double, vp]
+        L.snaps_eps_search_workspace_bytes.restype = sz
+        L.snaps_eps_search_workspace_bytes.argtypes = [i32, i32, i32, i32, i32]
+        L.snaps_eps_search.restype = i32
+        L.snaps_eps_search.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, i32, i32, vp, i32, vp, vp, vp, vp, sz, vp]
         L.snaps_select_k_workspace_bytes.restype = sz
         L.snaps_select_k_workspace_bytes.argtypes = [i64, i32, i32]
         L.snaps_knn_select_k.restype = i32
@@ -524,3 +529,40 @@ def eps_from_histogram(hist_host, rmax, N: int, pairs_per_mask: int, target_s: f
                                           r.ctypes.data_as(ctypes.c_void_p), N, pairs_per_mask, float(target_s),
                                           eps.ctypes.data_as(ctypes.c_void_p)))
     return eps
+
+
+def eps_search(X, masks, sample_q, sample_c, targets, n_bins: int = 4096, *, hist=False, stream=None):
+    """snaps_eps_search -> dict eps_mean [n_masks], eps [n_masks, n_targets] (CUDA fp32) and, if asked,
+    hist [n_masks, n_bins] (int64)."""
+    import torch
+    m = _masks(masks)
+    q = np.ascontiguousarray(np.asarray(sample_q, dtype=np.int32))
+    c = np.ascontiguousarray(np.asarray(sample_c, dtype=np.int32))
+    t = np.ascontiguousarray(np.asarray(targets, dtype=np.float64).ravel())
+    N, n_feat = X.shape
+    dev = X.device
+    out = {"eps_mean": torch.empty(len(m), dtype=torch.float32, device=dev),
+           "eps": torch.empty((len(m), len(t)), dtype=torch.float32, device=dev)}
+    if hist:
+        out["hist"] = torch.empty((len(m), n_bins), dtype=torch.int64, device=dev)
+    ws = torch.empty(int(lib().snaps_eps_search_workspace_bytes(len(q), len(c), len(m), n_bins, len(t))),
+                     dtype=torch.uint8, device=dev)
+    _check(lib().snaps_eps_search(
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
+        q.ctypes.data_as(ctypes.c_void_p), len(q), c.ctypes.data_as(ctypes.c_void_p), len(c), n_bins,
+        t.ctypes.data_as(ctypes.c_void_p), len(t), _dptr(out["eps_mean"]), _dptr(out["eps"]), _dptr(out.get("hist")),
+        _dptr(ws), ws.numel(), _stream(stream)))
+    out["_workspace"] = ws
+    return out
+
+
+def eps_for_selectivity(X, masks, target_neighbours: float, seed: int = 0, n_query_sample: int = 1000,
+                        n_cand_sample: int = 100_000, n_bins: int = 8192) -> np.ndarray:
+    """Radii for a target mean neighbour count from seeded samples (marshalling around snaps_eps_search:
+    the sample ids are drawn here, the search runs on the device).  -> fp32 [n_masks] on the host."""
+    N = X.shape[0]
+    rng = np.random.default_rng(seed)
+    q = np.sort(rng.choice(N, min(n_query_sample, N), replace=False))
+    c = np.sort(rng.choice(N, min(n_cand_sample, N), replace=False))
+    out = eps_search(X, masks, q, c, [target_neighbours], n_bins)
+    return out["eps"][:, 0].cpu().numpy()

@@ -9,6 +9,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <iterator>
 #include <map>
 #include <utility>
 #include <vector>
@@ -982,6 +983,43 @@ snaps_status snaps_sample_distance_histogram(const float* d_X, int64_t N, int n_
         return fail(SNAPS_WORKSPACE_TOO_SMALL, "histogram workspace too small");
     CUDA_TRY(snaps::dist_hist_launch(d_X, ld, n_feat, h_sample_q, nq, h_sample_c, nc, h_masks, h_rmax, n_masks,
                                      n_bins, out_hist, d_workspace, static_cast<cudaStream_t>(stream)));
+    return SNAPS_OK;
+}
+
+size_t snaps_eps_search_workspace_bytes(int nq, int nc, int n_masks, int n_bins, int n_targets) {
+    if (nq < 1 || nc < 1 || n_masks < 1 || n_bins < 1 || n_bins > 8192 || n_targets < 1) return 0;
+    return snaps::eps_search_workspace_bytes(nq, nc, n_masks, n_bins, n_targets);
+}
+
+snaps_status snaps_eps_search(const float* d_X, int64_t N, int n_feat, int64_t ld, const uint16_t* h_masks, int n_masks,
+                              const int32_t* h_sample_q, int nq, const int32_t* h_sample_c, int nc, int n_bins,
+                              const double* h_target_s, int n_targets, float* out_eps_mean, float* out_eps,
+                              unsigned long long* out_hist, void* d_workspace, size_t workspace_bytes, void* stream) {
+    const Job job = Job{d_X, N, n_feat, ld, h_masks, n_masks, 0, N, 0, SNAPS_ENGINE_LATTICE};
+    snaps_status rc = check_job(job, 0);
+    if (rc) return rc;
+    if (!h_sample_q || !h_sample_c || !h_target_s || !out_eps_mean || !out_eps || nq < 1 || nc < 1 || n_targets < 1)
+        return fail(SNAPS_INVALID_ARG, "NULL or empty samples, targets or outputs");
+    if (n_bins < 1 || n_bins > 8192) return fail(SNAPS_INVALID_ARG, "n_bins = %d outside 1..8192", n_bins);
+    for (int t = 0; t < n_targets; ++t)
+        if (!(h_target_s[t] > 0.0)) return fail(SNAPS_INVALID_ARG, "target selectivity %d is not > 0", t);
+    // pairs with c != q: both samples are id lists; count the ids they share
+    std::vector<int32_t> a(h_sample_q, h_sample_q + nq), b(h_sample_c, h_sample_c + nc);
+    for (int32_t v : a) if (v < 0 || v >= N) return fail(SNAPS_INVALID_ARG, "query sample id out of range");
+    for (int32_t v : b) if (v < 0 || v >= N) return fail(SNAPS_INVALID_ARG, "candidate sample id out of range");
+    std::sort(a.begin(), a.end());
+    std::sort(b.begin(), b.end());
+    if (std::adjacent_find(a.begin(), a.end()) != a.end() || std::adjacent_find(b.begin(), b.end()) != b.end())
+        return fail(SNAPS_INVALID_ARG, "sample ids must be distinct");
+    std::vector<int32_t> both;
+    std::set_intersection(a.begin(), a.end(), b.begin(), b.end(), std::back_inserter(both));
+    const long long pairs = static_cast<long long>(nq) * nc - static_cast<long long>(both.size());
+    if (pairs < 1) return fail(SNAPS_INVALID_ARG, "no sampled pair with c != q");
+    if (!d_workspace || workspace_bytes < snaps::eps_search_workspace_bytes(nq, nc, n_masks, n_bins, n_targets))
+        return fail(SNAPS_WORKSPACE_TOO_SMALL, "eps search workspace too small");
+    CUDA_TRY(snaps::eps_search_launch(d_X, N, ld, n_feat, h_sample_q, nq, h_sample_c, nc, pairs, h_masks, n_masks, n_bins,
+                                      h_target_s, n_targets, out_eps_mean, out_eps, out_hist, d_workspace,
+                                      static_cast<cudaStream_t>(stream)));
     return SNAPS_OK;
 }
 
