@@ -283,8 +283,10 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
         float qhi[9];
         {
             const float* qr = p.Xp + static_cast<size_t>(q) * kRowFloats;
+            float qlo[kLow];
 #pragma unroll
-            for (int j = 0; j < kLow; ++j) fq.qlo[j] = qr[j];
+            for (int j = 0; j < kLow; ++j) qlo[j] = qr[j];
+            filter_query_set_row(fq, qlo);
 #pragma unroll
             for (int j = 0; j < 9; ++j) qhi[j] = qr[kLow + j];
             if (lane < 15) QROW(lane) = qr[lane];
@@ -297,10 +299,7 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             SLOT(lane) = bd->slot[lane];
             SLOT(lane + 32) = bd->slot[lane + 32];
             knn_seed<S>(ws, p.Xp, q, k, H, has_prev, lane);
-            // group 0 = lattice slots {}, {0}, {1}, {0,1}: when only {0,1} is asked for (always so for
-            // masks of >= 2 features when H is empty), its own sum is the group's bound -- X[0] alone
-            // would be 0 there and let every candidate through
-            filter_query_init(fq, qhi, H, (SLOT(0) < 0) & (SLOT(1) < 0) & (SLOT(2) < 0));
+            filter_query_init(fq, qhi, H);
             float G[16];
             RELOAD_G();
             int qhead = 0, qtail = 0;  // queue positions (warp-uniform, monotone)
@@ -309,7 +308,7 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
 #define FILTER_BLOCK(r, t_)                                                                   \
     {                                                                                         \
         PairTerms pt;                                                                         \
-        const bool pass = lattice_filter<false>(r, fq, G, pt);                                \
+        const bool pass = lattice_filter<G0>(r, fq, G, pt);                                   \
         const unsigned bal = __ballot_sync(kFull, pass);                                      \
         if (bal) {                                                                            \
             qtail += queue_push(QUEUE4, kQueue, qtail, pass, bal, lt, (t_) * 32 + lane, pt);  \
@@ -320,18 +319,25 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             }                                                                                 \
         }                                                                                     \
     }
-            Blk ra, rb;
-            load_block(ra, p.Xb, 0, lane);
-            rb = ra;
+            auto stream_table = [&](auto g0_tag) {
+                constexpr bool G0 = decltype(g0_tag)::value;
+                Blk ra, rb;
+                load_block(ra, p.Xb, 0, lane);
+                rb = ra;
 #pragma unroll 1
-            for (int t = 0; t < n_blocks; t += 2) {
-                if (t + 1 < n_blocks) load_block(rb, p.Xb, t + 1, lane);
-                FILTER_BLOCK(ra, t)
-                if (t + 1 < n_blocks) {
-                    if (t + 2 < n_blocks) load_block(ra, p.Xb, t + 2, lane);
-                    FILTER_BLOCK(rb, t + 1)
+                for (int t = 0; t < n_blocks; t += 2) {
+                    if (t + 1 < n_blocks) load_block(rb, p.Xb, t + 1, lane);
+                    FILTER_BLOCK(ra, t)
+                    if (t + 1 < n_blocks) {
+                        if (t + 2 < n_blocks) load_block(ra, p.Xb, t + 2, lane);
+                        FILTER_BLOCK(rb, t + 1)
+                    }
                 }
-            }
+            };
+            // group 0 = lattice slots {}, {0}, {1}, {0,1}: when only {0,1} is asked for (the batch without
+            // high features), the group is bounded by that slot's own sum (lattice_filter<true>)
+            if ((SLOT(0) < 0) & (SLOT(1) < 0) & (SLOT(2) < 0)) stream_table(TrueTag{});
+            else stream_table(FalseTag{});
 #undef FILTER_BLOCK
             if (qtail > qhead) knn_refine<S>(ws, k, lane, q, p.N, qhead, qtail - qhead);
             knn_emit<S>(ws, p, q, lane);

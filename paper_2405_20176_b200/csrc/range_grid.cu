@@ -80,8 +80,10 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
         float qhi[9];
         {
             const float* qr = p.Xp + static_cast<size_t>(q) * kRowFloats;
+            float qlo[kLow];
 #pragma unroll
-            for (int j = 0; j < kLow; ++j) fq.qlo[j] = qr[j];
+            for (int j = 0; j < kLow; ++j) qlo[j] = qr[j];
+            filter_query_set_row(fq, qlo);
 #pragma unroll
             for (int j = 0; j < 9; ++j) qhi[j] = qr[kLow + j];
         }
@@ -99,7 +101,8 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
             }
         }
         __syncwarp();
-        filter_query_init(fq, qhi, H, (G_SLOT(0) < 0) & (G_SLOT(1) < 0) & (G_SLOT(2) < 0));
+        filter_query_init(fq, qhi, H);
+        const bool g0_both = (G_SLOT(0) < 0) & (G_SLOT(1) < 0) & (G_SLOT(2) < 0);
         float Gm[16];
 #pragma unroll
         for (int u = 0; u < 16; ++u)
@@ -113,7 +116,7 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
             const Blk r = nx;
             if (t + 1 < n_blocks) load_block(nx, p.Xb, t + 1, lane);
             PairTerms pt;
-            const bool pass = lattice_filter<false>(r, fq, Gm, pt);
+            const bool pass = g0_both ? lattice_filter<true>(r, fq, Gm, pt) : lattice_filter<false>(r, fq, Gm, pt);
             const unsigned bal = __ballot_sync(kFull, pass);
             if (bal) {
                 qtail += queue_push(G_QUEUE4, kGQueue, qtail, pass, bal, lt, t * 32 + lane, pt);

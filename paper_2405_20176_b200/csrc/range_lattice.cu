@@ -94,8 +94,10 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
         float qhi[9];
         {
             const float* qr = p.Xp + static_cast<size_t>(q) * kRowFloats;
+            float qlo[kLow];
 #pragma unroll
-            for (int j = 0; j < kLow; ++j) fq.qlo[j] = qr[j];
+            for (int j = 0; j < kLow; ++j) qlo[j] = qr[j];
+            filter_query_set_row(fq, qlo);
 #pragma unroll
             for (int j = 0; j < 9; ++j) qhi[j] = qr[kLow + j];
         }
@@ -113,9 +115,7 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
                 R_SUM(L) = 0.f;
             }
             __syncwarp();
-            // group 0 = lattice slots {}, {0}, {1}, {0,1}: when only {0,1} is asked for, its own sum is
-            // the group's bound (X[0] alone is 0 when H is empty and would let every candidate through)
-            filter_query_init(fq, qhi, H, (R_SLOT(0) < 0) & (R_SLOT(1) < 0) & (R_SLOT(2) < 0));
+            filter_query_init(fq, qhi, H);
             float G[16];   // group maxima of the (constant) thresholds
 #pragma unroll
             for (int u = 0; u < 16; ++u) {
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
 #define FILTER_BLOCK(r, t_)                                                                   \
     {                                                                                         \
         PairTerms pt;                                                                         \
-        const bool pass = lattice_filter<false>(r, fq, G, pt);                                \
+        const bool pass = lattice_filter<G0>(r, fq, G, pt);                                   \
         const unsigned bal = __ballot_sync(kFull, pass);                                      \
         if (bal) {                                                                            \
             qtail += queue_push(R_QUEUE4, kRQueue, qtail, pass, bal, lt, (t_) * 32 + lane, pt); \
@@ -136,18 +136,25 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
             }                                                                                 \
         }                                                                                     \
     }
-            Blk ra, rb;
-            load_block(ra, p.Xb, 0, lane);
-            rb = ra;
+            auto stream_table = [&](auto g0_tag) {
+                constexpr bool G0 = decltype(g0_tag)::value;
+                Blk ra, rb;
+                load_block(ra, p.Xb, 0, lane);
+                rb = ra;
 #pragma unroll 1
-            for (int t = 0; t < n_blocks; t += 2) {
-                if (t + 1 < n_blocks) load_block(rb, p.Xb, t + 1, lane);
-                FILTER_BLOCK(ra, t)
-                if (t + 1 < n_blocks) {
-                    if (t + 2 < n_blocks) load_block(ra, p.Xb, t + 2, lane);
-                    FILTER_BLOCK(rb, t + 1)
+                for (int t = 0; t < n_blocks; t += 2) {
+                    if (t + 1 < n_blocks) load_block(rb, p.Xb, t + 1, lane);
+                    FILTER_BLOCK(ra, t)
+                    if (t + 1 < n_blocks) {
+                        if (t + 2 < n_blocks) load_block(ra, p.Xb, t + 2, lane);
+                        FILTER_BLOCK(rb, t + 1)
+                    }
                 }
-            }
+            };
+            // group 0 = lattice slots {}, {0}, {1}, {0,1}: when only {0,1} is asked for, the group is
+            // bounded by that slot's own sum (X[0] alone is 0 when H is empty)
+            if ((R_SLOT(0) < 0) & (R_SLOT(1) < 0) & (R_SLOT(2) < 0)) stream_table(TrueTag{});
+            else stream_table(FalseTag{});
 #undef FILTER_BLOCK
             if (qtail > qhead) range_refine<WITH_SUM>(ws, lane, q, p.N, qhead, qtail - qhead);
             // ---- a7: counts, sums, means (0 when there is no neighbour: PAPER.md:266, reading A6)

@@ -62,21 +62,60 @@ __device__ __forceinline__ void load_block(Blk& dst, const float4* __restrict__ 
     dst.v3 = __ldg(b + 96);
 }
 
+// Packed fp32 pairs (sm_100: add / mul / fma .rn.f32x2 -> SASS FADD2 / FMUL2 / FFMA2): two IEEE
+// round-to-nearest results per issued instruction, bit-identical to the scalar operations.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+
+struct TrueTag { static constexpr bool value = true; };
+struct FalseTag { static constexpr bool value = false; };
+
 // The per-query, per-batch constants of the filter.
 struct FilterQuery {
-    float qlo[kLow];   // the query's lattice features
-    float w[9];        // high features: diff = c*w - q*w with w in {0,1} (1 = feature in H)
-    float wq[9];
-    bool g0_both;      // group 0 asked for {0,1} only: its own sum is the group's bound
+    f32x2 nq01, nq23, nq45;   // the query's lattice features, negated, in pairs: c - q = c + (-q)
+    f32x2 w2[4], nwq2[4];     // high features 6..13 in pairs: diff = c*w - q*w with w in {0,1} (1 = feature in H)
+    float w14, nwq14;         // high feature 14
 };
 
-__device__ __forceinline__ void filter_query_init(FilterQuery& f, const float (&qhi)[9], uint32_t H, bool g0_both) {
+__device__ __forceinline__ void filter_query_set_row(FilterQuery& f, const float (&qlo)[kLow]) {
+    f.nq01 = pack2(-qlo[0], -qlo[1]);
+    f.nq23 = pack2(-qlo[2], -qlo[3]);
+    f.nq45 = pack2(-qlo[4], -qlo[5]);
+}
+
+__device__ __forceinline__ void filter_query_init(FilterQuery& f, const float (&qhi)[9], uint32_t H) {
+    float w[9];
 #pragma unroll
-    for (int j = 0; j < 9; ++j) {
-        f.w[j] = ((H >> (kLow + j)) & 1u) ? 1.f : 0.f;
-        f.wq[j] = f.w[j] * qhi[j];
+    for (int j = 0; j < 9; ++j) w[j] = ((H >> (kLow + j)) & 1u) ? 1.f : 0.f;
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        f.w2[p] = pack2(w[2 * p], w[2 * p + 1]);
+        f.nwq2[p] = pack2(-(w[2 * p] * qhi[2 * p]), -(w[2 * p + 1] * qhi[2 * p + 1]));
     }
-    f.g0_both = g0_both;
+    f.w14 = w[8];
+    f.nwq14 = -(w[8] * qhi[8]);
 }
 
 // What the refine step needs of a candidate that passed: the high-feature part of every sum and the
@@ -87,44 +126,62 @@ struct PairTerms {
 };
 
 // FILTER of one candidate (this lane's row of block r): the six lattice squared differences, the
-// high-feature part `base` (FMA chain in feature order), the 16 partial sums X[u] over subsets u
-// of features {2,3,4,5} (add-only), and the test of each X[u] -- a lower bound of the four sums
-// X[u] (+sq0) (+sq1) of group u -- against the group's largest threshold G[u].
-// INCL = let equality through (not used by the in-order scans).
-template <bool INCL>
+// high-feature part `base`, the 16 partial sums X[u] over subsets u of features {2,3,4,5} (add-only),
+// and the test of each X[u] -- a lower bound of the four sums X[u] (+sq0) (+sq1) of group u --
+// against the group's largest threshold G[u].
+// Arithmetic in packed pairs where two values take the same operation: the squared differences of
+// features (0,1), (2,3), (4,5); base = two FMA chains over the even and the odd high features
+// (6,8,10,12 and 7,9,11,13), their sum, then feature 14 -- one fixed order, used wherever a base is
+// formed; the partial sums pairwise (X[2v], X[2v+1]) + (sq, sq).  45 scalar operations become 25.
+// G0BOTH: group 0 = lattice slots {}, {0}, {1}, {0,1} and only {0,1} is asked for (the batch with
+// H empty): its own sum is the group's bound -- X[0] alone would be 0 there and let every candidate through.
+template <bool G0BOTH>
 __device__ __forceinline__ bool lattice_filter(const Blk& r, const FilterQuery& f, const float (&G)[16],
                                                PairTerms& out) {
-    const float c[15] = {r.v0.x, r.v0.y, r.v0.z, r.v0.w, r.v1.x, r.v1.y, r.v1.z, r.v1.w,
-                         r.v2.x, r.v2.y, r.v2.z, r.v2.w, r.v3.x, r.v3.y, r.v3.z};
     // keep the padding word of the fourth load live until here: otherwise its register is handed
     // out as scratch while the prefetch is still in flight and the warp stalls on it
     asm volatile("" ::"f"(r.v3.w));
-#pragma unroll
-    for (int j = 0; j < kLow; ++j) {
-        const float diff = c[j] - f.qlo[j];
-        out.sq[j] = __fmul_rn(diff, diff);
+    const f32x2 d01 = add2(pack2(r.v0.x, r.v0.y), f.nq01);
+    const f32x2 d23 = add2(pack2(r.v0.z, r.v0.w), f.nq23);
+    const f32x2 d45 = add2(pack2(r.v1.x, r.v1.y), f.nq45);
+    const f32x2 s01 = mul2(d01, d01), s23 = mul2(d23, d23), s45 = mul2(d45, d45);
+    unpack2(s01, out.sq[0], out.sq[1]);
+    unpack2(s23, out.sq[2], out.sq[3]);
+    unpack2(s45, out.sq[4], out.sq[5]);
+    f32x2 b2 = 0ull;
+    {
+        const f32x2 c67 = pack2(r.v1.z, r.v1.w), c89 = pack2(r.v2.x, r.v2.y), cab = pack2(r.v2.z, r.v2.w),
+                    ccd = pack2(r.v3.x, r.v3.y);
+        f32x2 d;
+        d = fma2(c67, f.w2[0], f.nwq2[0]); b2 = fma2(d, d, b2);
+        d = fma2(c89, f.w2[1], f.nwq2[1]); b2 = fma2(d, d, b2);
+        d = fma2(cab, f.w2[2], f.nwq2[2]); b2 = fma2(d, d, b2);
+        d = fma2(ccd, f.w2[3], f.nwq2[3]); b2 = fma2(d, d, b2);
     }
-    float base = 0.f;
-#pragma unroll
-    for (int j = 0; j < 9; ++j) {
-        const float diff = __fmaf_rn(c[kLow + j], f.w[j], -f.wq[j]);
-        base = __fmaf_rn(diff, diff, base);
-    }
+    float be, bo;
+    unpack2(b2, be, bo);
+    const float d14 = __fmaf_rn(r.v3.z, f.w14, f.nwq14);
+    const float base = __fmaf_rn(d14, d14, __fadd_rn(be, bo));
     out.base = base;
-    float X[16];
-    X[0] = base;
+    // X[u], u = subset of {2,3,4,5}: pairs (X[2v], X[2v+1]) = (., . + sq2)
+    const f32x2 q3 = pack2(out.sq[3], out.sq[3]), q4 = pack2(out.sq[4], out.sq[4]), q5 = pack2(out.sq[5], out.sq[5]);
+    f32x2 P[8];
+    P[0] = pack2(base, __fadd_rn(base, out.sq[2]));
+    P[1] = add2(P[0], q3);
+    P[2] = add2(P[0], q4);
+    P[3] = add2(P[1], q4);
 #pragma unroll
-    for (int u = 1; u < 16; ++u) {
-        const int hb = 31 - __clz(u);
-        X[u] = __fadd_rn(X[u & ~(1 << hb)], out.sq[2 + hb]);
-    }
+    for (int v = 0; v < 4; ++v) P[4 + v] = add2(P[v], q5);
+    float X[16];
+#pragma unroll
+    for (int v = 0; v < 8; ++v) unpack2(P[v], X[2 * v], X[2 * v + 1]);
     float x0 = X[0];
-    if (f.g0_both) x0 = __fadd_rn(__fadd_rn(X[0], out.sq[0]), out.sq[1]);
-    bool pa = INCL ? (x0 <= G[0]) : (x0 < G[0]), pb = false;
+    if (G0BOTH) x0 = __fadd_rn(__fadd_rn(X[0], out.sq[0]), out.sq[1]);
+    bool pa = x0 < G[0], pb = false;
 #pragma unroll
     for (int u = 0; u < 16; u += 2) {
-        if (u > 0) pa |= INCL ? (X[u] <= G[u]) : (X[u] < G[u]);
-        pb |= INCL ? (X[u + 1] <= G[u + 1]) : (X[u + 1] < G[u + 1]);
+        if (u > 0) pa |= X[u] < G[u];
+        pb |= X[u + 1] < G[u + 1];
     }
     return pa | pb;
 }
