@@ -440,6 +440,10 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-lsst", action="store_true", help="skip the LSST-scale leg (config 4) of the default run")
     ap.add_argument("--no-dssj", action="store_true", help="skip the DSSJ leg (config 3) of the default run")
+    ap.add_argument("--masks-limit", type=int, default=0,
+                    help="headline step on the first M masks only, for `ncu --set full` captures (ncu replays a launch "
+                         "~40 times and saves / restores its 12.5 GB of outputs around each replay); the line is marked "
+                         "`partial` and is NOT a bench value")
     ap.add_argument("--c5-n", type=int, default=0, help="config 5 with a reduced N (quick runs)")
     ap.add_argument("--c5-masks", type=int, default=0, help="config 5 on its first M masks only (quick runs)")
     args = ap.parse_args()
@@ -491,6 +495,8 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
     weak = world > 1 and args.scaling == "weak"
     X = workloads.make_table(cfg.n, cfg.seed + (rank if weak else 0), cols=list(range(cfg.n_feat)), outlier_frac=0.01)
     masks_all = cfg.masks()
+    if args.masks_limit > 0:
+        masks_all = masks_all[:args.masks_limit]
     mine = np.arange(len(masks_all)) if (world == 1 or weak) else shard_masks(masks_all, rank, world)
     masks = masks_all[mine]
     N, n_feat, k, n_masks = len(X), X.shape[1], cfg.k, len(masks)
@@ -595,7 +601,7 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
 
     # ---- the other configs, side by side (north star): DSSJ (config 3), LSST scale (config 4)
     dssj = lsst = None
-    default_run = world == 1 and args.config == "c2_snapshot1_knn"
+    default_run = world == 1 and args.config == "c2_snapshot1_knn" and args.masks_limit == 0
     Xd = ws = out = None
     torch.cuda.empty_cache()
     if default_run and not args.no_dssj:
@@ -619,6 +625,7 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
 
     if rank == 0:
         line = {
+            **({"partial": f"first {args.masks_limit} masks only (--masks-limit): not a bench value"} if args.masks_limit > 0 else {}),
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
             "scaling": "weak" if weak else "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",

@@ -404,6 +404,30 @@ snaps_status snaps_eps_search(const float *d_X, int64_t N, int n_feat, int64_t l
                               void *d_workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * eps^select per feature space in one call (section 3.5.2, 229-239 section 3.5.3) --
+ * the DSSJ twin of snaps_knn_select_k: (1) eps_min and eps_max for the selectivities s_min < s_max by
+ * snaps_eps_search; (2) the grid of G evenly spaced radii between them (fp32; |G| is not given in the
+ * paper, reading A17); (3) one range join at eps_max binned over the grid; (4) for
+ * the neighbour-count metric and the mean-distance metric: ranks at every radius, their top-n overlap
+ * with the ranks at eps_min (U_min) and at eps_max (U_max) (Eq. 2), and the radius that minimises
+ * |U_min - U_max| (Eq. 3).
+ *   out_eps_grid   device [n_masks][G] fp32 or NULL: the radii
+ *   out_j_count, out_j_mean  device [n_masks] int32: index of the selected radius per metric
+ *   out_u          device [4][G][n_masks] fp32 or NULL (as snaps_knn_select_k)
+ * Workspace: snaps_select_eps_workspace_bytes(...) (it holds the [n_masks][G][N] scores and orders:
+ * call it on a few hundred masks at a time).
+ */
+size_t snaps_select_eps_workspace_bytes(int64_t N, int n_feat, int n_masks, int G, int nq, int nc,
+                                        int n_bins, int flags);
+
+snaps_status snaps_range_select_eps(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                    const uint16_t *h_masks, int n_masks,
+                                    const int32_t *h_sample_q, int nq, const int32_t *h_sample_c, int nc,
+                                    int n_bins, double s_min, double s_max, int G, int n_top, int flags,
+                                    float *out_eps_grid, int32_t *out_j_count, int32_t *out_j_mean,
+                                    float *out_u, void *d_workspace, size_t workspace_bytes, void *stream);
+
+/*
  * Host arithmetic on a histogram copied back from the device: the cumulative histogram gives the
  * mean number of neighbours per point at each bin edge, mean(r_b) = cum[b] * (N-1) / (nq * nc')
  * with nc' = candidates per query (nc, minus one where the query is in the candidate sample --

@@ -82,3 +82,37 @@ def eps_from_histogram(hist, rmax, N: int, pairs_per_mask: int, target_s: float)
         if len(hit):
             eps[mi] = float(rmax[mi]) * (hit[0] + 1) / hist.shape[1]
     return eps
+
+
+def mean_sample_distance(X, masks, q_ids, c_ids):
+    """eps_mean: the mean of D(q, c; mask) over the sampled (query, candidate) pairs with
+    c != q by index -- "the mean distance between points in a dataset", estimated on a sample and used as
+    the upper bound of the search radius.  fp64.  -> (eps_mean [n_masks], number of pairs)."""
+    X = np.ascontiguousarray(X, dtype=np.float32)
+    q_ids = np.asarray(q_ids, dtype=np.int64)
+    c_ids = np.asarray(c_ids, dtype=np.int64)
+    out = np.zeros(len(masks), dtype=np.float64)
+    pairs = 0
+    for mi, m in enumerate(masks):
+        tot, cnt = 0.0, 0
+        for q in q_ids:
+            row = dist_row(X, m, int(q))[c_ids]
+            keep = c_ids != q
+            tot += float(row[keep].sum())
+            cnt += int(keep.sum())
+        out[mi] = tot / cnt
+        pairs = cnt
+    return out, pairs
+
+
+def eps_search(X, masks, q_ids, c_ids, n_bins: int, targets):
+    """The search of PAPER.md:229-237, step by step: eps_mean from the sample; the histogram of the sampled
+    distances over [0, eps_mean) (the range as the 32-bit value the method carries); its
+    cumulative form -> for every target selectivity the first bin edge that reaches it (eps_mean if none).
+    -> (eps_mean fp32 [n_masks], eps fp32 [n_masks][n_targets], hist, distances per mask)."""
+    N = len(X)
+    eps_mean, pairs = mean_sample_distance(X, masks, q_ids, c_ids)
+    rmax = eps_mean.astype(np.float32)
+    hist, dists = sampled_histogram(X, masks, q_ids, c_ids, rmax, n_bins)
+    eps = np.stack([eps_from_histogram(hist, rmax, N, pairs, float(t)) for t in targets], axis=1)
+    return rmax, eps.astype(np.float32), hist, dists

@@ -80,17 +80,55 @@ def knn_scores_at_k(idx_kmax, dist_kmax, kj: int, N: int):
     return dist[:, -1], dist.mean(axis=1), np.bincount(idx.ravel(), minlength=N)
 
 
+def mean_in_list_order_fp32(dist_kmax, kj: int) -> np.ndarray:
+    """The mean kNN distance as a 32-bit value: the first k_j distances added one by one in list order
+    in fp32, then divided by k_j ("32-bit floating point" throughout).  Rank decisions on
+    the distance-aware kNN metric are taken on this value (reading A21), so that objects whose
+    means differ by less than an fp32 rounding do not change order between implementations."""
+    d = np.asarray(dist_kmax, dtype=np.float32)[:, :kj]
+    return (np.cumsum(d, axis=1, dtype=np.float32)[:, -1] / np.float32(kj)).astype(np.float32)
+
+
 def select_k(idx_kmax, dist_kmax, k_grid, n: int, N: int):
     """The k-grid procedure of PAPER.md:256-258 for ONE mask, step by step: for every k_j the scores
     from the k_max lists, their top-n sets, U_min / U_max against the smallest and largest k
     (Eq. 2), and the selected grid index (Eq. 3) -- for the in-degree and the mean-distance metric.
+    The mean-distance ranks are decided on the fp32 mean (reading A21).
     -> dict metric -> (j_select, u_min, u_max)."""
     out = {}
     for metric, pick in (("knn_indegree", 2), ("knn_mean", 1)):
         tops = []
         for kj in k_grid:
             sc = knn_scores_at_k(idx_kmax, dist_kmax, int(kj), N)
-            tops.append(topn_ids(metric, sc[pick], n))
+            score = sc[pick] if metric == "knn_indegree" else mean_in_list_order_fp32(dist_kmax, int(kj))
+            tops.append(topn_ids(metric, score, n))
         u_min, u_max = similarity_curves(tops, n)
         out[metric] = (select_parameter(u_min, u_max, n), u_min, u_max)
+    return out
+
+
+def eps_grid(eps_min, eps_max, G: int) -> np.ndarray:
+    """The grid G of PAPER.md:181: |G| evenly spaced radii, eps_1 = eps_min, eps_|G| = eps_max
+    (PAPER.md:183), carried as 32-bit values with every operation rounded:
+    eps_j = eps_min + (j - 1) * ((eps_max - eps_min) / (|G| - 1)), the last one eps_max itself."""
+    e0, e1 = np.float32(eps_min), np.float32(eps_max)
+    step = np.float32(np.float32(e1 - e0) / np.float32(G - 1))
+    grid = np.array([np.float32(e0 + np.float32(np.float32(g) * step)) for g in range(G)], dtype=np.float32)
+    grid[G - 1] = e1
+    return grid
+
+
+def select_eps(counts, means, n: int):
+    """The eps-grid procedure of PAPER.md:181-189 for ONE mask from the join results at every radius
+    (counts [G][N], means [G][N]; means 0 where the count is 0): top-n sets per radius for the number-of-
+    neighbours metric and the mean-distance metric, U_min / U_max against the smallest and the largest
+    radius (Eq. 2), the selected grid index (Eq. 3).  -> dict metric -> (j_select, u_min, u_max)."""
+    out = {}
+    G = len(counts)
+    tops = [topn_ids("dssj_count", counts[g], n) for g in range(G)]
+    u_min, u_max = similarity_curves(tops, n)
+    out["dssj_count"] = (select_parameter(u_min, u_max, n), u_min, u_max)
+    tops = [topn_ids("dssj_mean", means[g], n, counts=counts[g]) for g in range(G)]
+    u_min, u_max = similarity_curves(tops, n)
+    out["dssj_mean"] = (select_parameter(u_min, u_max, n), u_min, u_max)
     return out

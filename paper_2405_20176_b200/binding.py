@@ -19,6 +19,7 @@ EXPORTED_SYMBOLS = [
     "snaps_select_k_workspace_bytes", "snaps_knn_select_k",
     "snaps_dist_hist_workspace_bytes", "snaps_sample_distance_histogram", "snaps_eps_from_histogram",
     "snaps_eps_search_workspace_bytes", "snaps_eps_search",
+    "snaps_select_eps_workspace_bytes", "snaps_range_select_eps",
 ]
 
 ENGINES = {"auto": 0, "lattice": 1, "grid": 2}
@@ -118,6 +119,11 @@ def lib():
         L.snaps_eps_search_workspace_bytes.argtypes = [i32, i32, i32, i32, i32]
         L.snaps_eps_search.restype = i32
         L.snaps_eps_search.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, i32, i32, vp, i32, vp, vp, vp, vp, sz, vp]
+        L.snaps_select_eps_workspace_bytes.restype = sz
+        L.snaps_select_eps_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, i32, i32]
+        L.snaps_range_select_eps.restype = i32
+        L.snaps_range_select_eps.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, i32, i32, ctypes.c_double,
+                                             ctypes.c_double, i32, i32, i32, vp, vp, vp, vp, vp, sz, vp]
         L.snaps_select_k_workspace_bytes.restype = sz
         L.snaps_select_k_workspace_bytes.argtypes = [i64, i32, i32]
         L.snaps_knn_select_k.restype = i32
@@ -566,3 +572,30 @@ def eps_for_selectivity(X, masks, target_neighbours: float, seed: int = 0, n_que
     c = np.sort(rng.choice(N, min(n_cand_sample, N), replace=False))
     out = eps_search(X, masks, q, c, [target_neighbours], n_bins)
     return out["eps"][:, 0].cpu().numpy()
+
+
+def range_select_eps(X, masks, sample_q, sample_c, s_min: float, s_max: float, G: int, n_top: int, n_bins: int = 4096,
+                     *, engine="auto", stream=None):
+    """snaps_range_select_eps -> dict eps_grid [n_masks, G], j_count / j_mean [n_masks] (grid index of the
+    selected radius per DSSJ metric) and u [4, G, n_masks]."""
+    import torch
+    m = _masks(masks)
+    q = np.ascontiguousarray(np.asarray(sample_q, dtype=np.int32))
+    c = np.ascontiguousarray(np.asarray(sample_c, dtype=np.int32))
+    N, n_feat = X.shape
+    dev = X.device
+    out = {"eps_grid": torch.empty((len(m), G), dtype=torch.float32, device=dev),
+           "j_count": torch.empty(len(m), dtype=torch.int32, device=dev),
+           "j_mean": torch.empty(len(m), dtype=torch.int32, device=dev),
+           "u": torch.empty((4, G, len(m)), dtype=torch.float32, device=dev)}
+    nbytes = int(lib().snaps_select_eps_workspace_bytes(N, n_feat, len(m), G, len(q), len(c), n_bins, _flags(engine)))
+    if nbytes == 0:
+        raise SnapsError(1, "invalid sizes for the eps selection workspace")
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+    _check(lib().snaps_range_select_eps(
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m),
+        q.ctypes.data_as(ctypes.c_void_p), len(q), c.ctypes.data_as(ctypes.c_void_p), len(c), n_bins,
+        float(s_min), float(s_max), G, n_top, _flags(engine), _dptr(out["eps_grid"]), _dptr(out["j_count"]),
+        _dptr(out["j_mean"]), _dptr(out["u"]), _dptr(ws), ws.numel(), _stream(stream)))
+    out["_workspace"] = ws
+    return out

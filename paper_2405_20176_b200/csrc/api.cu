@@ -440,8 +440,9 @@ snaps_status grid_knn_enqueue(Engine* E, int m0, int nm, int k, const KnnOut& o)
     return SNAPS_OK;
 }
 
-// radii: device [n_masks][G] fl(eps^2) rows (G = 0: h_eps2 gives one value per mask)
-snaps_status grid_range_enqueue(Engine* E, int m0, int nm, const float* h_eps2, int G, const RangeOut& o) {
+// G > 0: d_radii = device [n_masks][G] fl(eps^2) rows; G = 0: h_eps2 gives one value per mask
+snaps_status grid_range_enqueue(Engine* E, int m0, int nm, const float* h_eps2, int G, const float* d_radii,
+                                const RangeOut& o) {
     const Job& j = E->job;
     const size_t nq = static_cast<size_t>(j.nq());
     const size_t per_mask = nq * static_cast<size_t>(G > 0 ? G : 1);
@@ -452,7 +453,7 @@ snaps_status grid_range_enqueue(Engine* E, int m0, int nm, const float* h_eps2, 
         CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, &E->gi, E->st));
         const size_t r = static_cast<size_t>(m - m0);
         p.G = G;
-        if (G > 0) p.eps2_grid = E->w.radii + static_cast<size_t>(m) * G;
+        if (G > 0) p.eps2_grid = d_radii + static_cast<size_t>(m) * G;
         else p.eps2 = h_eps2[m];
         p.out_count = o.count + r * per_mask;
         p.out_sum = o.sum ? o.sum + r * per_mask : nullptr;
@@ -577,7 +578,7 @@ snaps_status run_batched(Batched* B, const std::vector<snaps::BatchDesc>* all_ba
                 rc = lattice_range_enqueue(E, E->w.batches + (*group_off)[group],
                                            static_cast<int>((*group_off)[group + 1] - (*group_off)[group]), o);
             else
-                rc = grid_range_enqueue(E, m0, nm, B->h_eps2, 0, o);
+                rc = grid_range_enqueue(E, m0, nm, B->h_eps2, 0, nullptr, o);
         }
         if (rc != SNAPS_OK) return rc;
         CUDA_TRY(cudaEventRecord(side->computed[s], E->st));
@@ -730,6 +731,41 @@ snaps_status range_batched(const float* X, int64_t N, int n_feat, int64_t ld, co
     return run_batched(&B, &all, &group_off);
 }
 
+// The radius-grid join of either engine over thresholds already on the device ([n_masks][G]: fl(eps^2) for the
+// grid engine, its successor for the sub-lattice engine).
+snaps_status range_grid_run(Engine* E, int G, const float* d_thr, const RangeOut& o) {
+    const Job& j = E->job;
+    if (j.engine == SNAPS_ENGINE_GRID) return grid_range_enqueue(E, 0, j.n_masks, nullptr, G, d_thr, o);
+    std::vector<snaps::BatchDesc> batches;
+    plan_lattice(j.h_masks, j.n_masks, nullptr, 0, &batches);
+    const int nb = static_cast<int>(batches.size());
+    CUDA_TRY(cudaMemcpyAsync(E->w.batches, batches.data(), sizeof(snaps::BatchDesc) * nb, cudaMemcpyHostToDevice, E->st));
+    CUDA_TRY(cudaMemsetAsync(E->w.counter, 0, 256, E->st));
+    snaps::RangeGridParams p;
+    p.Xp = E->w.Xp;
+    p.Xb = E->w.Xb;
+    p.n_blocks = n_blocks_for(j.N);
+    p.N = static_cast<int>(j.N);
+    p.q_begin = static_cast<int>(j.q_begin);
+    p.nq = static_cast<int>(j.nq());
+    p.G = G;
+    p.batches = E->w.batches;
+    p.n_batches = nb;
+    p.thr_grid = d_thr;
+    p.warps = snaps::kRangeGridMaxThreads / 32;
+    while (p.warps > 1 && snaps::range_grid_smem_bytes(G, p.warps) > 227 * 1024) --p.warps;
+    p.work_counter = E->w.counter;
+    p.out_count = o.count;
+    p.out_sum = o.sum;
+    p.out_mean = o.mean;
+    const int64_t items = static_cast<int64_t>(p.nq) * nb;
+    const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
+    const bool prof = prof_begin(E->st);
+    CUDA_TRY(snaps::range_grid_launch(p, grid, E->st));
+    prof_end(prof, E->st);
+    return SNAPS_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -802,7 +838,7 @@ snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64
     rc = engine_begin(&E);
     if (rc) return rc;
     const RangeOut o = {out_count, out_sumdist, out_mean};
-    if (E.job.engine == SNAPS_ENGINE_GRID) return grid_range_enqueue(&E, 0, n_masks, e2.data(), 0, o);
+    if (E.job.engine == SNAPS_ENGINE_GRID) return grid_range_enqueue(&E, 0, n_masks, e2.data(), 0, nullptr, o);
     std::vector<snaps::BatchDesc> batches;
     plan_lattice(h_masks, n_masks, thr.data(), 0, &batches);
     CUDA_TRY(cudaMemcpyAsync(E.w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
@@ -916,45 +952,12 @@ snaps_status snaps_range_selfjoin_grid(const float* d_X, int64_t N, int n_feat, 
     if (rc) return rc;
     rc = engine_begin(&E);
     if (rc) return rc;
-    if (grid_engine) {
-        // the workspace has 32 radii per mask
-        CUDA_TRY(cudaMemcpyAsync(E.w.radii, thr.data(), thr.size() * 4, cudaMemcpyHostToDevice, E.st));
-        const RangeOut o = {out_count, out_sumdist, out_mean};
-        return grid_range_enqueue(&E, 0, n_masks, nullptr, G, o);
-    }
     const size_t grid_bytes = align_up(static_cast<size_t>(n_masks) * G * 4, 256);
     if (E.w.extra_bytes < grid_bytes)
         return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace lacks %zu bytes for the radius grid", grid_bytes);
-    std::vector<snaps::BatchDesc> batches;
-    plan_lattice(h_masks, n_masks, nullptr, 0, &batches);
-    const int nb = static_cast<int>(batches.size());
-    // pageable host sources: the copies are staged before cudaMemcpyAsync returns
-    CUDA_TRY(cudaMemcpyAsync(E.w.batches, batches.data(), sizeof(snaps::BatchDesc) * nb, cudaMemcpyHostToDevice, E.st));
+    // pageable host source: the copy is staged before cudaMemcpyAsync returns
     CUDA_TRY(cudaMemcpyAsync(E.w.extra, thr.data(), thr.size() * 4, cudaMemcpyHostToDevice, E.st));
-    CUDA_TRY(cudaMemsetAsync(E.w.counter, 0, 256, E.st));
-    snaps::RangeGridParams p;
-    p.Xp = E.w.Xp;
-    p.Xb = E.w.Xb;
-    p.n_blocks = n_blocks_for(N);
-    p.N = static_cast<int>(N);
-    p.q_begin = static_cast<int>(q_begin);
-    p.nq = static_cast<int>(q_end - q_begin);
-    p.G = G;
-    p.batches = E.w.batches;
-    p.n_batches = nb;
-    p.thr_grid = reinterpret_cast<const float*>(E.w.extra);
-    p.warps = snaps::kRangeGridMaxThreads / 32;
-    while (p.warps > 1 && snaps::range_grid_smem_bytes(G, p.warps) > 227 * 1024) --p.warps;
-    p.work_counter = E.w.counter;
-    p.out_count = out_count;
-    p.out_sum = out_sumdist;
-    p.out_mean = out_mean;
-    const int64_t items = static_cast<int64_t>(p.nq) * nb;
-    const int grid = static_cast<int>(std::min<int64_t>((items + p.warps - 1) / p.warps, sm_count()));
-    const bool prof = prof_begin(E.st);
-    CUDA_TRY(snaps::range_grid_launch(p, grid, E.st));
-    prof_end(prof, E.st);
-    return SNAPS_OK;
+    return range_grid_run(&E, G, reinterpret_cast<const float*>(E.w.extra), RangeOut{out_count, out_sumdist, out_mean});
 }
 
 size_t snaps_dist_hist_workspace_bytes(int nq, int nc, int n_masks) {
@@ -1020,6 +1023,102 @@ snaps_status snaps_eps_search(const float* d_X, int64_t N, int n_feat, int64_t l
     CUDA_TRY(snaps::eps_search_launch(d_X, N, ld, n_feat, h_sample_q, nq, h_sample_c, nc, pairs, h_masks, n_masks, n_bins,
                                       h_target_s, n_targets, out_eps_mean, out_eps, out_hist, d_workspace,
                                       static_cast<cudaStream_t>(stream)));
+    return SNAPS_OK;
+}
+
+// ---- DSSJ parameter selection in one call --------------------------------
+namespace {
+struct SelectEpsLayout {
+    size_t search, mm, grid, thr, score, order, u, rank, total;
+};
+SelectEpsLayout select_eps_layout(int64_t N, int n_masks, int G, int nq, int nc, int n_bins) {
+    SelectEpsLayout L;
+    const size_t rows = static_cast<size_t>(n_masks) * G;
+    L.search = align_up(snaps::eps_search_workspace_bytes(nq, nc, n_masks, n_bins, 2), 256);
+    L.mm = align_up(static_cast<size_t>(n_masks) * 3 * 4, 256);          // eps_mean, then (eps_min, eps_max) pairs
+    L.grid = align_up(rows * 4, 256);
+    L.thr = align_up(rows * 4, 256);
+    L.score = align_up(rows * static_cast<size_t>(N) * 4, 256);          // x3: count, sum, mean
+    L.order = align_up(rows * static_cast<size_t>(N) * 4, 256);
+    L.u = align_up(sizeof(float) * 4 * rows, 256);
+    L.rank = align_up(snaps::rank_workspace_bytes(N, static_cast<int>(rows)), 256);
+    L.total = L.search + L.mm + L.grid + L.thr + 3 * L.score + L.order + L.u + L.rank;
+    return L;
+}
+}  // namespace
+
+size_t snaps_select_eps_workspace_bytes(int64_t N, int n_feat, int n_masks, int G, int nq, int nc, int n_bins, int flags) {
+    if (N < 2 || n_feat < 1 || n_feat > SNAPS_MAX_FEATURES || n_masks < 1 || G < 2 || G > snaps::kRangeGridMaxRadii ||
+        nq < 1 || nc < 1 || n_bins < 1 || n_bins > 8192)
+        return 0;
+    const int engine = resolve_engine(flags, N, 0);
+    if (engine != SNAPS_ENGINE_LATTICE && engine != SNAPS_ENGINE_GRID) return 0;
+    return base_workspace_bytes(N, n_feat, n_masks, engine, flags) + select_eps_layout(N, n_masks, G, nq, nc, n_bins).total;
+}
+
+snaps_status snaps_range_select_eps(const float* d_X, int64_t N, int n_feat, int64_t ld, const uint16_t* h_masks,
+                                    int n_masks, const int32_t* h_sample_q, int nq, const int32_t* h_sample_c, int nc,
+                                    int n_bins, double s_min, double s_max, int G, int n_top, int flags,
+                                    float* out_eps_grid, int32_t* out_j_count, int32_t* out_j_mean, float* out_u,
+                                    void* d_workspace, size_t workspace_bytes, void* stream) {
+    prof_reset();
+    Engine E;
+    E.job = Job{d_X, N, n_feat, ld, h_masks, n_masks, 0, N, flags, resolve_engine(flags, N, 0)};
+    E.st = static_cast<cudaStream_t>(stream);
+    snaps_status rc = check_job(E.job, 0);
+    if (rc) return rc;
+    if (flags & SNAPS_FLAG_X_ON_HOST) return fail(SNAPS_UNSUPPORTED, "snaps_range_select_eps takes a device table");
+    if (G < 2 || G > snaps::kRangeGridMaxRadii) return fail(SNAPS_INVALID_ARG, "G = %d outside 2..%d", G, snaps::kRangeGridMaxRadii);
+    if (!(s_min > 0.0) || !(s_max > s_min)) return fail(SNAPS_INVALID_ARG, "need 0 < s_min < s_max");
+    if (n_top < 1 || n_top > N) return fail(SNAPS_INVALID_ARG, "n_top = %d outside 1..N", n_top);
+    if (!out_j_count || !out_j_mean) return fail(SNAPS_INVALID_ARG, "NULL outputs");
+    if ((N + 31) / 32 * 4 > 200 * 1024) return fail(SNAPS_UNSUPPORTED, "N too large for the top-n bitmap");
+    rc = carve(d_workspace, workspace_bytes, E.job, &E.w);
+    if (rc) return rc;
+    const SelectEpsLayout L = select_eps_layout(N, n_masks, G, nq, nc, n_bins);
+    if (E.w.extra_bytes < L.total) return fail(SNAPS_WORKSPACE_TOO_SMALL, "workspace lacks %zu bytes", L.total - E.w.extra_bytes);
+    unsigned char* p = E.w.extra;
+    void* search_ws = p; p += L.search;
+    float* eps_mean = reinterpret_cast<float*>(p);
+    float* eps_mm = eps_mean + n_masks; p += L.mm;
+    float* eps_grid = reinterpret_cast<float*>(p); p += L.grid;
+    float* thr = reinterpret_cast<float*>(p); p += L.thr;
+    uint32_t* count = reinterpret_cast<uint32_t*>(p); p += L.score;
+    float* sum = reinterpret_cast<float*>(p); p += L.score;
+    float* mean = reinterpret_cast<float*>(p); p += L.score;
+    int32_t* order = reinterpret_cast<int32_t*>(p); p += L.order;
+    float* u = out_u ? out_u : reinterpret_cast<float*>(p); p += L.u;
+    void* rws = p;
+    // 1. eps_min, eps_max for the two target selectivities (NEXT-2)
+    const double targets[2] = {s_min, s_max};
+    rc = snaps_eps_search(d_X, N, n_feat, ld, h_masks, n_masks, h_sample_q, nq, h_sample_c, nc, n_bins, targets, 2, eps_mean,
+                          eps_mm, nullptr, search_ws, L.search, stream);
+    if (rc) return rc;
+    // 2. the eps grid and its squared thresholds
+    CUDA_TRY(snaps::eps_grid_launch(eps_mm, n_masks, G, E.job.engine == SNAPS_ENGINE_LATTICE ? 1 : 0, eps_grid, thr, E.st));
+    if (out_eps_grid)
+        CUDA_TRY(cudaMemcpyAsync(out_eps_grid, eps_grid, sizeof(float) * static_cast<size_t>(n_masks) * G, cudaMemcpyDeviceToDevice, E.st));
+    // 3. one join at eps_max gives every eps_j
+    rc = engine_begin(&E);
+    if (rc) return rc;
+    rc = range_grid_run(&E, G, thr, RangeOut{count, sum, mean});
+    if (rc) return rc;
+    // 4. ranks, Eq. 2 against the smallest and the largest radius, Eq. 3 -- for both DSSJ metrics
+    const int rows = n_masks * G;
+    for (int metric = 0; metric < 2; ++metric) {
+        const int kind = metric == 0 ? SNAPS_METRIC_DSSJ_COUNT : SNAPS_METRIC_DSSJ_MEAN;
+        float* u_min = u + static_cast<size_t>(2 * metric) * rows;
+        float* u_max = u + static_cast<size_t>(2 * metric + 1) * rows;
+        CUDA_TRY(snaps::rank_launch(kind, metric == 0 ? static_cast<const void*>(count) : static_cast<const void*>(mean), count, N,
+                                    rows, nullptr, order, rws, L.rank, E.st));
+        for (int g = 0; g < G; ++g) {
+            CUDA_TRY(snaps::topn_overlap_strided_launch(order, order, N, n_masks, n_top, G, 0, G, g,
+                                                        u_min + static_cast<size_t>(g) * n_masks, E.st));
+            CUDA_TRY(snaps::topn_overlap_strided_launch(order, order, N, n_masks, n_top, G, G - 1, G, g,
+                                                        u_max + static_cast<size_t>(g) * n_masks, E.st));
+        }
+        CUDA_TRY(snaps::select_launch(u_min, u_max, G, n_masks, n_top, metric == 0 ? out_j_count : out_j_mean, E.st));
+    }
     return SNAPS_OK;
 }
 

@@ -125,6 +125,29 @@ __global__ void eps_from_hist_kernel(const unsigned long long* __restrict__ hist
     eps[i] = e;
 }
 
+// The eps grid G (Fig. 3 "evenly spaced search distances"): G radii from eps_min to eps_max in
+// fp32, eps_g = eps_min + g * ((eps_max - eps_min) / (G - 1)) with every operation rounded, the last one
+// eps_max itself; beside it the squared thresholds the join kernels compare with (closed ball, reading A2:
+// fl(eps^2) for the grid engine, its successor for the sub-lattice engine's strict compare).
+__global__ void eps_grid_kernel(const float* __restrict__ eps_mm, int n_masks, int G, int successor,
+                                float* __restrict__ eps_grid, float* __restrict__ thr) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_masks * G) return;
+    const int m = i / G, g = i - m * G;
+    const float e_min = eps_mm[2 * m], e_max = eps_mm[2 * m + 1];
+    const float step = __fdiv_rn(__fsub_rn(e_max, e_min), static_cast<float>(G - 1));
+    const float e = g == G - 1 ? e_max : __fadd_rn(e_min, __fmul_rn(static_cast<float>(g), step));
+    const float e2 = static_cast<float>(static_cast<double>(e) * static_cast<double>(e));
+    eps_grid[i] = e;
+    thr[i] = successor ? nextafterf(e2, __int_as_float(0x7f800000)) : e2;
+}
+
+cudaError_t eps_grid_launch(const float* eps_mm, int n_masks, int G, int successor, float* eps_grid, float* thr,
+                            cudaStream_t st) {
+    eps_grid_kernel<<<(n_masks * G + 127) / 128, 128, 0, st>>>(eps_mm, n_masks, G, successor, eps_grid, thr);
+    return cudaGetLastError();
+}
+
 size_t dist_hist_workspace_bytes(int nq, int nc, int n_masks) {
     auto al = [](size_t x) { return (x + 255) / 256 * 256; };
     return al(static_cast<size_t>(nq) * 64) + al(static_cast<size_t>(nc) * 64) + al(static_cast<size_t>(nq) * 4) +

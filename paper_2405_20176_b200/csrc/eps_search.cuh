@@ -19,4 +19,9 @@ cudaError_t eps_search_launch(const float* X, int64_t N, int64_t ld, int n_feat,
                               const double* h_targets, int n_targets, float* out_eps_mean, float* out_eps,
                               unsigned long long* out_hist, void* ws, cudaStream_t st);
 
+
+// G evenly spaced radii between eps_mm[m][0] and eps_mm[m][1] and their squared thresholds.
+cudaError_t eps_grid_launch(const float* eps_mm, int n_masks, int G, int successor, float* eps_grid, float* thr,
+                            cudaStream_t st);
+
 }  // namespace snaps

@@ -118,23 +118,27 @@ cudaError_t rank_launch(int metric, const void* values, const uint32_t* counts, 
 }
 
 // Eq. 2: one CTA per row pair; a bitmap of A's top-n in shared memory, B's top-n probes it.
+// Row r of the output compares row r * stride_a + off_a of order_a with row r * stride_b + off_b of order_b.
 __global__ void topn_overlap_kernel(const int32_t* __restrict__ order_a, const int32_t* __restrict__ order_b,
-                                    int64_t N, int n, float* __restrict__ out_f) {
+                                    int64_t N, int n, int stride_a, int off_a, int stride_b, int off_b,
+                                    float* __restrict__ out_f) {
     extern __shared__ uint32_t bits[];
     __shared__ int s_hits;
     const int64_t row = blockIdx.x;
+    order_a += (row * stride_a + off_a) * N;
+    order_b += (row * stride_b + off_b) * N;
     const int words = static_cast<int>((N + 31) / 32);
     for (int i = threadIdx.x; i < words; i += blockDim.x) bits[i] = 0u;
     if (threadIdx.x == 0) s_hits = 0;
     __syncthreads();
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
-        const int id = order_a[row * N + i];
+        const int id = order_a[i];
         atomicOr(&bits[id >> 5], 1u << (id & 31));
     }
     __syncthreads();
     int hits = 0;
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
-        const int id = order_b[row * N + i];
+        const int id = order_b[i];
         hits += (bits[id >> 5] >> (id & 31)) & 1u;
     }
     atomicAdd(&s_hits, hits);
@@ -142,14 +146,20 @@ __global__ void topn_overlap_kernel(const int32_t* __restrict__ order_a, const i
     if (threadIdx.x == 0) out_f[row] = static_cast<float>(s_hits) / static_cast<float>(n);
 }
 
-cudaError_t topn_overlap_launch(const int32_t* order_a, const int32_t* order_b, int64_t N, int n_rows, int n,
-                                float* out_f, cudaStream_t stream) {
+cudaError_t topn_overlap_strided_launch(const int32_t* order_a, const int32_t* order_b, int64_t N, int n_rows, int n,
+                                        int stride_a, int off_a, int stride_b, int off_b, float* out_f,
+                                        cudaStream_t stream) {
     const size_t smem = static_cast<size_t>((N + 31) / 32) * 4;
     cudaError_t e = cudaFuncSetAttribute(topn_overlap_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    topn_overlap_kernel<<<n_rows, 256, smem, stream>>>(order_a, order_b, N, n, out_f);
+    topn_overlap_kernel<<<n_rows, 256, smem, stream>>>(order_a, order_b, N, n, stride_a, off_a, stride_b, off_b, out_f);
     return cudaGetLastError();
+}
+
+cudaError_t topn_overlap_launch(const int32_t* order_a, const int32_t* order_b, int64_t N, int n_rows, int n,
+                                float* out_f, cudaStream_t stream) {
+    return topn_overlap_strided_launch(order_a, order_b, N, n_rows, n, 1, 0, 1, 0, out_f, stream);
 }
 
 // Eq. 3 per row: argmin_j |U_min[j] - U_max[j]| (first minimiser).  u_*: [G][n_rows].

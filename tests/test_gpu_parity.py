@@ -233,20 +233,28 @@ def _sampled_knn_check(snaps, oracle_mod, cfg, out, X, masks, n_masks_s, n_queri
 
 def test_config2_full_size_sampled(snaps, oracle_mod):
     """BASELINE.json configs[1] exactly as bench.py launches it (N=31,693, 32,752 masks, k=10,
-    scores only): sampled rows against the oracle, whole-output invariants, and the in-degree of
-    two complete masks against a full oracle join of those masks."""
+    scores only).  SURVEY 8(c) oracle tiers: ALL masks x 16 sampled queries (every one of the 512 batches
+    and every lattice slot), whole-output invariants, the in-degree of two complete masks against a full
+    oracle join, and ids + distances of eight whole batches (512 masks) x 256 sampled queries through the
+    streamed call."""
     import torch
     cfg = workloads.get_config("c2_snapshot1_knn")
     X, masks = cfg.table(), cfg.masks()
-    N = len(X)
-    out = snaps.knn_selfjoin(_dev(X), masks, cfg.k, lists=False)
+    N, k = len(X), cfg.k
+    Xd = _dev(X)
+    out = snaps.knn_selfjoin(Xd, masks, k, lists=False)
     torch.cuda.synchronize()
-    ms, qs = _sampled_knn_check(snaps, oracle_mod, cfg, out, X, masks, 28, 48, seed=5)
+    rng = np.random.default_rng(5)
+    qs = np.sort(rng.choice(N, 16, replace=False))
+    oi, od = oracle_mod.knn_selfjoin(X, masks, k, queries=qs)          # all 32,752 masks
+    kth = out["kth"][:, qs].cpu().numpy().astype(np.float64)
+    mean = out["mean"][:, qs].cpu().numpy().astype(np.float64)
+    assert (np.abs(kth - od[:, :, -1]) <= 1e-4 * od[:, :, -1] + 1e-7).all()
+    assert (np.abs(mean - od.mean(axis=2)) <= 1e-4 * od.mean(axis=2) + 1e-7).all()
     # invariants over the whole output (PAPER.md:136; mean <= kth; monotone along lattice edges)
-    assert bool((out["indeg"].sum(dim=1) == N * cfg.k).all())
+    assert bool((out["indeg"].sum(dim=1) == N * k).all())
     assert bool((out["mean"] <= out["kth"] * (1 + 1e-6)).all()) and bool((out["kth"] > 0).all())
     pos = {int(m): i for i, m in enumerate(masks)}
-    rng = np.random.default_rng(6)
     for m in rng.choice(masks, 40, replace=False):
         for f in range(15):
             sup = int(m) | (1 << f)
@@ -254,37 +262,42 @@ def test_config2_full_size_sampled(snaps, oracle_mod):
                 a, b = out["kth"][pos[int(m)]], out["kth"][pos[sup]]
                 assert bool((a <= b * (1 + 1e-5) + 1e-7).all())      # D_(k)(S) <= D_(k)(S u {f})
     # in-degree: two complete masks, full oracle join
-    for mi in (ms[0], ms[-1]):
-        oi, od = oracle_mod.knn_selfjoin(X, masks[mi:mi + 1], cfg.k + 1)
-        unamb = (od[0, :, cfg.k] - od[0, :, cfg.k - 1]) > 1e-5 * od[0, :, cfg.k]
-        hist = np.bincount(oi[0, :, :cfg.k].ravel(), minlength=N)
+    for mi in (int(rng.integers(len(masks))), len(masks) - 1):
+        oi1, od1 = oracle_mod.knn_selfjoin(X, masks[mi:mi + 1], k + 1)
+        unamb = (od1[0, :, k] - od1[0, :, k - 1]) > 1e-5 * od1[0, :, k]
+        hist = np.bincount(oi1[0, :, :k].ravel(), minlength=N)
         got = out["indeg"][mi].cpu().numpy()
         if unamb.all():
             assert (got == hist).all()
         else:   # only ambiguous queries' k-th neighbours may differ
             assert np.abs(got - hist).sum() <= 2 * (~unamb).sum()
+    del out
+    # ids + distances: eight whole batches (all 64 lattice slots of eight sets H), streamed in groups of 100 masks
+    hs = rng.choice(np.unique(masks.astype(np.int64) >> 6), 8, replace=False)
+    sel = np.flatnonzero(np.isin(masks.astype(np.int64) >> 6, hs))
+    assert 8 * 57 <= len(sel) <= 8 * 64
+    st = snaps.knn_selfjoin_streamed(Xd, masks[sel], k, masks_per_batch=100, lists=True)
+    torch.cuda.synchronize()
+    qs2 = np.sort(rng.choice(N, 256, replace=False))
+    oi2, od2 = oracle_mod.knn_selfjoin(X, masks[sel], k + 1, queries=qs2)
+    check_knn(st["idx"][:, qs2].numpy(), st["dist"][:, qs2].numpy(), oi2, od2, queries=qs2)
 
 
 def test_config3_full_size_sampled(snaps, oracle_mod):
-    """BASELINE.json configs[2]: DSSJ over all 32,752 masks at N=31,693 with per-dimension eps_d for
-    ~50 neighbours (calibrated by the oracle on a 1,000-point sample); sampled rows + invariants."""
+    """BASELINE.json configs[2] as bench.py launches it: DSSJ over all 32,752 masks at N=31,693 with the
+    stored per-dimension eps_d (~50 neighbours; workloads/config_eps.json); ALL masks x 16 sampled queries
+    against the oracle, plus invariants."""
     import torch
-    from oracle.calibrate import eps_per_dimension
     cfg = workloads.get_config("c3_snapshot1_dssj")
     X, masks = cfg.table(), cfg.masks()
     N = len(X)
-    eps = eps_per_dimension(X, masks, cfg.target_neighbours, seed=cfg.seed, max_masks_per_dim=4,
-                            n_query_sample=300).astype(np.float32)
+    eps = workloads.config_eps(cfg.name, masks)
     out = snaps.range_selfjoin(_dev(X), masks, eps)
     torch.cuda.synchronize()
     rng = np.random.default_rng(7)
-    pc = workloads.popcount(masks)
-    ms = np.sort(np.concatenate([rng.choice(np.flatnonzero(pc == d), min(2, int((pc == d).sum())), replace=False)
-                                 for d in np.unique(pc)]))
-    qs = np.sort(rng.choice(N, 48, replace=False))
-    cnt = out["count"][ms][:, qs].cpu().numpy()
-    check_range(cnt, out["sumdist"][ms][:, qs].cpu().numpy(), out["mean"][ms][:, qs].cpu().numpy(),
-                oracle_mod, X, masks[ms], eps[ms], queries=qs)
+    qs = np.sort(rng.choice(N, 16, replace=False))
+    check_range(out["count"][:, qs].cpu().numpy(), out["sumdist"][:, qs].cpu().numpy(), out["mean"][:, qs].cpu().numpy(),
+                oracle_mod, X, masks, eps, queries=qs)
     mean_cnt = out["count"].float().mean().item()
     assert 10 < mean_cnt < 250, mean_cnt                     # calibrated for ~50 (sample noise allowed)
     # no self-pairs, counts bounded by N-1; the mean is 0 exactly where the count is 0 (A6)
@@ -394,7 +407,7 @@ def test_query_range_slices_concatenate(snaps, oracle_mod):
 def test_config4_full_size_sampled(snaps, oracle_mod):
     """BASELINE.json configs[3] at full size: N=1,000,000 x 15 (seed 3, 0.1% outliers), the 105
     two-feature subspaces plus the full space, k=10, lists and scores batched through pinned host
-    memory.  The library takes the pivot sweep at this N.  Sampled rows against the oracle."""
+    memory.  The library takes the grid engine at this N.  All masks x 64 sampled queries against the oracle."""
     import torch
     cfg = workloads.get_config("c4_lsst_pairs")
     X, masks, k = cfg.table(), cfg.masks(), cfg.k
@@ -402,8 +415,8 @@ def test_config4_full_size_sampled(snaps, oracle_mod):
     st = snaps.knn_selfjoin_streamed(_dev(X), masks, k, masks_per_batch=16, lists=True)
     torch.cuda.synchronize()
     rng = np.random.default_rng(9)
-    qs = np.sort(rng.choice(n, 24, replace=False))
-    sel = np.concatenate([np.arange(0, len(masks), 7), [len(masks) - 1]])
+    qs = np.sort(rng.choice(n, 64, replace=False))
+    sel = np.arange(len(masks))                                  # all 106 masks
     oi, od = oracle_mod.knn_selfjoin(X, masks[sel], k + 1, queries=qs)
     check_knn(st["idx"][sel][:, qs].numpy(), st["dist"][sel][:, qs].numpy(), oi, od, queries=qs)
     kth = st["kth"][sel][:, qs].numpy().astype(np.float64)
@@ -444,26 +457,76 @@ def test_eps_grid_by_repeating_masks(snaps, oracle_mod):
     assert (np.diff(c, axis=1) >= 0).all() and (c[:, -1] > c[:, 0]).any()
 
 
-def test_config5_scale_low_dimensional_masks(snaps, oracle_mod):
-    """BASELINE.json configs[4]'s N and k (N=5,000,000 x 15, seed 4, k=16; DSSJ beside it) on six
-    two- and three-feature masks, which the pivot sweep prunes; c5's own 256 random masks average 7.5
-    features and are out of reach at this N.  Sampled rows against the oracle."""
+def test_config5_real_mask_list(snaps, oracle_mod):
+    """BASELINE.json configs[4]'s own mask list (256 masks sampled from the 32,752, seed 4; 2-12 features),
+    k=16 kNNSJ + DSSJ (~100 neighbours), outputs through the recycling sink (two pinned host buffers), at
+    N=1,000,000 (the full N=5,000,000 pass takes minutes: `python bench.py --config c5_lsst_oversub`).
+    Sampled (mask, query) rows of EVERY mask against the oracle; in-degree sums over every mask."""
     import torch
-    n, k = 5_000_000, 16
-    X = workloads.make_table(n, 4, outlier_frac=0.001)
-    masks = np.array([(1 << 6) | (1 << 9), (1 << 7) | (1 << 14), (1 << 0) | (1 << 3), (1 << 2) | (1 << 11),
-                      (1 << 4) | (1 << 5), (1 << 8) | (1 << 13) | (1 << 1)], dtype=np.uint16)
+    cfg = workloads.get_config("c5_lsst_oversub")
+    n, k = 1_000_000, cfg.k
+    X = workloads.make_table(n, cfg.seed, outlier_frac=0.001)
+    masks = cfg.masks()
+    assert len(masks) == 256 and workloads.popcount(masks).max() >= 10
     Xd = _dev(X)
-    out = snaps.knn_selfjoin(Xd, masks, k)
-    torch.cuda.synchronize()
     rng = np.random.default_rng(3)
-    qs = np.sort(rng.choice(n, 12, replace=False))
+    qs = np.sort(rng.choice(n, 8, replace=False))
+    got = {"idx": np.empty((256, 8, k), np.int32), "dist": np.empty((256, 8, k), np.float32),
+           "kth": np.empty((256, 8), np.float32), "indeg_sum": np.zeros(256, np.int64), "groups": 0}
+
+    def consume(m0, m1, a):
+        got["idx"][m0:m1] = a["idx"][:, qs]
+        got["dist"][m0:m1] = a["dist"][:, qs]
+        got["kth"][m0:m1] = a["kth"][:, qs]
+        got["indeg_sum"][m0:m1] = a["indeg"].sum(axis=1, dtype=np.int64)
+        got["groups"] += 1
+
+    ws = snaps.knn_selfjoin_sink(Xd, masks, k, 6, consume, want=("idx", "dist", "kth", "indeg"))
+    assert got["groups"] == (256 + 5) // 6
     oi, od = oracle_mod.knn_selfjoin(X, masks, k + 1, queries=qs)
-    check_knn(out["idx"][:, qs].cpu().numpy(), out["dist"][:, qs].cpu().numpy(), oi, od, queries=qs)
-    assert bool((out["indeg"].sum(dim=1) == n * k).all())
-    eps = (np.median(od[:, :, -1], axis=1) * 1.5).astype(np.float32)
-    del out
-    r = snaps.range_selfjoin(Xd, masks, eps)
-    torch.cuda.synchronize()
-    check_range(r["count"][:, qs].cpu().numpy(), r["sumdist"][:, qs].cpu().numpy(), r["mean"][:, qs].cpu().numpy(),
-                oracle_mod, X, masks, eps, queries=qs)
+    check_knn(got["idx"], got["dist"], oi, od, queries=qs)
+    assert (np.abs(got["kth"] - od[:, :, k - 1]) <= 1e-4 * od[:, :, k - 1] + 1e-7).all()
+    assert (got["indeg_sum"] == n * k).all()                        # PAPER.md:136, every mask
+    # DSSJ: radii from the library's own search (NEXT-2) for ~100 neighbours, then the join through the sink
+    eps = snaps.eps_for_selectivity(Xd, masks, cfg.target_neighbours, seed=cfg.seed)
+    r = {"count": np.empty((256, 8), np.uint32), "sumdist": np.empty((256, 8), np.float32),
+         "mean": np.empty((256, 8), np.float32), "total": 0}
+
+    def consume_r(m0, m1, a):
+        r["count"][m0:m1] = a["count"][:, qs]
+        r["sumdist"][m0:m1] = a["sumdist"][:, qs]
+        r["mean"][m0:m1] = a["eps_mean"][:, qs]
+        r["total"] += int(a["count"].sum(dtype=np.int64))
+
+    snaps.range_selfjoin_sink(Xd, masks, eps, 6, consume_r, workspace=ws)
+    check_range(r["count"], r["sumdist"], r["mean"], oracle_mod, X, masks, eps, queries=qs)
+    assert 30 < r["total"] / (256.0 * n) < 300                      # the search aimed at ~100 neighbours
+
+
+def test_sink_matches_resident(snaps, oracle_mod):
+    # the recycling sink hands out exactly what the resident call writes, group by group, both engines
+    import torch
+    X = workloads.make_table(1500, 37, cols=list(range(11)))
+    masks = workloads.all_masks(11)[::13]
+    Xd = _dev(X)
+    for engine in ("lattice", "grid"):
+        ref = snaps.knn_selfjoin(Xd, masks, 9, engine=engine)
+        rr = snaps.range_selfjoin(Xd, masks, np.full(len(masks), 0.15, np.float32), engine=engine)
+        torch.cuda.synchronize()
+        seen = []
+
+        def consume(m0, m1, a):
+            seen.append((m0, m1))
+            for n in ("idx", "dist", "kth", "mean", "indeg"):
+                assert (a[n] == ref[n][m0:m1].cpu().numpy()).all(), (engine, n)
+
+        snaps.knn_selfjoin_sink(Xd, masks, 9, 7, consume, want=("idx", "dist", "kth", "mean", "indeg"), n_buffers=3,
+                                engine=engine)
+        assert seen == [(m, min(m + 7, len(masks))) for m in range(0, len(masks), 7)]
+
+        def consume_r(m0, m1, a):
+            assert (a["count"] == rr["count"][m0:m1].cpu().numpy().view(np.uint32)).all()
+            assert (a["sumdist"] == rr["sumdist"][m0:m1].cpu().numpy()).all()
+            assert (a["eps_mean"] == rr["mean"][m0:m1].cpu().numpy()).all()
+
+        snaps.range_selfjoin_sink(Xd, masks, np.full(len(masks), 0.15, np.float32), 5, consume_r, engine=engine)

@@ -149,29 +149,34 @@ def test_radius_grid_single_scan_matches_oracle_per_radius(snaps):
 
 def test_select_k_pipeline_matches_oracle(snaps):
     """snaps_knn_select_k (one call: k grid -> scores -> ranks -> Eq. 2 -> Eq. 3) against the oracle
-    procedure on the same k_max lists, mask by mask."""
+    procedure, mask by mask, on the SAME k_max lists: the oracle's own join, cast to the fp32 lists the
+    device call takes.  Index work: U curves and selected grid points are compared exactly; the ranks by
+    mean distance are decided on the fp32 mean on both sides (reading A21)."""
     import torch
+    import oracle as oracle_mod
     N, k_max, n = 2500, 32, 25
     X = workloads.make_table(N, 31, outlier_frac=0.01)
     masks = workloads.all_masks(15)[::1409]
-    join = snaps.knn_selfjoin(_t(X), masks, k_max, scores=False)
+    oi, od = oracle_mod.knn_selfjoin(X, masks, k_max)
+    idx, dist = oi.astype(np.int32), od.astype(np.float32)
     grid = [2, 3, 4, 6, 8, 11, 16, 23, 32]
-    out = snaps.knn_select_k(join["idx"], join["dist"], grid, n)
+    out = snaps.knn_select_k(_t(idx), _t(dist), grid, n)
     torch.cuda.synchronize()
-    idx, dist = join["idx"].cpu().numpy(), join["dist"].cpu().numpy()
     u = out["u"].cpu().numpy()
     for m in range(len(masks)):
         ref = oracle_ranking.select_k(idx[m], dist[m], grid, n, N)
-        # the device means are fp32 sums: ranks by mean distance can differ from the fp64 oracle only
-        # through near-ties, which move a top-n membership by at most a few objects
         ji, umin_i, umax_i = ref["knn_indegree"]
         assert np.array_equal(u[0][:, m], umin_i.astype(np.float32)) and np.array_equal(u[1][:, m], umax_i.astype(np.float32))
         assert int(out["j_indeg"][m]) == ji
         jm, umin_m, umax_m = ref["knn_mean"]
-        assert np.abs(u[2][:, m] - umin_m).max() <= 2.0 / n and np.abs(u[3][:, m] - umax_m).max() <= 2.0 / n
-        dev_j = int(out["j_mean"][m])
-        assert dev_j == oracle_ranking.select_parameter(u[2][:, m], u[3][:, m], n)   # Eq. 3 on the device's own curves
+        assert np.array_equal(u[2][:, m], umin_m.astype(np.float32)) and np.array_equal(u[3][:, m], umax_m.astype(np.float32))
+        assert int(out["j_mean"][m]) == jm
     assert (u[0][0] == 1.0).all() and (u[1][-1] == 1.0).all() and (u[2][0] == 1.0).all() and (u[3][-1] == 1.0).all()
+    # the same call on the device's own lists runs end to end (join -> selection without leaving the GPU)
+    join = snaps.knn_selfjoin(_t(X), masks, k_max, scores=False)
+    out2 = snaps.knn_select_k(join["idx"], join["dist"], grid, n)
+    torch.cuda.synchronize()
+    assert (out2["j_indeg"].cpu().numpy() == out["j_indeg"].cpu().numpy()).mean() > 0.9
     with pytest.raises(snaps.SnapsError):
         snaps.knn_select_k(join["idx"], join["dist"], [4, 2, 8], n)
 
@@ -210,3 +215,92 @@ def test_sampled_distance_histogram_and_eps_search(snaps):
     # the radius does what it is for: the eps-join at it finds about the target number of neighbours
     cnt = snaps.range_selfjoin(_t(X), masks, e_dev)["count"].float().mean(dim=1).cpu().numpy()
     assert (cnt > 10).all() and (cnt < 40).all()
+
+
+def test_eps_search_matches_oracle(snaps):
+    """snaps_eps_search (PAPER.md:229-237 in one device call: eps_mean, histogram over [0, eps_mean), radii
+    for two target selectivities) against oracle.calibrate.eps_search, step by step."""
+    import torch
+    from oracle.calibrate import eps_search
+    N = 3000
+    X = workloads.make_table(N, 41, outlier_frac=0.01)
+    masks = np.array([0b11, 0x7FFF, (1 << 9) | (1 << 3) | 1, 0b1111000, (1 << 13) | (1 << 12)], dtype=np.uint16)
+    rng = np.random.default_rng(9)
+    q = np.sort(rng.choice(N, 200, replace=False)).astype(np.int32)
+    c = np.sort(rng.choice(N, 1200, replace=False)).astype(np.int32)
+    n_bins, targets = 512, [3.0, 450.0]          # s_min ~ 0.001 |D|, s_max ~ 0.15 |D| (PAPER.md:229)
+    out = snaps.eps_search(_t(X), masks, q, c, targets, n_bins, hist=True)
+    torch.cuda.synchronize()
+    rmax, eps, hist, dists = eps_search(X, masks, q, c, n_bins, targets)
+    g_mean = out["eps_mean"].cpu().numpy()
+    assert np.abs(g_mean - rmax).max() <= 2e-6 * rmax.max()                   # fp32 value of an fp64-accumulated mean
+    g_hist = out["hist"].cpu().numpy()
+    for mi in range(len(masks)):
+        edges = np.arange(1, n_bins + 1) * (float(rmax[mi]) / n_bins)
+        lo = np.array([(dists[mi] < e * (1 - 2e-6)).sum() for e in edges])
+        hi = np.array([(dists[mi] < e * (1 + 2e-6)).sum() for e in edges])
+        cum = np.cumsum(g_hist[mi])
+        assert (lo <= cum).all() and (cum <= hi).all()
+    g_eps = out["eps"].cpu().numpy()
+    assert np.abs(g_eps - eps).max() <= (rmax / n_bins).max() * 1.001          # at most one bin apart
+    assert (np.abs(g_eps - eps) <= 1e-6 * eps).mean() >= 0.8                   # and mostly the same edge
+    assert (g_eps[:, 0] < g_eps[:, 1]).all() and (g_eps[:, 1] <= g_mean * 1.000001).all()
+    # the radii do what they are for
+    for t, col in zip(targets, (0, 1)):
+        cnt = snaps.range_selfjoin(_t(X), masks, g_eps[:, col], sums=False)["count"].float().mean(dim=1).cpu().numpy()
+        assert (cnt > 0.5 * t).all() and (cnt < 2.0 * t).all(), (t, cnt)
+
+
+@pytest.mark.parametrize("engine", ["lattice", "grid"])
+def test_select_eps_pipeline_matches_oracle(snaps, engine):
+    """snaps_range_select_eps (one call: eps_min / eps_max search -> eps grid -> one join at eps_max -> ranks
+    -> Eq. 2 -> Eq. 3) against the oracle procedure written out step by step (calibrate.eps_search,
+    ranking.eps_grid, one range join per radius, ranking.select_eps), mask by mask.  Index work is compared
+    exactly wherever no pair sits within 1e-6 of a grid radius (reading A2) and, for the mean-distance
+    metric, no object sits within 1e-5 relative of the top-n boundary (near-tie rule: the device mean is an
+    fp32 sum in scan order)."""
+    import torch
+    import oracle as oracle_mod
+    from oracle.calibrate import eps_search
+    N, G, n = 1800, 8, 18
+    X = workloads.make_table(N, 43, outlier_frac=0.01)
+    masks = np.array([0b11, 0x7FFF, (1 << 9) | (1 << 3) | 1, 0b1111000, (1 << 13) | (1 << 12), 0b111111], dtype=np.uint16)
+    rng = np.random.default_rng(11)
+    q = np.sort(rng.choice(N, 300, replace=False)).astype(np.int32)
+    c = np.arange(N, dtype=np.int32)
+    s_min, s_max, n_bins = 0.002 * N, 0.15 * N, 1024
+    out = snaps.range_select_eps(_t(X), masks, q, c, s_min, s_max, G, n, n_bins, engine=engine)
+    torch.cuda.synchronize()
+    _, eps, _, _ = eps_search(X, masks, q, c, n_bins, [s_min, s_max])
+    u = out["u"].cpu().numpy()
+    g_grid = out["eps_grid"].cpu().numpy()
+    exact_masks = 0
+    for m in range(len(masks)):
+        grid = oracle_ranking.eps_grid(eps[m, 0], eps[m, 1], G)
+        assert np.abs(g_grid[m] - grid).max() <= 2e-6 * grid.max()
+        one = np.array([masks[m]] * G, dtype=np.uint16)
+        cnt, _, mean = oracle_mod.range_selfjoin(X, one, grid.astype(np.float64))
+        # the device's radii may sit an fp32 rounding or two from the oracle's (asserted above): widen the band of A2
+        lo, _, _ = oracle_mod.range_selfjoin(X, one, grid.astype(np.float64) * (1 - 4e-6))
+        hi, _, _ = oracle_mod.range_selfjoin(X, one, grid.astype(np.float64) * (1 + 4e-6))
+        ref = oracle_ranking.select_eps(cnt, mean, n)
+        jc, umin_c, umax_c = ref["dssj_count"]
+        if (lo == hi).all():
+            exact_masks += 1
+            assert np.array_equal(u[0][:, m], umin_c.astype(np.float32)) and np.array_equal(u[1][:, m], umax_c.astype(np.float32))
+            assert int(out["j_count"][m]) == jc
+            # mean-distance metric: exact unless an object sits on the top-n boundary of some radius
+            near = 0
+            for g in range(G):
+                key = np.where(cnt[g] == 0, np.inf, mean[g])           # most outlying first = descending
+                srt = np.sort(key)[::-1]
+                b = srt[n - 1]
+                near += int((np.abs(key - b) <= 1e-5 * max(b, 1e-30)).sum() - 1) if np.isfinite(b) else 0
+            jm, umin_m, umax_m = ref["dssj_mean"]
+            if near == 0:
+                assert np.array_equal(u[2][:, m], umin_m.astype(np.float32)) and np.array_equal(u[3][:, m], umax_m.astype(np.float32))
+                assert int(out["j_mean"][m]) == jm
+            else:
+                assert np.abs(u[2][:, m] - umin_m).max() <= near / n and np.abs(u[3][:, m] - umax_m).max() <= near / n
+    assert exact_masks >= len(masks) - 1
+    assert (u[0][0] == 1.0).all() and (u[1][-1] == 1.0).all() and (u[2][0] == 1.0).all() and (u[3][-1] == 1.0).all()

@@ -65,3 +65,48 @@ def test_shard_masks_single_process_properties():
         parts = [shard_masks(masks, r, world) for r in range(world)]
         cat = np.sort(np.concatenate(parts))
         assert (cat == np.arange(len(masks))).all()
+
+
+def _query_worker(rank, world, port, out_dir):
+    """SURVEY 8(e)(ii) on CPU: each rank owns the query slice `shard_queries` gives it; lists concatenate in
+    rank order and the per-rank in-degree rows (histograms over the rank's own queries) add up to the
+    full in-degree under one all-reduce -- the only exchange of query-range sharding.  The per-rank join
+    is played by the oracle (the CUDA kernels need a GPU; their slice outputs are checked against the full
+    join in tests/test_gpu_parity.py::test_query_range_slices_concatenate)."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import oracle
+    from paper_2405_20176_b200.sharding import shard_queries, shard_masks_by_cost
+    n, k = 601, 5
+    X = workloads.make_table(n, 21, cols=list(range(6)))
+    masks = workloads.all_masks(6)[::5]
+    q0, q1 = shard_queries(n, rank, world)
+    idx, dist_ = oracle.knn_selfjoin(X, masks, k, queries=np.arange(q0, q1))
+    indeg = np.stack([np.bincount(idx[m].ravel(), minlength=n) for m in range(len(masks))]).astype(np.int32)
+    t = torch.from_numpy(indeg)
+    dist.all_reduce(t)                                              # the in-degree sum over ranks
+    sizes = [torch.zeros(1, dtype=torch.int64) for _ in range(world)]
+    dist.all_gather(sizes, torch.tensor([q1 - q0], dtype=torch.int64))
+    pad = int(max(s.item() for s in sizes))
+    buf = torch.full((len(masks), pad, k), -1, dtype=torch.int32)
+    buf[:, :q1 - q0] = torch.from_numpy(idx)
+    parts = [torch.zeros_like(buf) for _ in range(world)]
+    dist.all_gather(parts, buf)
+    cat = torch.cat([p[:, :int(s.item())] for p, s in zip(parts, sizes)], dim=1).numpy()
+    full_idx, full_dist = oracle.knn_selfjoin(X, masks, k)
+    _, _, full_indeg = oracle.knn_scores(n, full_idx, full_dist)
+    assert (cat == full_idx).all()                                  # slices concatenate in rank order
+    assert (t.numpy() == full_indeg).all()                          # in-degree rows add up
+    # slices are a disjoint cover; cost-balanced mask dealing is one too
+    assert sum(int(s.item()) for s in sizes) == n
+    m_all = np.sort(np.concatenate([shard_masks_by_cost(masks, r, world) for r in range(world)]))
+    assert (m_all == np.arange(len(masks))).all()
+    dist.barrier()
+    dist.destroy_process_group()
+    open(os.path.join(out_dir, f"q_ok{rank}"), "w").write("ok")
+
+
+def test_query_range_sharding_world2_gloo(tmp_path):
+    world = 2
+    mp.spawn(_query_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    assert all((tmp_path / f"q_ok{r}").exists() for r in range(world))

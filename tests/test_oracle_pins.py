@@ -316,3 +316,40 @@ def test_sampled_histogram_closed_form_and_selectivity(oracle_mod):
     eps = eps_from_histogram(hist, [n * h], n, n * (n - 1), 6.0)
     mean_at = lambda r: oracle_mod.range_selfjoin(X, [0b001], [r])[0].mean()
     assert mean_at(eps[0] * (1 - 1e-9)) >= 6.0 > mean_at((eps[0] - h) * (1 - 1e-9))
+
+
+def test_eps_search_lattice_closed_forms(oracle_mod):
+    """eps_mean and the radii of oracle.calibrate.eps_search on the 1-D lattice with every object sampled:
+    the mean of |i - j| h over i != j is (n + 1) h / 3; the radius for a target of s neighbours is the
+    first bin edge whose ball holds them."""
+    from oracle.calibrate import eps_search, mean_sample_distance
+    n, h = 48, 2.0 ** -8
+    X = workloads.lattice_table(n, 3, h, seed=4)
+    ids = np.arange(n)
+    em, pairs = mean_sample_distance(X, [0b001], ids, ids)
+    assert pairs == n * (n - 1) and abs(em[0] - (n + 1) * h / 3) < 1e-15
+    # a two-feature mask with a duplicated column scales every distance by sqrt(2)
+    X2 = X.copy()
+    X2[:, 1] = X2[:, 0]
+    em2, _ = mean_sample_distance(X2, [0b011], ids, ids)
+    assert abs(em2[0] / em[0] - np.sqrt(2.0)) < 1e-12
+    rmax, eps, hist, _ = eps_search(X, [0b001], ids, ids, 256, [2.0, 6.0])
+    assert rmax[0] == np.float32((n + 1) * h / 3) and hist[0].sum() <= pairs
+    mean_at = lambda r: oracle_mod.range_selfjoin(X, [0b001], [r])[0].mean()
+    w = float(rmax[0]) / 256
+    for t, e in zip((2.0, 6.0), eps[0]):
+        assert mean_at(float(e) * (1 - 1e-9)) >= t > mean_at((float(e) - w) * (1 - 1e-9))
+
+
+def test_eps_grid_matches_figure_2(oracle_mod):
+    """the example feature space of Fig. 2 has eps_min = 0.0360, eps_max = 0.1707 and its
+    selected radius eps = 0.1256 is grid point arg = 15 (counted from 1).  With evenly spaced radii that
+    fixes |G| = 22 (step 0.0064); the oracle's grid must put its 15th point there, up to the rounding of
+    the published four-digit values.  (A division by |G| instead of |G| - 1, or an index off by one, misses
+    by more than ten times that.)"""
+    from oracle.ranking import eps_grid
+    g = eps_grid(0.0360, 0.1707, 22)
+    assert g[0] == np.float32(0.0360) and g[-1] == np.float32(0.1707) and len(g) == 22
+    assert abs(float(g[14]) - 0.1256) < 3.5e-4
+    assert abs(float(g[15]) - 0.1256) > 3e-3 and abs(float(g[13]) - 0.1256) > 3e-3
+    assert np.allclose(np.diff(g.astype(np.float64)), (0.1707 - 0.0360) / 21, rtol=1e-5)
