@@ -231,13 +231,15 @@ __device__ __noinline__ void knn_emit(float* ws, const KnnParams& p, int q, int 
             const int id = L_ID(NE - k + e, L);
             sum += d;
             dk = d;
-            if (p.out_idx) p.out_idx[o * k + e] = id;
-            if (p.out_dist) p.out_dist[o * k + e] = d;
+            // streaming stores: the outputs are written once and must not push the in-degree rows of the
+            // batches in flight (L2-resident atomics) out of the L2
+            if (p.out_idx) __stcs(&p.out_idx[o * k + e], id);
+            if (p.out_dist) __stcs(&p.out_dist[o * k + e], d);
             if (p.out_indeg)
                 atomicAdd(&p.out_indeg[static_cast<size_t>(sl) * static_cast<size_t>(p.N) + id], 1);
         }
-        if (p.out_kth) p.out_kth[o] = dk;
-        if (p.out_mean) p.out_mean[o] = sum / static_cast<float>(k);
+        if (p.out_kth) __stcs(&p.out_kth[o], dk);
+        if (p.out_mean) __stcs(&p.out_mean[o], sum / static_cast<float>(k));
     }
     __syncwarp();
 }

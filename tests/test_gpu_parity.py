@@ -530,3 +530,53 @@ def test_sink_matches_resident(snaps, oracle_mod):
             assert (a["eps_mean"] == rr["mean"][m0:m1].cpu().numpy()).all()
 
         snaps.range_selfjoin_sink(Xd, masks, np.full(len(masks), 0.15, np.float32), 5, consume_r, engine=engine)
+
+
+# ---------------------------------------------------------------- NEXT-3: the paper's operating points
+@pytest.mark.parametrize("k", [64, 256])
+def test_paper_operating_point_large_k(snaps, oracle_mod, k):
+    """PAPER.md:440 (LSST5M: k_max = 256) on the SNAPShot1-shaped table: N = 31,693, 64 masks stratified over
+    d = 2..15, k = 64 and 256 (the grid engine; the sub-lattice engine stops at 32).  Sampled queries of every
+    mask against the oracle, in-degree sums over the whole output."""
+    import torch
+    cfg = workloads.get_config("c2_snapshot1_knn")
+    X, allm = cfg.table(), cfg.masks()
+    N = len(X)
+    rng = np.random.default_rng(k)
+    pc = workloads.popcount(allm)
+    masks = allm[np.sort(np.concatenate([rng.choice(np.flatnonzero(pc == d), min(5, int((pc == d).sum())), replace=False)
+                                         for d in range(2, 16)]))][:64]
+    out = snaps.knn_selfjoin(_dev(X), masks, k)
+    torch.cuda.synchronize()
+    qs = np.sort(rng.choice(N, 12, replace=False))
+    oi, od = oracle_mod.knn_selfjoin(X, masks, k + 1, queries=qs)
+    check_knn(out["idx"][:, qs].cpu().numpy(), out["dist"][:, qs].cpu().numpy(), oi, od, queries=qs)
+    kth = out["kth"][:, qs].cpu().numpy().astype(np.float64)
+    assert (np.abs(kth - od[:, :, k - 1]) <= 1e-4 * od[:, :, k - 1] + 1e-7).all()
+    assert bool((out["indeg"].sum(dim=1) == N * k).all())
+
+
+def test_paper_operating_point_large_selectivity(snaps, oracle_mod):
+    """PAPER.md:229 (s_min ~ 0.001 |D|, s_max ~ 0.15 |D| ~ 4,754 neighbours on SNAPShot1): the radius grid from
+    eps_min to eps_max in ONE scan through the grid engine at N = 31,693; radii from the
+    library's own search; sampled queries of every radius against the oracle evaluated once per radius."""
+    import torch
+    cfg = workloads.get_config("c3_snapshot1_dssj")
+    X = cfg.table()
+    N = len(X)
+    masks = np.array([0b11, (1 << 9) | (1 << 3) | 1, 0b1111000, 0x7FFF, (1 << 14) | (1 << 7) | (1 << 6) | (1 << 2)], dtype=np.uint16)
+    rng = np.random.default_rng(17)
+    q = np.sort(rng.choice(N, 400, replace=False))
+    c = np.sort(rng.choice(N, 8000, replace=False))
+    es = snaps.eps_search(_dev(X), masks, q, c, [0.001 * N, 0.15 * N], 2048)["eps"].cpu().numpy()
+    G = 6
+    grid = np.stack([np.linspace(es[m, 0], es[m, 1], G, dtype=np.float32) for m in range(len(masks))])
+    out = snaps.range_selfjoin_grid(_dev(X), masks, grid, engine="grid")
+    torch.cuda.synchronize()
+    qs = np.sort(rng.choice(N, 10, replace=False))
+    for g in range(G):
+        check_range(out["count"][:, g][:, qs].cpu().numpy(), out["sumdist"][:, g][:, qs].cpu().numpy(),
+                    out["mean"][:, g][:, qs].cpu().numpy(), oracle_mod, X, masks, grid[:, g], queries=qs)
+    mean_cnt = out["count"].float().mean(dim=2).cpu().numpy()
+    assert (mean_cnt[:, 0] > 0.0003 * N).all() and (mean_cnt[:, 0] < 0.004 * N).all()      # ~0.001 |D|
+    assert (mean_cnt[:, -1] > 0.08 * N).all() and (mean_cnt[:, -1] < 0.3 * N).all()         # ~0.15 |D|
