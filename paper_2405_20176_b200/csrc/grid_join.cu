@@ -30,7 +30,6 @@ constexpr int kWarps = 8;            // warps per CTA at most (independent; fewe
 constexpr int kTile = 64;            // candidates per tile
 constexpr int kSeedHalf = 112;       // seed window: this many sorted positions either side of the warp
 constexpr int kMaxG = 32;
-constexpr int kPend = 8;             // kNN: candidates a lane may hold back before the warp merges them into the heaps
 
 constexpr int MODE_KNN = 0, MODE_RANGE = 1, MODE_RANGE_GRID = 2;
 
@@ -38,7 +37,7 @@ __host__ __device__ constexpr int dp_of(int d) { return (d + 3) / 4 * 4; }
 
 // per-warp shared-memory floats
 __host__ __device__ constexpr int warp_words(int d, int mode, int k, int G) {
-    return kTile * dp_of(d) + (mode == MODE_KNN ? 64 * k + 64 * kPend : 0) + (mode == MODE_RANGE_GRID ? 64 * G + 32 : 0);
+    return kTile * dp_of(d) + (mode == MODE_KNN ? 64 * k : 0) + (mode == MODE_RANGE_GRID ? 64 * G + 32 : 0);
 }
 
 struct Heap {
@@ -114,10 +113,6 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
     hp.i = reinterpret_cast<int*>(hp.d + 32 * k);
     hp.k = k;
     hp.lane = lane;
-    // kNN: per-lane buffer of candidates that passed the threshold test and wait for the merge
-    float* pend_d = wsm + kTile * DP + 64 * k;
-    int* pend_p = reinterpret_cast<int*>(pend_d + 32 * kPend);
-    int npend = 0;
     // radius grid: per-lane histogram of hits by smallest radius, distance sums beside it
     int* gcnt = reinterpret_cast<int*>(wsm + kTile * DP);
     float* gsum = wsm + kTile * DP + 32 * p.G;
@@ -193,18 +188,18 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
     }
     __syncwarp();
 
-    // ---- one candidate against this lane's query.  kNN: the candidate is only noted; heap inserts are
-    // divergent per-lane loops, so the warp runs them for all lanes at once (`merge_pending`) when a lane's
-    // buffer is nearly full or a new grid row needs tight thresholds -- a lane that inserted alone would keep
-    // 31 lanes idle for ~50 instructions (the ncu capture of the immediate-insert version showed 13.5 of 32
-    // lanes active per instruction).  Until the merge the lane's threshold is stale, i.e. too large: safe.
+    // ---- one candidate against this lane's query
     auto consider = [&](float acc, int cpos) {
         if (MODE == MODE_KNN) {
-            pend_d[npend * 32 + lane] = acc;
-            pend_p[npend * 32 + lane] = cpos;
-            ++npend;
-        } else if (MODE == MODE_RANGE) {
             if (cpos == pos) return;                         // self by index (reading A4)
+            const int id = __ldg(p.perm + cpos);
+            if (acc < tau || id < tau_id) {
+                hp.sift(acc, id, k);
+                tau = hp.D(0);
+                tau_id = hp.I(0);
+            }
+        } else if (MODE == MODE_RANGE) {
+            if (cpos == pos) return;
             cnt += 1;
             sum += sqrtf(acc);
         } else {
@@ -214,21 +209,6 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
             gcnt[g * 32 + lane] += 1;
             gsum[g * 32 + lane] += sqrtf(acc);
         }
-    };
-    auto merge_pending = [&]() {
-        for (int e = 0; e < npend; ++e) {
-            const float d = pend_d[e * 32 + lane];
-            const int cpos = pend_p[e * 32 + lane];
-            if (cpos == pos) continue;                       // self by index (reading A4)
-            if (d > tau) continue;
-            const int id = __ldg(p.perm + cpos);
-            if (d < tau || id < tau_id) {
-                hp.sift(d, id, k);
-                tau = hp.D(0);
-                tau_id = hp.I(0);
-            }
-        }
-        npend = 0;
     };
 
     // ---- stream sorted positions [a, b) through the tile; lanes with `active` evaluate them
@@ -262,9 +242,9 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
             }
             __syncwarp();
             if (t0 + kTilePairs < pb) fetch(t0 + kTilePairs);
+            if (active) {
 #pragma unroll 2
-            for (int r = 0; r < n; ++r) {
-                if (active) {
+                for (int r = 0; r < n; ++r) {
                     f32x2 acc = 0ull;                        // (0.f, 0.f)
 #pragma unroll
                     for (int g = 0; g < G4; ++g) {
@@ -286,7 +266,6 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
                         if (a1 <= tau && c0 + 1 < b) consider(a1, c0 + 1);
                     }
                 }
-                if (MODE == MODE_KNN && __any_sync(kFull, npend > kPend - 2)) merge_pending();
             }
         }
         __syncwarp();
@@ -348,8 +327,6 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
                     if (!live1) continue;
                     const int s1 = side1 == 0 ? home[1] + o1 : home[1] - o1;
                     if (s1 < 0 || s1 >= B1) { live1 = false; continue; }
-                    // tight thresholds before the row's ranges are formed
-                    if (MODE == MODE_KNN && __any_sync(kFull, npend > 0)) merge_pending();
                     const float g1 = slab_gap(1, b1, s1);
                     const float lb01 = __fmaf_rn(g1, g1, lb0);
                     const bool alive = valid && lb01 <= tau;
@@ -398,7 +375,6 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
         }
     }
 
-    if (MODE == MODE_KNN) merge_pending();
     // ---- a7: emit
     if (!valid) return;
     if (MODE == MODE_KNN) {
