@@ -48,7 +48,9 @@ typedef int snaps_status;
 #define SNAPS_UNSUPPORTED 4
 
 #define SNAPS_MAX_FEATURES 15 /* PAPER.md:109 "We examine d <= 15" */
-#define SNAPS_MAX_K 256        /* grid engine (k_max = 256 on LSST5M) */
+#define SNAPS_MAX_K 4096       /* grid engine (k_max = 4096 on SNAPShot1; 256 on LSST5M).
+                                  Lists up to 256 entries live in shared memory; longer ones are built in
+                                  place in out_idx / out_dist, which must then both be given */
 #define SNAPS_LATTICE_MAX_K 32 /* sub-lattice engine: lists live in shared memory */
 
 /*
@@ -58,7 +60,7 @@ typedef int snaps_status;
  *                         pair's squared differences; brute force with an exact filter.  For
  *                         mask lists with sub-lattice structure (all subsets) on L2-sized tables.
  *   SNAPS_ENGINE_GRID     one subspace at a time through a grid index on up to three of its
- *                         features.  For arbitrary mask lists, large N, k <= 256.
+ *                         features.  For arbitrary mask lists, large N, k <= 4096.
  * Both engines compute the same joins; a pair's fp32 distance may differ in the last bit between
  * them (different summation order), so equal-distance ties may resolve differently.
  * SNAPS_FLAG_X_ON_HOST: the table pointer is a HOST pointer (pinned or pageable); the call copies
@@ -105,7 +107,8 @@ int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t *h_masks, int 
  *   d_X        device (host with SNAPS_FLAG_X_ON_HOST), [N][ld] fp32; every column finite,
  *              including columns no mask uses
  *   h_masks    host, [n_masks] uint16
- *   k          1 <= k <= min(N-1, SNAPS_MAX_K); the sub-lattice engine holds k <= 32
+ *   k          1 <= k <= min(N-1, SNAPS_MAX_K); the sub-lattice engine holds k <= 32; k > 256 needs
+ *              out_idx and out_dist (the lists are built in place)
  *   q_begin, q_end   the queries: 0 <= q_begin < q_end <= N; nq = q_end - q_begin.  A rank of a
  *              multi-GPU run owns one slice (no exchange step);
  *              (0, N) is the whole self-join

@@ -670,6 +670,8 @@ snaps_status knn_batched(const float* X, int64_t N, int n_feat, int64_t ld, cons
         any |= B.arr[a].want;
     }
     if (!any) return fail(SNAPS_INVALID_ARG, "no output asked for");
+    if (k > snaps::kGridMaxK && (!B.arr[0].want || !B.arr[1].want))
+        return fail(SNAPS_INVALID_ARG, "k = %d > %d: the lists are built in place, idx and dist outputs are required", k, snaps::kGridMaxK);
     if (sink) {
         rc = sink_check(sink, off);
         if (rc) return rc;
@@ -805,6 +807,8 @@ snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t
         return fail(SNAPS_INVALID_ARG, "k = %d outside 1..min(N-1, %d)", k, SNAPS_MAX_K);
     if (!out_idx && !out_dist && !out_kth && !out_mean && !out_indeg)
         return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
+    if (k > snaps::kGridMaxK && (!out_idx || !out_dist))
+        return fail(SNAPS_INVALID_ARG, "k = %d > %d: the lists are built in place, out_idx and out_dist are required", k, snaps::kGridMaxK);
     rc = carve(d_workspace, workspace_bytes, E.job, &E.w);
     if (rc) return rc;
     rc = engine_begin(&E);

@@ -14,8 +14,9 @@
 //     prefetched into registers); every lane evaluates every candidate of the tile with broadcast
 //     128-bit shared-memory reads: d FSUB + d FFMA + one compare per pair;
 //   * kNN: per-lane max-heap of (d^2, id) in shared memory (conflict-free: entry e of lane l at
-//     e*32 + l), root = threshold; a 256-position window around the warp seeds the heaps first;
-//     heapsort at the end; ties by the smaller id (reading A3);
+//     e*32 + l; for k > 256 in the lane's own rows of the output lists), root = threshold; a window of
+//     the sorted order around the warp seeds the heaps first; heapsort at the end; ties by the smaller
+//     id (reading A3);
 //   * DSSJ: per-lane count and sum in registers (or G counters for a radius grid).
 // The distance of a pair is the FMA chain over the mask's features in ascending order, the same
 // wherever it is formed, so results do not depend on the grid resolution or the scan order
@@ -31,7 +32,7 @@ constexpr int kTile = 64;            // candidates per tile
 constexpr int kSeedHalf = 112;       // seed window: this many sorted positions either side of the warp
 constexpr int kMaxG = 32;
 
-constexpr int MODE_KNN = 0, MODE_RANGE = 1, MODE_RANGE_GRID = 2;
+constexpr int MODE_KNN = 0, MODE_RANGE = 1, MODE_RANGE_GRID = 2, MODE_KNN_BIG = 3;
 
 __host__ __device__ constexpr int dp_of(int d) { return (d + 3) / 4 * 4; }
 
@@ -40,13 +41,16 @@ __host__ __device__ constexpr int warp_words(int d, int mode, int k, int G) {
     return kTile * dp_of(d) + (mode == MODE_KNN ? 64 * k : 0) + (mode == MODE_RANGE_GRID ? 64 * G + 32 : 0);
 }
 
+// Per-lane max-heap of (d^2, id).  BIG = false: in shared memory, entry e of lane l at e*32 + l (conflict-free
+// whatever path each lane's sift takes).  BIG = true (k > 256): in the lane's own rows of the output lists
+// (out_dist / out_idx of its query), which the heapsort at the end leaves in their final ascending order.
+template <bool BIG>
 struct Heap {
-    float* d;   // [k][32]
-    int* i;     // [k][32]
-    int k;
+    float* d;
+    int* i;
     int lane;
-    __device__ __forceinline__ float& D(int e) { return d[e * 32 + lane]; }
-    __device__ __forceinline__ int& I(int e) { return i[e * 32 + lane]; }
+    __device__ __forceinline__ float& D(int e) { return BIG ? d[e] : d[e * 32 + lane]; }
+    __device__ __forceinline__ int& I(int e) { return BIG ? i[e] : i[e * 32 + lane]; }
     // replace the root (the largest key) by (v, id) and restore the heap over entries [0, n)
     __device__ __forceinline__ void sift(float v, int id, int n) {
         int e = 0;
@@ -108,10 +112,11 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
     const int k = p.k;
     float* wsm = reinterpret_cast<float*>(smem_raw) + static_cast<size_t>(warp) * warp_words(D, MODE, k, p.G);
     float4* tile4 = reinterpret_cast<float4*>(wsm);
-    Heap hp;
+    constexpr bool KNN = MODE == MODE_KNN || MODE == MODE_KNN_BIG;
+    constexpr bool BIG = MODE == MODE_KNN_BIG;
+    Heap<BIG> hp;
     hp.d = wsm + kTile * DP;
     hp.i = reinterpret_cast<int*>(hp.d + 32 * k);
-    hp.k = k;
     hp.lane = lane;
     // radius grid: per-lane histogram of hits by smallest radius, distance sums beside it
     int* gcnt = reinterpret_cast<int*>(wsm + kTile * DP);
@@ -130,6 +135,10 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
     if (valid) {
         key = p.keys[pos];
         my_id = p.perm[pos];
+        if (BIG) {
+            hp.d = p.out_dist + static_cast<size_t>(my_id - p.q_begin) * k;
+            hp.i = p.out_idx + static_cast<size_t>(my_id - p.q_begin) * k;
+        }
         const float* row = p.Xp + static_cast<size_t>(my_id) * kRowFloats;
 #pragma unroll
         for (int j = 0; j < D; ++j) q[j] = __ldg(row + pl->feat[j]);
@@ -171,11 +180,12 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
     int tau_id = 0x7fffffff;
     int cnt = 0;
     float sum = 0.f;
-    if (MODE == MODE_KNN) {
-        for (int e = 0; e < k; ++e) {
-            hp.D(e) = __int_as_float(0x7f800000);
-            hp.I(e) = 0x7fffffff;
-        }
+    if (KNN) {
+        if (!BIG || valid)
+            for (int e = 0; e < k; ++e) {
+                hp.D(e) = __int_as_float(0x7f800000);
+                hp.I(e) = 0x7fffffff;
+            }
     } else if (MODE == MODE_RANGE) {
         if (valid) tau = p.eps2;
     } else {
@@ -190,7 +200,7 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
 
     // ---- one candidate against this lane's query
     auto consider = [&](float acc, int cpos) {
-        if (MODE == MODE_KNN) {
+        if (KNN) {
             if (cpos == pos) return;                         // self by index (reading A4)
             const int id = __ldg(p.perm + cpos);
             if (acc < tau || id < tau_id) {
@@ -273,7 +283,7 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
 
     // ---- kNN: seed the heaps from the sorted neighbourhood of the warp
     int w0 = 0, w1 = 0;
-    if (MODE == MODE_KNN) {
+    if (KNN) {
         const int p_first = __shfl_sync(kFull, pos, 0);
         const int n_valid = min(32, static_cast<int>(p.nq - qi0));
         const int p_last = __shfl_sync(kFull, pos, n_valid - 1);
@@ -377,7 +387,7 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
 
     // ---- a7: emit
     if (!valid) return;
-    if (MODE == MODE_KNN) {
+    if (KNN) {
         // heapsort: ascending by (d^2, id) in entries 0..k-1
         for (int n = k - 1; n >= 1; --n) {
             const float v = hp.D(n);
@@ -393,8 +403,12 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
             const int id = hp.I(e);
             s += dd;
             dk = dd;
-            if (p.out_idx) p.out_idx[o * k + e] = id;
-            if (p.out_dist) p.out_dist[o * k + e] = dd;
+            if (BIG) {
+                hp.D(e) = dd;                                 // the heap rows ARE the output lists
+            } else {
+                if (p.out_idx) p.out_idx[o * k + e] = id;
+                if (p.out_dist) p.out_dist[o * k + e] = dd;
+            }
             if (p.out_indeg) atomicAdd(&p.out_indeg[id], 1);
         }
         if (p.out_kth) p.out_kth[o] = dk;
@@ -461,7 +475,11 @@ cudaError_t launch_mode(const GridJoinParams& p, int d, cudaStream_t st) {
 }  // namespace
 
 cudaError_t grid_knn_launch(const GridJoinParams& p, int d, cudaStream_t st) {
-    if (p.k < 1 || p.k > kGridMaxK) return cudaErrorInvalidValue;
+    if (p.k < 1 || p.k > kGridMaxKBig) return cudaErrorInvalidValue;
+    if (p.k > kGridMaxK) {
+        if (!p.out_idx || !p.out_dist) return cudaErrorInvalidValue;   // the heaps live in the output lists
+        return launch_mode<MODE_KNN_BIG>(p, d, st);
+    }
     return launch_mode<MODE_KNN>(p, d, st);
 }
 

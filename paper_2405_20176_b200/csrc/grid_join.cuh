@@ -4,7 +4,8 @@
 
 namespace snaps {
 
-constexpr int kGridMaxK = 256;          // kNN list length the grid engine supports (k_max = 256 on LSST5M)
+constexpr int kGridMaxK = 256;          // kNN lists up to this length live in shared memory (k_max = 256 on LSST5M)
+constexpr int kGridMaxKBig = 4096;      // beyond it the heaps live in the output lists (k_max = 4096 on SNAPShot1)
 
 struct GridJoinParams {
     // index of this mask (grid_index.cuh)

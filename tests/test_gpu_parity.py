@@ -202,7 +202,9 @@ def test_argument_errors(snaps):
     with pytest.raises(snaps.SnapsError):
         snaps.knn_selfjoin(X, [0b10000], 3)              # bit >= n_feat
     with pytest.raises(snaps.SnapsError):
-        snaps.knn_selfjoin(X, [0b11], 33)                # k > SNAPS_MAX_K
+        snaps.knn_selfjoin(X, [0b11], 4097)              # k > SNAPS_MAX_K
+    with pytest.raises(snaps.SnapsError):
+        snaps.knn_selfjoin(torch.rand((600, 4), device="cuda"), [0b11], 300, lists=False)   # k > 256 builds the lists in place
     with pytest.raises(snaps.SnapsError):
         snaps.range_selfjoin(X, [0b11], [float("nan")])
     with pytest.raises(snaps.SnapsError):
@@ -580,3 +582,22 @@ def test_paper_operating_point_large_selectivity(snaps, oracle_mod):
     mean_cnt = out["count"].float().mean(dim=2).cpu().numpy()
     assert (mean_cnt[:, 0] > 0.0003 * N).all() and (mean_cnt[:, 0] < 0.004 * N).all()      # ~0.001 |D|
     assert (mean_cnt[:, -1] > 0.08 * N).all() and (mean_cnt[:, -1] < 0.3 * N).all()         # ~0.15 |D|
+
+
+def test_paper_operating_point_k4096(snaps, oracle_mod):
+    """k_max = 4096 on SNAPShot1 (13 % of the catalogue).  N = 31,693, three masks, k = 4096: the
+    grid engine with its heaps in the output lists.  Sampled queries against the oracle; whole-output invariants."""
+    import torch
+    cfg = workloads.get_config("c2_snapshot1_knn")
+    X = cfg.table()
+    N, k = len(X), 4096
+    masks = np.array([0b11, (1 << 9) | (1 << 3) | 1 | (1 << 12), 0x7FFF], dtype=np.uint16)
+    out = snaps.knn_selfjoin(_dev(X), masks, k)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(4096)
+    qs = np.sort(rng.choice(N, 6, replace=False))
+    oi, od = oracle_mod.knn_selfjoin(X, masks, k + 1, queries=qs)
+    check_knn(out["idx"][:, qs].cpu().numpy(), out["dist"][:, qs].cpu().numpy(), oi, od, queries=qs)
+    assert bool((out["indeg"].sum(dim=1) == N * k).all())
+    assert bool((out["dist"][:, :, 1:] >= out["dist"][:, :, :-1]).all())
+    assert torch.equal(out["kth"], out["dist"][:, :, -1])
