@@ -176,6 +176,21 @@ snaps_status snaps_outlier_scores(int64_t N, int n_masks, int k,
                                   float *out_eps_mean, void *stream);
 
 /*
+ * kNN -> DSSJ reuse (the paper's future work: "providing the set of k nearest neighbors from
+ * kNNSJ to DSSJ for its computation").  From kNN lists already on the device: for every (mask, query) the
+ * number of listed neighbours with D <= eps_mask, their distance sum and mean, and out_complete = 1 where
+ * the k-th neighbour lies beyond eps -- the list then holds the whole eps-neighbourhood and the values ARE
+ * the range join's (up to the rounding of D = sqrt(d^2) against eps, the 1e-6 band of reading A2); where
+ * out_complete = 0 the object still needs snaps_range_selfjoin (its count is a lower bound).
+ *   knn_dist  device [n_masks][nq][k] fp32 ascending, as written by snaps_knn_selfjoin
+ *   d_eps     DEVICE [n_masks] fp32 (e.g. a column of snaps_eps_search's output)
+ *   out_count device [n_masks][nq] uint32; out_sumdist, out_mean fp32 or NULL; out_complete uint8 or NULL
+ */
+snaps_status snaps_range_from_knn(int64_t nq, int n_masks, int k, const float *knn_dist,
+                                  const float *d_eps, uint32_t *out_count, float *out_sumdist,
+                                  float *out_mean, uint8_t *out_complete, void *stream);
+
+/*
  * ---- a8: batched ("oversubscribed") joins for outputs that exceed device
  * (or host) memory.  Masks are processed in groups of masks_per_batch; each group's outputs are
  * produced into a two-slot device staging ring inside d_workspace and copied on a side stream

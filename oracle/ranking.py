@@ -132,3 +132,16 @@ def select_eps(counts, means, n: int):
     u_min, u_max = similarity_curves(tops, n)
     out["dssj_mean"] = (select_parameter(u_min, u_max, n), u_min, u_max)
     return out
+
+
+def range_from_knn(dist_k, eps: float):
+    """kNN -> DSSJ reuse for ONE mask, from the definitions: with the k nearest neighbours of
+    every object sorted by distance, the objects within eps are a prefix of the list; if the k-th neighbour
+    lies beyond eps the prefix is the whole eps-neighbourhood.
+    dist_k: [N][k] ascending.  -> (count, sumdist, mean, complete)."""
+    d = np.asarray(dist_k)
+    inside = d <= d.dtype.type(eps)
+    cnt = inside.sum(axis=1)
+    s = np.where(inside, d, 0).sum(axis=1, dtype=np.float64)
+    mean = np.where(cnt > 0, s / np.maximum(cnt, 1), 0.0)
+    return cnt, s, mean, cnt < d.shape[1]

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = [
     "snaps_select_k_workspace_bytes", "snaps_knn_select_k",
     "snaps_dist_hist_workspace_bytes", "snaps_sample_distance_histogram", "snaps_eps_from_histogram",
     "snaps_eps_search_workspace_bytes", "snaps_eps_search",
-    "snaps_select_eps_workspace_bytes", "snaps_range_select_eps",
+    "snaps_select_eps_workspace_bytes", "snaps_range_select_eps", "snaps_range_from_knn",
 ]
 
 ENGINES = {"auto": 0, "lattice": 1, "grid": 2}
@@ -124,6 +124,8 @@ def lib():
         L.snaps_range_select_eps.restype = i32
         L.snaps_range_select_eps.argtypes = [vp, i64, i32, i64, vp, i32, vp, i32, vp, i32, i32, ctypes.c_double,
                                              ctypes.c_double, i32, i32, i32, vp, vp, vp, vp, vp, sz, vp]
+        L.snaps_range_from_knn.restype = i32
+        L.snaps_range_from_knn.argtypes = [i64, i32, i32, vp, vp, vp, vp, vp, vp, vp]
         L.snaps_select_k_workspace_bytes.restype = sz
         L.snaps_select_k_workspace_bytes.argtypes = [i64, i32, i32]
         L.snaps_knn_select_k.restype = i32
@@ -598,4 +600,23 @@ def range_select_eps(X, masks, sample_q, sample_c, s_min: float, s_max: float, G
         float(s_min), float(s_max), G, n_top, _flags(engine), _dptr(out["eps_grid"]), _dptr(out["j_count"]),
         _dptr(out["j_mean"]), _dptr(out["u"]), _dptr(ws), ws.numel(), _stream(stream)))
     out["_workspace"] = ws
+    return out
+
+
+def range_from_knn(knn_dist, eps, stream=None):
+    """snaps_range_from_knn: lists [n_masks, nq, k] (CUDA fp32) + radii [n_masks] (CUDA fp32 or array-like) ->
+    dict count (int32 view) / sumdist / mean [n_masks, nq] and complete (uint8: 1 = the list holds the whole
+    eps-neighbourhood)."""
+    import torch
+    n_masks, nq, k = knn_dist.shape
+    dev = knn_dist.device
+    e = eps if hasattr(eps, "is_cuda") else torch.as_tensor(np.asarray(eps, dtype=np.float32))
+    e = e.to(device=dev, dtype=torch.float32).contiguous()
+    assert e.numel() == n_masks and knn_dist.is_contiguous()
+    out = {"count": torch.empty((n_masks, nq), dtype=torch.int32, device=dev),
+           "sumdist": torch.empty((n_masks, nq), dtype=torch.float32, device=dev),
+           "mean": torch.empty((n_masks, nq), dtype=torch.float32, device=dev),
+           "complete": torch.empty((n_masks, nq), dtype=torch.uint8, device=dev)}
+    _check(lib().snaps_range_from_knn(nq, n_masks, k, _dptr(knn_dist), _dptr(e), _dptr(out["count"]),
+                                      _dptr(out["sumdist"]), _dptr(out["mean"]), _dptr(out["complete"]), _stream(stream)))
     return out

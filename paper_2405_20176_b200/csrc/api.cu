@@ -876,6 +876,16 @@ snaps_status snaps_outlier_scores(int64_t N, int n_masks, int k, const int32_t* 
     return SNAPS_OK;
 }
 
+snaps_status snaps_range_from_knn(int64_t nq, int n_masks, int k, const float* knn_dist, const float* d_eps,
+                                  uint32_t* out_count, float* out_sumdist, float* out_mean, uint8_t* out_complete,
+                                  void* stream) {
+    if (nq < 1 || n_masks < 1 || k < 1) return fail(SNAPS_INVALID_ARG, "bad sizes");
+    if (!knn_dist || !d_eps || !out_count) return fail(SNAPS_INVALID_ARG, "NULL lists, radii or out_count");
+    CUDA_TRY(snaps::range_from_knn_launch(nq, n_masks, k, knn_dist, d_eps, out_count, out_sumdist, out_mean, out_complete,
+                                          static_cast<cudaStream_t>(stream)));
+    return SNAPS_OK;
+}
+
 size_t snaps_stream_ring_bytes(int64_t nq, int64_t N, int k, int masks_per_batch) {
     if (nq < 1 || N < 2 || nq > N || k < 0 || masks_per_batch < 1) return 0;
     return ring_bytes(nq, N, k, masks_per_batch);

@@ -104,6 +104,45 @@ cudaError_t eps_mean_launch(int64_t total, const uint32_t* cnt, const float* sum
     return cudaGetLastError();
 }
 
+// kNN -> DSSJ reuse ("providing the set of k nearest neighbors from kNNSJ to DSSJ"): the sorted
+// distances of an object's k nearest neighbours contain its whole eps-neighbourhood whenever the k-th lies
+// beyond eps; count and distance sum are then read off the list and the object needs no range join.
+__global__ void range_from_knn_kernel(int64_t nq, int n_masks, int k, const float* __restrict__ dist,
+                                      const float* __restrict__ eps, uint32_t* __restrict__ out_count,
+                                      float* __restrict__ out_sum, float* __restrict__ out_mean,
+                                      uint8_t* __restrict__ out_complete) {
+    const int64_t total = nq * n_masks;
+    for (int64_t o = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; o < total;
+         o += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+        const float e = eps[o / nq];
+        const float* d = dist + o * k;
+        int cnt = 0;
+        float sum = 0.f;
+        for (int r = 0; r < k; ++r) {
+            const float v = d[r];
+            if (v <= e) {                 // closed ball (reading A2); the list is ascending
+                cnt += 1;
+                sum += v;
+            } else {
+                break;
+            }
+        }
+        out_count[o] = static_cast<uint32_t>(cnt);
+        if (out_sum) out_sum[o] = sum;
+        if (out_mean) out_mean[o] = cnt > 0 ? sum / static_cast<float>(cnt) : 0.f;
+        if (out_complete) out_complete[o] = cnt < k ? 1 : 0;   // the k-th neighbour lies beyond eps
+    }
+}
+
+cudaError_t range_from_knn_launch(int64_t nq, int n_masks, int k, const float* dist, const float* d_eps,
+                                  uint32_t* out_count, float* out_sum, float* out_mean, uint8_t* out_complete,
+                                  cudaStream_t stream) {
+    const int64_t total = nq * n_masks;
+    const int grid = static_cast<int>(std::min<int64_t>((total + 255) / 256, 148 * 32));
+    range_from_knn_kernel<<<grid, 256, 0, stream>>>(nq, n_masks, k, dist, d_eps, out_count, out_sum, out_mean, out_complete);
+    return cudaGetLastError();
+}
+
 // ---- FP32 instruction-rate probes (roofline denominator) ----
 constexpr int kProbeIters = 1024;
 constexpr int kProbeIlp = 16;

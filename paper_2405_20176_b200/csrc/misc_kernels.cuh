@@ -18,6 +18,10 @@ cudaError_t knn_scores_launch(int64_t N, int n_masks, int k, const int32_t* idx,
 cudaError_t eps_mean_launch(int64_t total, const uint32_t* cnt, const float* sum, float* out_mean,
                             cudaStream_t stream);
 
+cudaError_t range_from_knn_launch(int64_t nq, int n_masks, int k, const float* dist, const float* d_eps,
+                                  uint32_t* out_count, float* out_sum, float* out_mean, uint8_t* out_complete,
+                                  cudaStream_t stream);
+
 // kind 0: FFMA, 1: FADD, 2: FADD+FSETP pairs.  Returns lane-ops executed and elapsed ms.
 cudaError_t probe_fp32_launch(int kind, double* lane_ops, float* ms, float* d_scratch, cudaStream_t stream);
 

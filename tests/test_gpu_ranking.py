@@ -310,3 +310,33 @@ def test_select_eps_pipeline_matches_oracle(snaps, engine):
                 assert np.abs(u[2][:, m] - umin_m).max() <= near / n and np.abs(u[3][:, m] - umax_m).max() <= near / n
     assert exact_masks >= len(masks) - 1
     assert (u[0][0] == 1.0).all() and (u[1][-1] == 1.0).all() and (u[2][0] == 1.0).all() and (u[3][-1] == 1.0).all()
+
+
+def test_range_from_knn_matches_oracle_and_the_range_join(snaps):
+    """snaps_range_from_knn (PAPER.md:537 kNN -> DSSJ reuse): index work against the oracle function on the same
+    lists (exact), and against the device's own eps-join wherever the list is complete."""
+    import torch
+    import oracle as oracle_mod
+    N, k = 3000, 24
+    X = workloads.make_table(N, 47, outlier_frac=0.01)
+    masks = np.array([0b11, 0x7FFF, (1 << 9) | (1 << 3) | 1, 0b1111000], dtype=np.uint16)
+    _, od = oracle_mod.knn_selfjoin(X, masks, k)
+    dist = od.astype(np.float32)
+    eps = np.array([np.median(dist[m, :, 9]) * 1.0003 for m in range(len(masks))], dtype=np.float32)
+    out = snaps.range_from_knn(_t(dist), eps)
+    torch.cuda.synchronize()
+    for m in range(len(masks)):
+        cnt, s, mean, complete = oracle_ranking.range_from_knn(dist[m], eps[m])
+        assert (out["count"][m].cpu().numpy() == cnt).all() and (out["complete"][m].cpu().numpy() == complete).all()
+        assert np.allclose(out["sumdist"][m].cpu().numpy(), s, rtol=1e-5) and np.allclose(out["mean"][m].cpu().numpy(), mean, rtol=1e-5)
+    # on the device's own lists: complete objects need no range join
+    Xd = _t(X)
+    join = snaps.knn_selfjoin(Xd, masks, k, scores=False)
+    reuse = snaps.range_from_knn(join["dist"], eps)
+    rj = snaps.range_selfjoin(Xd, masks, eps)
+    torch.cuda.synchronize()
+    c = reuse["complete"].bool()
+    assert 0.2 < c.float().mean().item() < 0.9
+    agree = (reuse["count"][c] == rj["count"][c]).float().mean().item()
+    assert agree > 0.999                                            # all but pairs inside the 1e-6 band of A2
+    assert bool((reuse["count"][~c] == k).all()) and bool((rj["count"][~c] >= k).all())

@@ -63,3 +63,29 @@ def test_stored_config_eps_come_from_the_oracle_script():
                             n_query_sample=300).astype(np.float32)
     assert (workloads.config_eps(cfg.name, masks) == eps).all()
     assert (np.diff([eps[workloads.popcount(masks) == d][0] for d in range(2, 16)]) > 0).all()   # grows with d
+
+
+def test_range_from_knn_is_the_range_join_where_complete():
+    """oracle.ranking.range_from_knn against the oracle's own range join: wherever the k-th neighbour lies
+    beyond eps, count / sum / mean read off the kNN list equal the eps-join's; elsewhere the
+    count is the list length, a lower bound.  1-D lattice closed form on top: interior count = 2 floor(eps/h)."""
+    import oracle
+    import workloads
+    from oracle.ranking import range_from_knn
+    X = workloads.make_table(400, 5, cols=[0, 1, 2, 3])
+    masks = np.array([0b11, 0b1111, 0b0110], dtype=np.uint16)
+    k = 12
+    _, od = oracle.knn_selfjoin(X, masks, k)
+    for m in range(len(masks)):
+        eps = float(np.median(od[m, :, 5]))          # about half the objects complete
+        cnt, s, mean, complete = range_from_knn(od[m], eps)
+        rc, rs, rm = oracle.range_selfjoin(X, masks[m:m + 1], [eps])
+        assert 0.2 < complete.mean() < 0.9
+        assert (cnt[complete] == rc[0][complete]).all() and np.allclose(s[complete], rs[0][complete], rtol=1e-12)
+        assert np.allclose(mean[complete], rm[0][complete], rtol=1e-12)
+        assert (cnt[~complete] == k).all() and (rc[0][~complete] >= k).all()
+    h, n = 2.0 ** -6, 40
+    L = workloads.lattice_table(n, 2, h)
+    _, ld = oracle.knn_selfjoin(L, [0b01], 10)
+    cnt, _, _, complete = range_from_knn(ld[0], 2.5 * h)
+    assert (cnt[5:-5] == 4).all() and complete.all() and cnt[0] == 2
