@@ -433,6 +433,9 @@ def main():
     ap.add_argument("--config", default="c2_snapshot1_knn")
     ap.add_argument("--scaling", default="strong", choices=["strong", "weak"],
                     help="N > 1: strong = one catalogue, masks dealt to ranks; weak = one catalogue per rank")
+    ap.add_argument("--dealing", default="static", choices=["static", "dynamic"],
+                    help="strong scaling of config 2: static = batches dealt round-robin up front; dynamic = a shared "
+                         "counter hands out groups of 8 batches, the least loaded rank takes the next (PAPER.md:323)")
     ap.add_argument("--ref-queries", type=int, default=1024,
                     help="sampled queries per step of --impl reference")
     ap.add_argument("--cpu-queries", type=int, default=4096,
@@ -497,7 +500,8 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
     masks_all = cfg.masks()
     if args.masks_limit > 0:
         masks_all = masks_all[:args.masks_limit]
-    mine = np.arange(len(masks_all)) if (world == 1 or weak) else shard_masks(masks_all, rank, world)
+    dynamic = args.dealing == "dynamic" and not weak
+    mine = np.arange(len(masks_all)) if (world == 1 or weak or dynamic) else shard_masks(masks_all, rank, world)
     masks = masks_all[mine]
     N, n_feat, k, n_masks = len(X), X.shape[1], cfg.k, len(masks)
     job_masks = len(masks_all) * (world if weak else 1)       # subspaces the whole job finishes per step
@@ -512,24 +516,45 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
     snaps.profile_enable(True)
 
+    step_no = [0]
+    if dynamic:
+        # the least loaded GPU takes the next unit.  Units = groups of 8 sub-lattice batches (512
+        # masks); a counter in the job's store hands them out; every rank keeps what it computed in its own rows.
+        from paper_2405_20176_b200.sharding import DynamicDealer, mask_groups
+        groups = mask_groups(masks_all, 8)
+        store = (D.dist.distributed_c10d._get_default_store() if world > 1 else D.dist.HashStore())
+
     def step():
+        """-> (join-kernel ms, join launches, masks this rank processed)"""
         flush.zero_()
-        snaps.knn_selfjoin(Xd, masks, k, lists=False, out=out, workspace=ws)
+        if not dynamic:
+            snaps.knn_selfjoin(Xd, masks, k, lists=False, out=out, workspace=ws)
+            ms, n = snaps.profile_last_kernel_ms()     # waits for this step's join kernel
+            return ms, n + 3, n_masks                  # + the two staging kernels + the L2 flush fill
+        step_no[0] += 1
+        ms_tot, n_tot, row = 0.0, 1, 0
+        for u in DynamicDealer(store, len(groups), name=f"knn_step_{step_no[0]}"):
+            g = groups[u]
+            sub = {name: t[row:row + len(g)] for name, t in out.items()}
+            snaps.knn_selfjoin(Xd, masks_all[g], k, lists=False, out=sub, workspace=ws)
+            ms, n = snaps.profile_last_kernel_ms()
+            ms_tot, n_tot, row = ms_tot + ms, n_tot + n + 2, row + len(g)
+        return ms_tot, n_tot, row
 
     for _ in range(args.warmup):
         step()
     torch.cuda.synchronize()
     D.barrier()
     sampler = ClockSampler(dev.index or 0) if rank == 0 else None
-    kernel_ms, launches = [], 0
+    kernel_ms, launches, done = [], 0, []
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     ev0.record()
     for _ in range(args.steps):
-        step()
-        ms, n = snaps.profile_last_kernel_ms()     # waits for this step's join kernel
+        ms, n, nm = step()
         kernel_ms.append(ms)
-        launches += n + 3                          # + the two staging kernels + the L2 flush fill
+        launches += n
+        done.append(nm)
     ev1.record()
     torch.cuda.synchronize()
     D.barrier()
@@ -539,7 +564,12 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
     evals_per_s = float(N) * N * job_masks / (ms_per_step * 1e-3)
 
     # sanity on the last step's result: every mask's in-degree row sums to N*k
-    chk = int(out["indeg"][n_masks // 2].sum().item())
+    if dynamic:
+        tot = D.sum_over_ranks(float(done[-1]))
+        assert int(tot) == len(masks_all), f"dynamic dealing covered {tot} of {len(masks_all)} masks"
+        evals = float(N) * N * float(np.mean(done))               # what this rank processed per step
+        planned = evals * float(snaps.planned_evals(N, n_feat, masks_all)) / (float(N) * N * len(masks_all))
+    chk = int(out["indeg"][max(0, min(n_masks, done[-1]) // 2)].sum().item()) if done[-1] > 0 else N * k
     assert chk == N * k, f"in-degree sum {chk} != N*k = {N * k}"
 
     # ---- roofline of the dominant kernel (knn_lattice_kernel): ALU/FP32-issue bound
@@ -633,7 +663,9 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
                        "l2": "256 MB flush fill before every step; each step also writes 12.5 GB of scores",
                        "outputs": "scores only (lists of this config are 83 GB)",
                        "sharding": ("one catalogue per rank" if weak else
-                                    "one catalogue; masks dealt to ranks by sub-lattice batch, no collective") if world > 1 else "none"},
+                                    "one catalogue; groups of 8 batches handed out by a shared counter (least loaded rank next), no collective"
+                                    if dynamic else
+                                    "one catalogue; masks dealt to ranks by sub-lattice batch, no collective") if (world > 1 or dynamic) else "none"},
             "evals_per_s": evals_per_s, "fp32_peak_frac": roofline["frac"],
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
             "dssj": dssj, "lsst_scale": lsst,

@@ -60,3 +60,33 @@ def shard_masks_by_cost(masks, rank: int, world: int):
         pc += (m >> b) & 1
     order = np.argsort(pc, kind="stable")
     return np.sort(order[rank::world])
+
+
+def mask_groups(masks, batches_per_group: int = 8):
+    """The mask list cut into groups of whole sub-lattice batches in Gray order (the unit of work a rank
+    takes at a time under dynamic dealing).  -> list of index arrays into `masks`."""
+    m = np.asarray(masks, dtype=np.uint16).astype(np.int64)
+    high = m >> LOW_BITS
+    keys = np.unique(high)
+    order = keys[np.argsort(_gray_rank(keys), kind="stable")]
+    groups = []
+    for g0 in range(0, len(order), batches_per_group):
+        sel = np.isin(high, order[g0:g0 + batches_per_group])
+        groups.append(np.flatnonzero(sel))
+    return groups
+
+
+class DynamicDealer:
+    """"the least loaded GPU is assigned the next feature space".  A shared counter in the
+    job's torch.distributed store hands out work-unit indices in order: a rank that finishes early simply
+    takes the next unit.  No data-path collective; the only traffic is one integer per unit."""
+
+    def __init__(self, store, n_units: int, name: str = "snaps_next_unit"):
+        self.store, self.n_units, self.name = store, n_units, name
+
+    def __iter__(self):
+        while True:
+            unit = int(self.store.add(self.name, 1)) - 1
+            if unit >= self.n_units:
+                return
+            yield unit

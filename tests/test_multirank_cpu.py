@@ -110,3 +110,36 @@ def test_query_range_sharding_world2_gloo(tmp_path):
     world = 2
     mp.spawn(_query_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
     assert all((tmp_path / f"q_ok{r}").exists() for r in range(world))
+
+
+def _dealer_worker(rank, world, port, out_dir):
+    """Dynamic dealing: two ranks of different speed drain one counter; the units they take are a
+    disjoint cover, and the slower rank ends up with fewer of them."""
+    import time
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_2405_20176_b200.sharding import DynamicDealer, mask_groups
+    masks = workloads.all_masks(15)
+    groups = mask_groups(masks, 8)
+    assert len(groups) == 64 and sum(len(g) for g in groups) == len(masks)
+    assert len(np.unique(np.concatenate(groups))) == len(masks)
+    store = dist.distributed_c10d._get_default_store()
+    dist.barrier()
+    mine = []
+    for unit in DynamicDealer(store, len(groups), name="t_units"):
+        mine.append(unit)
+        time.sleep(0.02 if rank == 0 else 0.002)              # rank 0 is the slow GPU
+    got = [None] * world
+    dist.all_gather_object(got, mine)
+    allu = sorted(u for g in got for u in g)
+    assert allu == list(range(len(groups)))
+    assert len(got[0]) < len(got[1])
+    dist.barrier()
+    dist.destroy_process_group()
+    open(os.path.join(out_dir, f"d_ok{rank}"), "w").write("ok")
+
+
+def test_dynamic_dealing_world2_gloo(tmp_path):
+    world = 2
+    mp.spawn(_dealer_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    assert all((tmp_path / f"d_ok{r}").exists() for r in range(world))
