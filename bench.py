@@ -102,6 +102,28 @@ def oracle_sample(cfg, X, masks, n_queries, seed=0):
     return dt, evals, oracle.num_threads(), what
 
 
+def kdtree_sample(cfg, X, masks, budget_s=15.0, seed=0):
+    """A second, library CPU arm beside the oracle (context only): scipy's cKDTree built per subspace and queried
+    for all N objects with all host cores -- what a CPU user of the method would run per feature space.  One mask
+    per dimension d = 2..15, stopped after `budget_s` seconds; subspaces/s = masks done / time."""
+    from scipy.spatial import cKDTree
+    sm = stratified_masks(masks, 1, seed)
+    t0 = time.perf_counter()
+    done, dims = 0, []
+    for m in sm:
+        cols = [j for j in range(X.shape[1]) if (int(m) >> j) & 1]
+        Xs = np.ascontiguousarray(X[:, cols], dtype=np.float64)
+        cKDTree(Xs).query(Xs, k=cfg.k + 1, workers=-1)
+        done += 1
+        dims.append(len(cols))
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    return {"value": done / dt, "unit": UNIT, "kind": "scipy.spatial.cKDTree per subspace, all host cores (library; context only)",
+            "sample": f"{done} subspaces, one per dimension (d = {min(dims)}..{max(dims)}), all {len(X)} queries, k={cfg.k}",
+            "seconds": dt}
+
+
 def run_reference(args, rank):
     """--impl reference: the oracle as it stands on the host cores (rank 0 only)."""
     if rank != 0:
@@ -628,6 +650,10 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
         dt, ev, cores, what = oracle_sample(cfg, X, masks, args.cpu_queries)
         cpu = {"value": ev / dt / (float(N) * N), "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": what, "evals_per_s": ev / dt, "seconds": dt}
+        try:
+            cpu["library_arm"] = kdtree_sample(cfg, X, masks)
+        except Exception as e:                                   # scipy missing or too slow: the oracle figure stands
+            cpu["library_arm"] = {"error": repr(e)[:120]}
 
     # ---- the other configs, side by side (north star): DSSJ (config 3), LSST scale (config 4)
     dssj = lsst = None
