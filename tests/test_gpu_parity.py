@@ -601,3 +601,28 @@ def test_paper_operating_point_k4096(snaps, oracle_mod):
     assert bool((out["indeg"].sum(dim=1) == N * k).all())
     assert bool((out["dist"][:, :, 1:] >= out["dist"][:, :, :-1]).all())
     assert torch.equal(out["kth"], out["dist"][:, :, -1])
+
+
+def test_radius_grid_sub_lattice_engine_full_size(snaps, oracle_mod):
+    """The sub-lattice radius-grid kernel (range_grid.cu) at config 3's size: N = 31,693, two whole batches
+    (128 lattice slots, 125 masks), four radii per mask up to config 3's stored eps_d; sampled queries of every
+    (mask, radius) against the oracle, and the largest radius against the single-radius kernel."""
+    import torch
+    cfg = workloads.get_config("c3_snapshot1_dssj")
+    X, allm = cfg.table(), cfg.masks()
+    N = len(X)
+    hi = allm.astype(np.int64) >> 6
+    masks = allm[np.isin(hi, [0, 0b100100001])]
+    eps = workloads.config_eps(cfg.name, masks)
+    grid = (eps[:, None] * np.array([0.4, 0.6, 0.8, 1.0], dtype=np.float32)[None, :]).astype(np.float32)
+    Xd = _dev(X)
+    out = snaps.range_selfjoin_grid(Xd, masks, grid, engine="lattice")
+    one = snaps.range_selfjoin(Xd, masks, grid[:, -1].copy(), engine="lattice")
+    torch.cuda.synchronize()
+    assert torch.equal(out["count"][:, -1], one["count"])
+    rng = np.random.default_rng(21)
+    qs = np.sort(rng.choice(N, 8, replace=False))
+    for g in range(grid.shape[1]):
+        check_range(out["count"][:, g][:, qs].cpu().numpy(), out["sumdist"][:, g][:, qs].cpu().numpy(),
+                    out["mean"][:, g][:, qs].cpu().numpy(), oracle_mod, X, masks, grid[:, g], queries=qs)
+    assert bool((out["count"][:, 1:] >= out["count"][:, :-1]).all())          # nested result sets (PAPER.md:235)
