@@ -195,7 +195,7 @@ snaps_status check_job(const Job& j, int k_for_engine) {
 // ---- workspace ---------------------------------------------------------------------------
 // common:   [host-X copy] | Xp | counter(256)
 // lattice:  Xb | batch descriptors (n_masks)
-// grid:     device masks | plans | radii (n_masks x 32 floats) | table region | index region
+// grid:     device masks | plans | table region | index region
 // then:     whatever the caller added (staging ring, radius grid)
 struct Workspace {
     float* Xdense;             // dense copy of a host X, else nullptr
@@ -205,7 +205,6 @@ struct Workspace {
     snaps::BatchDesc* batches;
     uint16_t* d_masks;
     snaps::GridPlan* plans;
-    float* radii;
     unsigned char* grid_table;
     unsigned char* grid_index;
     size_t grid_index_bytes;
@@ -223,7 +222,6 @@ size_t base_workspace_bytes(int64_t N, int n_feat, int n_masks, int engine, int 
     } else {
         b += align_up(static_cast<size_t>(n_masks) * 2, 256);
         b += align_up(static_cast<size_t>(n_masks) * sizeof(snaps::GridPlan), 256);
-        b += align_up(static_cast<size_t>(n_masks) * 32 * 4, 256);
         b += snaps::grid_table_bytes(N) + snaps::grid_index_bytes(N);
     }
     return b;
@@ -255,8 +253,6 @@ snaps_status carve(void* d_ws, size_t bytes, const Job& j, Workspace* w) {
         p += align_up(static_cast<size_t>(j.n_masks) * 2, 256);
         w->plans = reinterpret_cast<snaps::GridPlan*>(p);
         p += align_up(static_cast<size_t>(j.n_masks) * sizeof(snaps::GridPlan), 256);
-        w->radii = reinterpret_cast<float*>(p);
-        p += align_up(static_cast<size_t>(j.n_masks) * 32 * 4, 256);
         w->grid_table = p;
         p += snaps::grid_table_bytes(j.N);
         w->grid_index = p;

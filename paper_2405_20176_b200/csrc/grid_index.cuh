@@ -19,7 +19,7 @@ constexpr int kGridMasterBits = 12;
 constexpr int kGridMaster = 1 << kGridMasterBits;       // master bins per feature
 constexpr int kGridEdgeStride = kGridMaster + 1;        // edges per feature (last = column maximum)
 constexpr int kGridDims = 3;                            // grid dimensions (leading ones may be unused)
-constexpr int kGridSlackRows = 64;                      // readable rows past the end of the compact table
+constexpr int kGridSlackRows = 64;                      // spare rows at the end of the compact table (odd N: the last pair's partner)
 
 // Per mask, written by grid_plan_kernel on the device (the choice of index features depends on the
 // data) except d / bits, which the host fixes from popcount(mask) and N.
