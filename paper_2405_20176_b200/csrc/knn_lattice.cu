@@ -14,12 +14,14 @@
 //     G[u] = max of the group's four current thresholds (register-held);
 //   * COMPACT: lanes that pass any group test push (id, base, sq0..5) into a per-warp
 //     shared-memory queue (ballot + popc); with running thresholds a few % of candidates pass;
-//   * REFINE (every 32 queued candidates, all lanes busy): lane = candidate forms the 64 subset
-//     sums by add-only enumeration in a fixed order; they cross to the list owners through a
-//     32 x 32 shared-memory transpose; lane = list merges the sums below its threshold into its
-//     sorted list, held in registers for the merge (right-aligned, branch-free insert); a list is
-//     12/20/28/36 words apart from the next so that whole lists move with conflict-free 128-bit
-//     accesses; thresholds and G are refreshed;
+//   * EXACT TEST (every 32 queued candidates, lane = candidate): the 64 subset sums by add-only
+//     enumeration in a fixed order, each compared with its list's current threshold (broadcast reads);
+//     about one queued candidate in four has a sum that can enter a list -- only those wait for
+//   * REFINE (every 32 survivors, all lanes busy): lane = candidate forms the 64 sums again; they
+//     cross to the list owners through a 32 x 32 shared-memory transpose; lane = list merges the
+//     sums below its threshold into its sorted list, held in registers for the merge (right-aligned,
+//     branch-free insert); a list is 12/20/28/36 words apart from the next so that whole lists move
+//     with conflict-free 128-bit accesses; thresholds and G are refreshed;
 //   * thresholds start from an upper bound seeded by evaluating k known objects
 //     (the first k ids or the previous batch's neighbours: consecutive batches
 //     differ in one feature), tightened by min over supersets (the k-th distance
@@ -47,14 +49,17 @@ namespace snaps {
 #define MT(T, j) ws[ROWS(5) + (T) * 36 + (j)]
 #define CANDID(j) wsi[ROWS(5) + 32 * 36 + (j)]
 #define QUEUE4 (reinterpret_cast<float4*>(ws + ROWS(5) + 32 * 36 + 32))
-constexpr int kQueue = 64;   // queue entries (8 words each); refine as soon as 32 are waiting
+constexpr int kQueue = 64;   // queue entries (8 words each); exact test as soon as 32 are waiting
+// the candidates that passed the exact test wait here for the refine step, at most 32 of them: the
+// refine step takes them all into registers before it writes the transpose, so the two share storage
+#define SURV4 (reinterpret_cast<float4*>(&MT(0, 0)))
 
 __host__ __device__ constexpr int knn_list_stride(int k) { return k <= 12 ? 12 : k <= 20 ? 20 : k <= 28 ? 28 : 36; }
 __host__ __device__ constexpr int knn_warp_words(int k) {
     return 128 * knn_list_stride(k) + 5 * 64 + 32 * 36 + 32 + kQueue * 8;
 }
 
-// REFINE: lanes 0..n-1 take the n oldest queue entries and form their 64 subset sums
+// REFINE: lanes 0..n-1 take the n waiting survivors of the exact test and form their 64 subset sums
 // (lane = candidate); the sums cross to the list owners through a 32 x 32 shared-memory
 // transpose (row stride 36 words: conflict-free both ways), 32 lists at a time; then
 // lane = list: the owner compares its list's 32 new sums with its threshold and merges the
@@ -64,12 +69,22 @@ __host__ __device__ constexpr int knn_warp_words(int k) {
 // The add order (high features by FMA in feature order -> features 2,3,4,5 -> 0 -> 1) is the
 // same wherever a squared distance is formed, so a value never depends on scheduling.
 template <int S>
-__device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N, int head, int n) {
+__device__ __noinline__ void knn_refine(float* ws, int k, int lane, int n) {
     constexpr int NE = S > 32 ? 32 : S;   // list elements held (S = 36 carries 4 words of padding)
     int* wsi = reinterpret_cast<int*>(ws);
     __syncwarp();
     PairTerms pt;
-    const int cand = queue_pop(QUEUE4, kQueue, head, lane, n, q, N, pt);
+    pt.base = __int_as_float(0x7f800000);
+#pragma unroll
+    for (int j = 0; j < kLow; ++j) pt.sq[j] = 0.f;
+    int cand = -1;
+    if (lane < n) {
+        const float4 a = SURV4[lane], b = SURV4[32 + lane];
+        cand = __float_as_int(a.x);
+        pt.base = a.y; pt.sq[0] = a.z; pt.sq[1] = a.w;
+        pt.sq[2] = b.x; pt.sq[3] = b.y; pt.sq[4] = b.z; pt.sq[5] = b.w;
+    }
+    __syncwarp();   // the transpose overwrites the survivors' storage
     CANDID(lane) = cand;
     float X8[8];   // partial sums over features 2,3,4; feature 5 is added per half (same order as X[16])
     lattice_partial8(pt, X8);
@@ -147,6 +162,36 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int q, int N
         GMAX(lane) = fmaxf(fmaxf(t.x, t.y), fmaxf(t.z, t.w));
     }
     __syncwarp();
+}
+
+// EXACT TEST (between COMPACT and REFINE): the group filter lets a candidate through when a lower
+// bound of four sums is below the largest of four thresholds; most of those candidates enter no
+// list.  Lanes 0..n-1 take the n oldest queue entries (lane = candidate), form the 64 sums exactly
+// as the refine step does and compare each with its list's current threshold (16 broadcast reads);
+// only candidates with a sum below a threshold go on, in order, to the survivors' array, and the
+// refine step -- whose cost does not depend on how many of its 32 candidates enter a list -- runs
+// when 32 of them wait.  Thresholds only fall, so a candidate dropped here could never enter later.
+// When the array fills up, the entries behind the last survivor taken stay queued and are tested
+// again after the refine step.  Returns (entries consumed) | (survivors now waiting) << 8.
+template <int S>
+__device__ __noinline__ int knn_exact_test(float* ws, int lane, int q, int N, int head, int n, int nb) {
+    __syncwarp();
+    PairTerms pt;
+    const int cand = queue_pop(QUEUE4, kQueue, head, lane, n, q, N, pt);
+    float X8[8];
+    lattice_partial8(pt, X8);
+    const bool pass = lattice_any_below(pt, X8, &THR(0));
+    const unsigned sb = __ballot_sync(kFull, pass);
+    const int pos = nb + __popc(sb & ((1u << lane) - 1u));
+    const bool take = pass && pos < 32;
+    if (take) {
+        SURV4[pos] = make_float4(__int_as_float(cand), pt.base, pt.sq[0], pt.sq[1]);
+        SURV4[32 + pos] = make_float4(pt.sq[2], pt.sq[3], pt.sq[4], pt.sq[5]);
+    }
+    const int tot = nb + __popc(sb);
+    if (tot <= 32) return n | (tot << 8);
+    const unsigned last = __ballot_sync(kFull, take && pos == 31);
+    return __ffs(last) | (32 << 8);
 }
 
 // Upper bounds on the final k-th squared distance of every list of the new batch.
@@ -305,6 +350,7 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             float G[16];
             RELOAD_G();
             int qhead = 0, qtail = 0;  // queue positions (warp-uniform, monotone)
+            int nsurv = 0;             // candidates waiting for the refine step
             // candidates: block t = rows 32t..32t+31, lane = row, four coalesced 128-bit loads;
             // two register sets alternate (one in use, one in flight) -- no register moves
 #define FILTER_BLOCK(r, t_)                                                                   \
@@ -314,10 +360,15 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
         const unsigned bal = __ballot_sync(kFull, pass);                                      \
         if (bal) {                                                                            \
             qtail += queue_push(QUEUE4, kQueue, qtail, pass, bal, lt, (t_) * 32 + lane, pt);  \
-            if (qtail - qhead >= 32) {                                                        \
-                knn_refine<S>(ws, k, lane, q, p.N, qhead, 32);                                \
-                qhead += 32;                                                                  \
-                RELOAD_G();                                                                   \
+            while (qtail - qhead >= 32) {                                                     \
+                const int r_ = knn_exact_test<S>(ws, lane, q, p.N, qhead, 32, nsurv);         \
+                qhead += r_ & 0xff;                                                           \
+                nsurv = r_ >> 8;                                                              \
+                if (nsurv == 32) {                                                            \
+                    knn_refine<S>(ws, k, lane, 32);                                           \
+                    nsurv = 0;                                                                \
+                    RELOAD_G();                                                               \
+                }                                                                             \
             }                                                                                 \
         }                                                                                     \
     }
@@ -341,7 +392,16 @@ __global__ void __launch_bounds__(kKnnMaxThreads, 1) knn_lattice_kernel(const Kn
             if ((SLOT(0) < 0) & (SLOT(1) < 0) & (SLOT(2) < 0)) stream_table(TrueTag{});
             else stream_table(FalseTag{});
 #undef FILTER_BLOCK
-            if (qtail > qhead) knn_refine<S>(ws, k, lane, q, p.N, qhead, qtail - qhead);
+            while (qtail > qhead) {
+                const int r = knn_exact_test<S>(ws, lane, q, p.N, qhead, min(32, qtail - qhead), nsurv);
+                qhead += r & 0xff;
+                nsurv = r >> 8;
+                if (nsurv == 32) {
+                    knn_refine<S>(ws, k, lane, 32);
+                    nsurv = 0;
+                }
+            }
+            if (nsurv) knn_refine<S>(ws, k, lane, nsurv);
             knn_emit<S>(ws, p, q, lane);
             has_prev = true;
         }

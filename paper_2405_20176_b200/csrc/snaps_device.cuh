@@ -33,13 +33,18 @@ struct alignas(16) BatchDesc {
 };
 static_assert(sizeof(BatchDesc) % 16 == 0, "BatchDesc rows are read with 128-bit loads");
 
-// Squared distance on a runtime mask from two staged rows (slow paths only).
-__device__ __forceinline__ float masked_d2(const float* __restrict__ a, const float* __restrict__ b,
-                                           uint32_t mask) {
+// Squared distance on a runtime mask between a staged row in global memory (80 bytes, 16-byte
+// aligned: four 128-bit loads cover the 15 features) and a query row held in registers; features
+// added in ascending order (slow paths only).
+__device__ __forceinline__ float masked_d2(const float* __restrict__ row, const float (&q)[15], uint32_t mask) {
+    const float4* r4 = reinterpret_cast<const float4*>(row);
+    const float4 a0 = __ldg(r4), a1 = __ldg(r4 + 1), a2 = __ldg(r4 + 2), a3 = __ldg(r4 + 3);
+    const float a[16] = {a0.x, a0.y, a0.z, a0.w, a1.x, a1.y, a1.z, a1.w,
+                         a2.x, a2.y, a2.z, a2.w, a3.x, a3.y, a3.z, a3.w};
     float acc = 0.f;
 #pragma unroll
     for (int j = 0; j < 15; ++j) {
-        float diff = a[j] - b[j];
+        float diff = a[j] - q[j];
         float sq = __fmul_rn(diff, diff);
         if ((mask >> j) & 1u) acc = __fadd_rn(acc, sq);
     }
@@ -186,14 +191,15 @@ __device__ __forceinline__ bool lattice_filter(const Blk& r, const FilterQuery& 
     return pa | pb;
 }
 
-// COMPACT: the lanes that passed append (id, base, sq0..5) to the warp's queue of 8-word entries.
-// Returns the number of entries appended (warp-uniform).
+// COMPACT: the lanes that passed append (id, base, sq0..5) to the warp's queue of 8-word entries,
+// kept as two arrays of 128-bit halves (queue[slot], queue[queue_len + slot]) so that consecutive
+// slots are 16 bytes apart: conflict-free 128-bit accesses.  Returns the number appended (warp-uniform).
 __device__ __forceinline__ int queue_push(float4* queue, int queue_len, int qtail, bool pass, unsigned bal,
                                           unsigned lanes_below, int cand, const PairTerms& t) {
     if (pass) {
-        float4* e = queue + 2 * ((qtail + __popc(bal & lanes_below)) % queue_len);
+        float4* e = queue + (qtail + __popc(bal & lanes_below)) % queue_len;
         e[0] = make_float4(__int_as_float(cand), t.base, t.sq[0], t.sq[1]);
-        e[1] = make_float4(t.sq[2], t.sq[3], t.sq[4], t.sq[5]);
+        e[queue_len] = make_float4(t.sq[2], t.sq[3], t.sq[4], t.sq[5]);
     }
     return __popc(bal);
 }
@@ -210,19 +216,43 @@ __device__ __forceinline__ void lattice_partial8(const PairTerms& t, float (&X8)
     }
 }
 
+// The four sums of group 4*uu (+ 32*half) in that order: lattice subsets T = 4*uu + {0, 1, 2, 3}.
+__device__ __forceinline__ void lattice_group_sums(const PairTerms& t, const float (&X8)[8], int half, int uu,
+                                                   float& s0, float& s1, float& s2, float& s3) {
+    s0 = half ? __fadd_rn(X8[uu], t.sq[5]) : X8[uu];
+    s1 = __fadd_rn(s0, t.sq[0]);
+    s2 = __fadd_rn(s0, t.sq[1]);
+    s3 = __fadd_rn(s1, t.sq[1]);
+}
+
 __device__ __forceinline__ void lattice_sums_to_transpose(const PairTerms& t, const float (&X8)[8], int half,
                                                           float* mt, int lane) {
 #pragma unroll
     for (int uu = 0; uu < 8; ++uu) {
-        const float s0 = half ? __fadd_rn(X8[uu], t.sq[5]) : X8[uu];
-        const float s1 = __fadd_rn(s0, t.sq[0]);
-        const float s2 = __fadd_rn(s0, t.sq[1]);
-        const float s3 = __fadd_rn(s1, t.sq[1]);
+        float s0, s1, s2, s3;
+        lattice_group_sums(t, X8, half, uu, s0, s1, s2, s3);
         mt[(4 * uu + 0) * 36 + lane] = s0;
         mt[(4 * uu + 1) * 36 + lane] = s1;
         mt[(4 * uu + 2) * 36 + lane] = s2;
         mt[(4 * uu + 3) * 36 + lane] = s3;
     }
+}
+
+// Whether any of a candidate's 64 sums is below its list's threshold (thr[T], T = 0..63, read as
+// 128-bit broadcasts): the same values, formed in the same order, as the refine step compares.
+__device__ __forceinline__ bool lattice_any_below(const PairTerms& t, const float (&X8)[8], const float* thr) {
+    bool pass = false;
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {
+#pragma unroll
+        for (int uu = 0; uu < 8; ++uu) {
+            float s0, s1, s2, s3;
+            lattice_group_sums(t, X8, half, uu, s0, s1, s2, s3);
+            const float4 h = *reinterpret_cast<const float4*>(thr + 32 * half + 4 * uu);
+            pass |= (s0 < h.x) | (s1 < h.y) | (s2 < h.z) | (s3 < h.w);
+        }
+    }
+    return pass;
 }
 
 // The entry a lane takes from the queue at refine time; self (reading A4) and padding rows (A19)
@@ -234,8 +264,8 @@ __device__ __forceinline__ int queue_pop(const float4* queue, int queue_len, int
     for (int j = 0; j < kLow; ++j) t.sq[j] = 0.f;
     int cand = -1;
     if (lane < n) {
-        const float4* e = queue + 2 * ((head + lane) % queue_len);
-        const float4 a = e[0], b = e[1];
+        const float4* e = queue + (head + lane) % queue_len;
+        const float4 a = e[0], b = e[queue_len];
         cand = __float_as_int(a.x);
         t.base = a.y; t.sq[0] = a.z; t.sq[1] = a.w;
         t.sq[2] = b.x; t.sq[3] = b.y; t.sq[4] = b.z; t.sq[5] = b.w;
