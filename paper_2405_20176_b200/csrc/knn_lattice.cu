@@ -74,16 +74,7 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int n) {
     int* wsi = reinterpret_cast<int*>(ws);
     __syncwarp();
     PairTerms pt;
-    pt.base = __int_as_float(0x7f800000);
-#pragma unroll
-    for (int j = 0; j < kLow; ++j) pt.sq[j] = 0.f;
-    int cand = -1;
-    if (lane < n) {
-        const float4 a = SURV4[lane], b = SURV4[32 + lane];
-        cand = __float_as_int(a.x);
-        pt.base = a.y; pt.sq[0] = a.z; pt.sq[1] = a.w;
-        pt.sq[2] = b.x; pt.sq[3] = b.y; pt.sq[4] = b.z; pt.sq[5] = b.w;
-    }
+    const int cand = survivors_pop(SURV4, lane, n, pt);
     __syncwarp();   // the transpose overwrites the survivors' storage
     CANDID(lane) = cand;
     float X8[8];   // partial sums over features 2,3,4; feature 5 is added per half (same order as X[16])
@@ -164,34 +155,11 @@ __device__ __noinline__ void knn_refine(float* ws, int k, int lane, int n) {
     __syncwarp();
 }
 
-// EXACT TEST (between COMPACT and REFINE): the group filter lets a candidate through when a lower
-// bound of four sums is below the largest of four thresholds; most of those candidates enter no
-// list.  Lanes 0..n-1 take the n oldest queue entries (lane = candidate), form the 64 sums exactly
-// as the refine step does and compare each with its list's current threshold (16 broadcast reads);
-// only candidates with a sum below a threshold go on, in order, to the survivors' array, and the
-// refine step -- whose cost does not depend on how many of its 32 candidates enter a list -- runs
-// when 32 of them wait.  Thresholds only fall, so a candidate dropped here could never enter later.
-// When the array fills up, the entries behind the last survivor taken stay queued and are tested
-// again after the refine step.  Returns (entries consumed) | (survivors now waiting) << 8.
+// EXACT TEST of 32 queued candidates against the 64 current thresholds (snaps_device.cuh).
 template <int S>
 __device__ __noinline__ int knn_exact_test(float* ws, int lane, int q, int N, int head, int n, int nb) {
     __syncwarp();
-    PairTerms pt;
-    const int cand = queue_pop(QUEUE4, kQueue, head, lane, n, q, N, pt);
-    float X8[8];
-    lattice_partial8(pt, X8);
-    const bool pass = lattice_any_below(pt, X8, &THR(0));
-    const unsigned sb = __ballot_sync(kFull, pass);
-    const int pos = nb + __popc(sb & ((1u << lane) - 1u));
-    const bool take = pass && pos < 32;
-    if (take) {
-        SURV4[pos] = make_float4(__int_as_float(cand), pt.base, pt.sq[0], pt.sq[1]);
-        SURV4[32 + pos] = make_float4(pt.sq[2], pt.sq[3], pt.sq[4], pt.sq[5]);
-    }
-    const int tot = nb + __popc(sb);
-    if (tot <= 32) return n | (tot << 8);
-    const unsigned last = __ballot_sync(kFull, take && pos == 31);
-    return __ffs(last) | (32 << 8);
+    return lattice_exact_test(QUEUE4, kQueue, SURV4, &THR(0), lane, q, N, head, n, nb);
 }
 
 // Upper bounds on the final k-th squared distance of every list of the new batch.

@@ -9,7 +9,9 @@
 //   * FILTER: the 16 partial sums X[u] over features 2..5 are lower bounds of their group's four
 //     sums, so a candidate can be an eps-neighbour in group u only if X[u] < G[u] = the group's
 //     largest eps^2 (constants per batch, register-held);
-//   * COMPACT passing candidates into a per-warp queue; REFINE every 32 of them: lane = candidate
+//   * COMPACT passing candidates into a per-warp queue; EXACT TEST every 32 of them (lane = candidate:
+//     the 64 subset sums against the 64 thresholds, snaps_device.cuh); REFINE every 32 candidates
+//     that have a sum below a threshold: lane = candidate
 //     forms the 64 subset sums (add-only, fixed order), a 32 x 32 shared-memory transpose hands
 //     them to the list owners (lane = list), which count the sums below eps^2 with one popcount
 //     and add sqrt(d^2) of the hits to the list's running sum in candidate order (deterministic;
@@ -18,7 +20,7 @@
 
 namespace snaps {
 
-constexpr int kRQueue = 64;  // queue entries of 8 words; refine as soon as 32 are waiting
+constexpr int kRQueue = 64;  // queue entries of 8 words; exact test as soon as 32 are waiting
 
 // per-warp shared-memory words
 #define R_THR(L) ws[(L)]
@@ -28,15 +30,24 @@ constexpr int kRQueue = 64;  // queue entries of 8 words; refine as soon as 32 a
 #define R_QROW(j) ws[256 + (j)]
 #define R_MT(T, j) ws[272 + (T) * 36 + (j)]
 #define R_QUEUE4 (reinterpret_cast<float4*>(ws + 272 + 32 * 36))
+// survivors of the exact test (at most 32): taken into registers before the transpose is written
+#define R_SURV4 (reinterpret_cast<float4*>(&R_MT(0, 0)))
 
 __host__ __device__ constexpr int range_warp_words() { return 272 + 32 * 36 + kRQueue * 8; }
 
+// self (A4) and padding rows (A19) get an infinite base when they leave the queue: they never count
+__device__ __noinline__ int range_exact_test(float* ws, int lane, int q, int N, int head, int n, int nb) {
+    __syncwarp();
+    return lattice_exact_test(R_QUEUE4, kRQueue, R_SURV4, &R_THR(0), lane, q, N, head, n, nb);
+}
+
 template <bool WITH_SUM>
-__device__ __noinline__ void range_refine(float* ws, int lane, int q, int N, int head, int n) {
+__device__ __noinline__ void range_refine(float* ws, int lane, int n) {
     int* wsi = reinterpret_cast<int*>(ws);
     __syncwarp();
     PairTerms pt;
-    queue_pop(R_QUEUE4, kRQueue, head, lane, n, q, N, pt);   // self (A4) and padding rows (A19) never count
+    survivors_pop(R_SURV4, lane, n, pt);
+    __syncwarp();   // the transpose overwrites the survivors' storage
     float X8[8];   // partial sums over features 2,3,4; feature 5 is added per half
     lattice_partial8(pt, X8);
 #pragma unroll
@@ -122,7 +133,7 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
                 const float4 t = *reinterpret_cast<const float4*>(&R_THR(4 * u));
                 G[u] = fmaxf(fmaxf(t.x, t.y), fmaxf(t.z, t.w));
             }
-            int qhead = 0, qtail = 0;
+            int qhead = 0, qtail = 0, nsurv = 0;
 #define FILTER_BLOCK(r, t_)                                                                   \
     {                                                                                         \
         PairTerms pt;                                                                         \
@@ -130,9 +141,14 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
         const unsigned bal = __ballot_sync(kFull, pass);                                      \
         if (bal) {                                                                            \
             qtail += queue_push(R_QUEUE4, kRQueue, qtail, pass, bal, lt, (t_) * 32 + lane, pt); \
-            if (qtail - qhead >= 32) {                                                        \
-                range_refine<WITH_SUM>(ws, lane, q, p.N, qhead, 32);                          \
-                qhead += 32;                                                                  \
+            while (qtail - qhead >= 32) {                                                     \
+                const int r_ = range_exact_test(ws, lane, q, p.N, qhead, 32, nsurv);          \
+                qhead += r_ & 0xff;                                                           \
+                nsurv = r_ >> 8;                                                              \
+                if (nsurv == 32) {                                                            \
+                    range_refine<WITH_SUM>(ws, lane, 32);                                     \
+                    nsurv = 0;                                                                \
+                }                                                                             \
             }                                                                                 \
         }                                                                                     \
     }
@@ -156,7 +172,16 @@ __global__ void __launch_bounds__(kRangeMaxThreads, 1) range_lattice_kernel(cons
             if ((R_SLOT(0) < 0) & (R_SLOT(1) < 0) & (R_SLOT(2) < 0)) stream_table(TrueTag{});
             else stream_table(FalseTag{});
 #undef FILTER_BLOCK
-            if (qtail > qhead) range_refine<WITH_SUM>(ws, lane, q, p.N, qhead, qtail - qhead);
+            while (qtail > qhead) {
+                const int r = range_exact_test(ws, lane, q, p.N, qhead, min(32, qtail - qhead), nsurv);
+                qhead += r & 0xff;
+                nsurv = r >> 8;
+                if (nsurv == 32) {
+                    range_refine<WITH_SUM>(ws, lane, 32);
+                    nsurv = 0;
+                }
+            }
+            if (nsurv) range_refine<WITH_SUM>(ws, lane, nsurv);
             // ---- a7: counts, sums, means (0 when there is no neighbour: PAPER.md:266, reading A6)
             __syncwarp();
 #pragma unroll

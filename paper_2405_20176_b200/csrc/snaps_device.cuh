@@ -274,4 +274,49 @@ __device__ __forceinline__ int queue_pop(const float4* queue, int queue_len, int
     return cand;
 }
 
+// EXACT TEST (between COMPACT and REFINE): the group filter lets a candidate through when a lower
+// bound of four sums is below the largest of four thresholds; most of those candidates enter no
+// list.  Lanes 0..n-1 take the n oldest queue entries (lane = candidate), form the 64 sums exactly
+// as the refine step does and compare each with its list's current threshold thr[T] (16 broadcast
+// reads); only candidates with a sum below a threshold go on, in order, to the survivors' array
+// surv (32 entries as two arrays of 128-bit halves; nb of them already wait), and the refine step
+// -- whose cost does not depend on how many of its 32 candidates count -- runs when 32 of them
+// wait.  Thresholds never rise, so a candidate dropped here could not count later.  When the array
+// fills up, the entries behind the last survivor taken stay queued and are tested again after the
+// refine step.  Returns (entries consumed) | (survivors now waiting) << 8.
+__device__ __forceinline__ int lattice_exact_test(const float4* queue, int queue_len, float4* surv, const float* thr,
+                                                  int lane, int q, int N, int head, int n, int nb) {
+    PairTerms pt;
+    const int cand = queue_pop(queue, queue_len, head, lane, n, q, N, pt);
+    float X8[8];
+    lattice_partial8(pt, X8);
+    const bool pass = lattice_any_below(pt, X8, thr);
+    const unsigned sb = __ballot_sync(kFull, pass);
+    const int pos = nb + __popc(sb & ((1u << lane) - 1u));
+    const bool take = pass && pos < 32;
+    if (take) {
+        surv[pos] = make_float4(__int_as_float(cand), pt.base, pt.sq[0], pt.sq[1]);
+        surv[32 + pos] = make_float4(pt.sq[2], pt.sq[3], pt.sq[4], pt.sq[5]);
+    }
+    const int tot = nb + __popc(sb);
+    if (tot <= 32) return n | (tot << 8);
+    const unsigned last = __ballot_sync(kFull, take && pos == 31);
+    return __ffs(last) | (32 << 8);
+}
+
+// The survivor a lane takes at refine time (lanes >= n: an infinite base, no sum can pass).
+__device__ __forceinline__ int survivors_pop(const float4* surv, int lane, int n, PairTerms& t) {
+    t.base = __int_as_float(0x7f800000);
+#pragma unroll
+    for (int j = 0; j < kLow; ++j) t.sq[j] = 0.f;
+    int cand = -1;
+    if (lane < n) {
+        const float4 a = surv[lane], b = surv[32 + lane];
+        cand = __float_as_int(a.x);
+        t.base = a.y; t.sq[0] = a.z; t.sq[1] = a.w;
+        t.sq[2] = b.x; t.sq[3] = b.y; t.sq[4] = b.z; t.sq[5] = b.w;
+    }
+    return cand;
+}
+
 }  // namespace snaps
