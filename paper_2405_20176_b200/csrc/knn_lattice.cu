@@ -182,10 +182,15 @@ __device__ __noinline__ void knn_seed(float* ws, const float* __restrict__ Xp, i
             // (consecutive batches differ in one feature) if that list is full, else the first k ids
             const bool from_prev = has_prev && L_D2(NE - 1, L) < __int_as_float(0x7f800000);
             float b1 = 0.f;
+            // two rows in flight per lane: the loads are scattered (L2 latency) and nothing else hides them
 #pragma unroll 1
-            for (int e = 0; e < k; ++e) {
-                const int c = from_prev ? L_ID(NE - k + e, L) : e + (e >= q ? 1 : 0);
-                b1 = fmaxf(b1, masked_d2(Xp + static_cast<size_t>(c) * kRowFloats, qrow, mask));
+            for (int e = 0; e < k; e += 2) {
+                const int e1 = min(e + 1, k - 1);
+                const int c0 = from_prev ? L_ID(NE - k + e, L) : e + (e >= q ? 1 : 0);
+                const int c1 = from_prev ? L_ID(NE - k + e1, L) : e1 + (e1 >= q ? 1 : 0);
+                const float d0 = masked_d2(Xp + static_cast<size_t>(c0) * kRowFloats, qrow, mask);
+                const float d1 = masked_d2(Xp + static_cast<size_t>(c1) * kRowFloats, qrow, mask);
+                b1 = fmaxf(b1, fmaxf(d0, d1));
             }
             bound = b1;
             // the stream re-evaluates these objects in another summation order: leave

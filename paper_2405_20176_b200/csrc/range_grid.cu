@@ -2,8 +2,9 @@
 // the result set of eps_max contains the result sets of every smaller eps_j, so the join runs once
 // at eps_max and each neighbour is binned by the smallest grid radius that contains it; cumulative
 // sums over the bins give the count and the distance sum for every eps_j.
-// Same filter / compact / refine structure as range_lattice.cu; the list owner keeps a
-// per-radius histogram (count, sum of distances) in shared memory.
+// Same filter / compact / exact test / refine structure as range_lattice.cu (the exact test is
+// against the largest radius of every list); the list owner keeps a per-radius histogram
+// (count, sum of distances) in shared memory.
 #include "range_grid.cuh"
 
 namespace snaps {
@@ -11,23 +12,32 @@ namespace snaps {
 constexpr int kGQueue = 64;
 
 // per-warp shared-memory words; G = number of radii (runtime)
-//   SLOT[64] | QROW[16] | MT 32x36 | queue 64x8 | THR[64][G] | HCNT[64][G] | HSUM[64][G]
+//   SLOT[64] | QROW[16] | MT 32x36 | queue 64x8 | TMAX[64] | THR[64][G] | HCNT[64][G] | HSUM[64][G]
 #define G_SLOT(L) wsi[(L)]
 #define G_MT(T, j) ws[80 + (T) * 36 + (j)]
 #define G_QUEUE4 (reinterpret_cast<float4*>(ws + 80 + 32 * 36))
-#define G_BASE (80 + 32 * 36 + kGQueue * 8)
+// survivors of the exact test (at most 32): taken into registers before the transpose is written
+#define G_SURV4 (reinterpret_cast<float4*>(&G_MT(0, 0)))
+#define G_TMAX(L) ws[80 + 32 * 36 + kGQueue * 8 + (L)]   // the largest radius of list L (-1: unused slot)
+#define G_BASE (80 + 32 * 36 + kGQueue * 8 + 64)
 #define G_THR(L, g) ws[G_BASE + (L) * G + (g)]
 #define G_HCNT(L, g) wsi[G_BASE + 64 * G + (L) * G + (g)]
 #define G_HSUM(L, g) ws[G_BASE + 128 * G + (L) * G + (g)]
 
 __host__ __device__ inline int range_grid_warp_words(int G) { return G_BASE + 192 * G; }
 
-__device__ __noinline__ void range_grid_refine(float* ws, int G, bool with_sum, int lane, int q, int N, int head,
-                                               int n) {
+// self by index (A4) and padding rows (A19) get an infinite base when they leave the queue
+__device__ __noinline__ int range_grid_exact_test(float* ws, int lane, int q, int N, int head, int n, int nb) {
+    __syncwarp();
+    return lattice_exact_test(G_QUEUE4, kGQueue, G_SURV4, &G_TMAX(0), lane, q, N, head, n, nb);
+}
+
+__device__ __noinline__ void range_grid_refine(float* ws, int G, bool with_sum, int lane, int n) {
     int* wsi = reinterpret_cast<int*>(ws);
     __syncwarp();
     PairTerms pt;
-    queue_pop(G_QUEUE4, kGQueue, head, lane, n, q, N, pt);   // self by index (A4), padding rows (A19)
+    survivors_pop(G_SURV4, lane, n, pt);
+    __syncwarp();   // the transpose overwrites the survivors' storage
     float X8[8];
     lattice_partial8(pt, X8);
 #pragma unroll
@@ -35,7 +45,7 @@ __device__ __noinline__ void range_grid_refine(float* ws, int G, bool with_sum, 
         lattice_sums_to_transpose(pt, X8, half, &G_MT(0, 0), lane);
         __syncwarp();
         const int T = 32 * half + lane;
-        const float thr = G_THR(T, G - 1);   // the largest radius of this list (-1 for unused slots)
+        const float thr = G_TMAX(T);
         unsigned mask = 0u;
 #pragma unroll
         for (int j4 = 0; j4 < 8; ++j4) {
@@ -99,6 +109,7 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
                 G_HCNT(L, g) = 0;
                 G_HSUM(L, g) = 0.f;
             }
+            G_TMAX(L) = G_THR(L, G - 1);
         }
         __syncwarp();
         filter_query_init(fq, qhi, H);
@@ -106,9 +117,8 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
         float Gm[16];
 #pragma unroll
         for (int u = 0; u < 16; ++u)
-            Gm[u] = fmaxf(fmaxf(G_THR(4 * u, G - 1), G_THR(4 * u + 1, G - 1)),
-                          fmaxf(G_THR(4 * u + 2, G - 1), G_THR(4 * u + 3, G - 1)));
-        int qhead = 0, qtail = 0;
+            Gm[u] = fmaxf(fmaxf(G_TMAX(4 * u), G_TMAX(4 * u + 1)), fmaxf(G_TMAX(4 * u + 2), G_TMAX(4 * u + 3)));
+        int qhead = 0, qtail = 0, nsurv = 0;
         Blk nx;
         load_block(nx, p.Xb, 0, lane);
 #pragma unroll 1
@@ -120,13 +130,27 @@ __global__ void __launch_bounds__(kRangeGridMaxThreads, 1) range_grid_kernel(con
             const unsigned bal = __ballot_sync(kFull, pass);
             if (bal) {
                 qtail += queue_push(G_QUEUE4, kGQueue, qtail, pass, bal, lt, t * 32 + lane, pt);
-                if (qtail - qhead >= 32) {
-                    range_grid_refine(ws, G, with_sum, lane, q, p.N, qhead, 32);
-                    qhead += 32;
+                while (qtail - qhead >= 32) {
+                    const int r_ = range_grid_exact_test(ws, lane, q, p.N, qhead, 32, nsurv);
+                    qhead += r_ & 0xff;
+                    nsurv = r_ >> 8;
+                    if (nsurv == 32) {
+                        range_grid_refine(ws, G, with_sum, lane, 32);
+                        nsurv = 0;
+                    }
                 }
             }
         }
-        if (qtail > qhead) range_grid_refine(ws, G, with_sum, lane, q, p.N, qhead, qtail - qhead);
+        while (qtail > qhead) {
+            const int r_ = range_grid_exact_test(ws, lane, q, p.N, qhead, min(32, qtail - qhead), nsurv);
+            qhead += r_ & 0xff;
+            nsurv = r_ >> 8;
+            if (nsurv == 32) {
+                range_grid_refine(ws, G, with_sum, lane, 32);
+                nsurv = 0;
+            }
+        }
+        if (nsurv) range_grid_refine(ws, G, with_sum, lane, nsurv);
         // cumulative over the radii: count(eps_g) = sum of the bins <= g
         __syncwarp();
         for (int h = 0; h < 2; ++h) {
