@@ -325,6 +325,8 @@ def run_range(args, cfg, snaps, torch, D, steps, warmup, peakinfo, emit=True):
     X = workloads.make_table(cfg.n, cfg.seed, cols=list(range(cfg.n_feat)), outlier_frac=0.01)
     masks_all = cfg.masks()
     eps_all = workloads.config_eps(cfg.name, masks_all)        # stored inputs (oracle/write_config_eps.py)
+    if args.masks_limit > 0:                                   # ncu captures only: not a bench value
+        masks_all, eps_all = masks_all[:args.masks_limit], eps_all[:args.masks_limit]
     mine = shard_masks(masks_all, D.rank, D.world)
     masks, eps = masks_all[mine], eps_all[mine]
     N, n_masks = len(X), len(masks_all)
@@ -359,6 +361,7 @@ def run_range(args, cfg, snaps, torch, D, steps, warmup, peakinfo, emit=True):
     evals = float(N) * N * len(masks)            # this rank's share (the kernel time is this rank's)
     n_batches = float(snaps.planned_evals(N, X.shape[1], masks)) / (64.0 * N * N)
     line = {
+        **({"partial": f"first {args.masks_limit} masks only (--masks-limit): not a bench value"} if args.masks_limit > 0 else {}),
         "metric": "subspaces/sec (DSSJ N=31,693, eps_d for ~50 neighbours)", "value": n_masks / (ms * 1e-3),
         "unit": UNIT, "n_gpus": D.world, "steps": steps, "warmup": warmup, "ms_per_step": ms,
         "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",

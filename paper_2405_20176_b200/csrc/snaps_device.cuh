@@ -197,7 +197,7 @@ __device__ __forceinline__ bool lattice_filter(const Blk& r, const FilterQuery& 
 __device__ __forceinline__ int queue_push(float4* queue, int queue_len, int qtail, bool pass, unsigned bal,
                                           unsigned lanes_below, int cand, const PairTerms& t) {
     if (pass) {
-        float4* e = queue + (qtail + __popc(bal & lanes_below)) % queue_len;
+        float4* e = queue + (static_cast<unsigned>(qtail + __popc(bal & lanes_below)) % static_cast<unsigned>(queue_len));
         e[0] = make_float4(__int_as_float(cand), t.base, t.sq[0], t.sq[1]);
         e[queue_len] = make_float4(t.sq[2], t.sq[3], t.sq[4], t.sq[5]);
     }
@@ -264,7 +264,7 @@ __device__ __forceinline__ int queue_pop(const float4* queue, int queue_len, int
     for (int j = 0; j < kLow; ++j) t.sq[j] = 0.f;
     int cand = -1;
     if (lane < n) {
-        const float4* e = queue + (head + lane) % queue_len;
+        const float4* e = queue + (static_cast<unsigned>(head + lane) % static_cast<unsigned>(queue_len));
         const float4 a = e[0], b = e[queue_len];
         cand = __float_as_int(a.x);
         t.base = a.y; t.sq[0] = a.z; t.sq[1] = a.w;
