@@ -27,12 +27,17 @@ namespace snaps {
 
 namespace {
 
-constexpr int kWarps = 8;            // warps per CTA at most (independent; fewer when the heaps are large)
+constexpr int MODE_KNN = 0, MODE_RANGE = 1, MODE_RANGE_GRID = 2, MODE_KNN_BIG = 3;
+
+// Warps per CTA.  The warps are independent and their running times differ widely (a warp of outliers
+// walks many more rows), so a CTA holds its registers and shared memory until its slowest warp is done:
+// with 8 warps per CTA 12.6 warps per SM were active on average where 16-24 fit.  Measured on config 5's
+// masks at N = 10^6 (join kernels, 64 masks): kNN 9.04 s with 8 warps, 7.45 s with 2, 6.83 s with 1;
+// DSSJ 2.46 / 1.92 / 1.99 s.
+__host__ __device__ constexpr int warps_per_cta(int mode) { return (mode == MODE_KNN || mode == MODE_KNN_BIG) ? 1 : 2; }
 constexpr int kTile = 64;            // candidates per tile
 constexpr int kSeedHalf = 112;       // seed window: this many sorted positions either side of the warp
 constexpr int kMaxG = 32;
-
-constexpr int MODE_KNN = 0, MODE_RANGE = 1, MODE_RANGE_GRID = 2, MODE_KNN_BIG = 3;
 
 __host__ __device__ constexpr int dp_of(int d) { return (d + 3) / 4 * 4; }
 
@@ -101,7 +106,7 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
 }
 
 template <int D, int MODE>
-__global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinParams p) {
+__global__ void __launch_bounds__(warps_per_cta(MODE) * 32) grid_join_kernel(const GridJoinParams p) {
     constexpr int DP = dp_of(D);
     constexpr int G4 = DP / 2;                     // float4 per pair of candidates: two columns x two objects
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -436,7 +441,7 @@ __global__ void __launch_bounds__(kWarps * 32) grid_join_kernel(const GridJoinPa
 template <int MODE, int D>
 cudaError_t launch_d(const GridJoinParams& p, cudaStream_t st) {
     const size_t per_warp = static_cast<size_t>(warp_words(D, MODE, p.k, p.G)) * 4;
-    int wpc = kWarps;
+    int wpc = warps_per_cta(MODE);
     while (wpc > 1 && wpc * per_warp > 200 * 1024) --wpc;
     const size_t smem = wpc * per_warp;
     auto kernel = grid_join_kernel<D, MODE>;
