@@ -138,6 +138,33 @@ snaps_status snaps_knn_selfjoin(const float *d_X, int64_t N, int n_feat, int64_t
                                 void *d_workspace, size_t workspace_bytes, void *stream);
 
 /*
+ * The same kNN self-join (scores of PAPER.md:251-252) for callers that cannot
+ * allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): no workspace argument.  The staged copies of the table, the work counter and the batch
+ * descriptors of the sub-lattice engine live in a fixed array of SNAPS_STATIC_SCRATCH_BYTES (5.8 MB)
+ * inside the library, which every GPU that loads the library holds until the process exits.  The call
+ * allocates nothing on the device (no cudaMalloc / cudaFree / allocating library routine).
+ *
+ * Arguments as snaps_knn_selfjoin with q_begin = 0, q_end = N, the sub-lattice engine, and
+ *   N        2 <= N <= SNAPS_STATIC_MAX_N (32,768: SNAPShot1's 31,693 objects fit)
+ *   n_masks  1 <= n_masks <= SNAPS_STATIC_MAX_MASKS (2,048)
+ *   k        1 <= k <= min(N-1, SNAPS_LATTICE_MAX_K)
+ *   d_X      device only.
+ * Larger sizes are rejected with SNAPS_UNSUPPORTED and a message that names the limit; results are
+ * identical to snaps_knn_selfjoin's (same kernels).  Every call on a device shares the one array: it
+ * keeps the last call's contents (each call rewrites all it reads and zeroes the work counter), and
+ * two calls that overlap on the same GPU -- different streams, different threads -- race; serialise them.
+ */
+#define SNAPS_STATIC_MAX_N 32768
+#define SNAPS_STATIC_MAX_MASKS 2048
+#define SNAPS_STATIC_SCRATCH_BYTES 5800192
+snaps_status snaps_knn_selfjoin_static(const float *d_X, int64_t N, int n_feat, int64_t ld,
+                                       const uint16_t *h_masks, int n_masks, int k,
+                                       int32_t *out_idx, float *out_dist,
+                                       float *out_kth, float *out_mean, int32_t *out_indeg,
+                                       void *stream);
+
+/*
  * eps range self-join, DSSJ (section 3.5): for
  * every mask S and query object i in [q_begin, q_end), the objects j != i with
  * D(i,j;S) <= eps_S (closed ball, reading A2; pairs within 1e-6 relative of eps

@@ -10,7 +10,7 @@ from . import build as _build
 
 EXPORTED_SYMBOLS = [
     "snaps_last_error", "snaps_version", "snaps_workspace_bytes", "snaps_planned_evals",
-    "snaps_knn_selfjoin", "snaps_range_selfjoin", "snaps_outlier_scores",
+    "snaps_knn_selfjoin", "snaps_knn_selfjoin_static", "snaps_range_selfjoin", "snaps_outlier_scores",
     "snaps_stream_ring_bytes", "snaps_knn_selfjoin_streamed", "snaps_sink_batch_bytes",
     "snaps_knn_selfjoin_sink", "snaps_range_selfjoin_sink", "snaps_probe_fp32_rate",
     "snaps_profile_enable", "snaps_profile_last_kernel_ms",
@@ -73,6 +73,8 @@ def lib():
         L.snaps_planned_evals.argtypes = [i64, i32, vp, i32]
         L.snaps_knn_selfjoin.restype = i32
         L.snaps_knn_selfjoin.argtypes = [vp, i64, i32, i64, vp, i32, i32, i64, i64, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+        L.snaps_knn_selfjoin_static.restype = i32
+        L.snaps_knn_selfjoin_static.argtypes = [vp, i64, i32, i64, vp, i32, i32, vp, vp, vp, vp, vp, vp]
         L.snaps_range_selfjoin.restype = i32
         L.snaps_range_selfjoin.argtypes = [vp, i64, i32, i64, vp, i32, vp, i64, i64, i32, vp, vp, vp, vp, sz, vp]
         L.snaps_outlier_scores.restype = i32
@@ -216,6 +218,35 @@ def knn_selfjoin(X, masks, k, *, lists=True, scores=True, out=None, workspace=No
         _dptr(out.get("idx")), _dptr(out.get("dist")), _dptr(out.get("kth")),
         _dptr(out.get("mean")), _dptr(out.get("indeg")), _dptr(ws), ws.numel(), _stream(stream)))
     out["_workspace"] = ws
+    return out
+
+
+STATIC_MAX_N = 32768          # SNAPS_STATIC_MAX_N
+STATIC_MAX_MASKS = 2048       # SNAPS_STATIC_MAX_MASKS
+
+
+def knn_selfjoin_static(X, masks, k, *, lists=True, scores=True, out=None, stream=None):
+    """snaps_knn_selfjoin_static: the kNN self-join with the library's built-in scratch array instead
+    of a workspace (the C call allocates nothing on the device; N <= 32,768, n_masks <= 2,048,
+    k <= 32; calls that overlap on one GPU race).  Outputs as knn_selfjoin; pass them in `out` to keep
+    this wrapper from allocating them."""
+    import torch
+    assert X.is_cuda and X.dtype == torch.float32 and X.dim() == 2 and X.stride(1) == 1
+    m = _masks(masks)
+    N, n_feat = X.shape
+    out = dict(out or {})
+    dev = X.device
+    if lists:
+        out.setdefault("idx", torch.empty((len(m), N, k), dtype=torch.int32, device=dev))
+        out.setdefault("dist", torch.empty((len(m), N, k), dtype=torch.float32, device=dev))
+    if scores:
+        out.setdefault("kth", torch.empty((len(m), N), dtype=torch.float32, device=dev))
+        out.setdefault("mean", torch.empty((len(m), N), dtype=torch.float32, device=dev))
+        out.setdefault("indeg", torch.empty((len(m), N), dtype=torch.int32, device=dev))
+    _check(lib().snaps_knn_selfjoin_static(
+        _dptr(X), N, n_feat, X.stride(0), m.ctypes.data_as(ctypes.c_void_p), len(m), k,
+        _dptr(out.get("idx")), _dptr(out.get("dist")), _dptr(out.get("kth")),
+        _dptr(out.get("mean")), _dptr(out.get("indeg")), _stream(stream)))
     return out
 
 

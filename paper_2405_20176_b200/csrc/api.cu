@@ -12,6 +12,7 @@
 #include <iterator>
 #include <map>
 #include <utility>
+#include <mutex>
 #include <vector>
 
 #include "../../include/snaps.h"
@@ -768,6 +769,36 @@ snaps_status range_grid_run(Engine* E, int G, const float* d_thr, const RangeOut
 
 }  // namespace
 
+// ---- built-in scratch of snaps_knn_selfjoin_static ------------------------------------------
+// One array per device that loads the library, held until the process exits.  In host code the
+// name below is a host-side stand-in for the symbol, not a device address: the address a kernel
+// can use comes from cudaGetSymbolAddress, asked for once per device with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[SNAPS_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+void* g_static_ptr[kMaxDevices] = {};
+
+snaps_status static_scratch_address(void** out) {
+    static_assert(SNAPS_STATIC_SCRATCH_BYTES % 256 == 0, "scratch size is a multiple of the carve alignment");
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(SNAPS_UNSUPPORTED, "device ordinal %d outside 0..%d", dev, kMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) return fail(SNAPS_CUDA_ERROR, "cudaGetSymbolAddress returned a null address");
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return SNAPS_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char* snaps_last_error(void) { return g_err; }
@@ -818,6 +849,43 @@ snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t
     CUDA_TRY(cudaMemcpyAsync(E.w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
                              cudaMemcpyHostToDevice, E.st));
     return lattice_knn_enqueue(&E, E.w.batches, static_cast<int>(batches.size()), k, o);
+}
+
+snaps_status snaps_knn_selfjoin_static(const float* d_X, int64_t N, int n_feat, int64_t ld,
+                                       const uint16_t* h_masks, int n_masks, int k, int32_t* out_idx,
+                                       float* out_dist, float* out_kth, float* out_mean, int32_t* out_indeg,
+                                       void* stream) {
+    prof_reset();
+    if (N > SNAPS_STATIC_MAX_N)
+        return fail(SNAPS_UNSUPPORTED, "N = %lld > %d, the limit of the built-in scratch array (use snaps_knn_selfjoin with a workspace)",
+                    (long long)N, SNAPS_STATIC_MAX_N);
+    if (n_masks > SNAPS_STATIC_MAX_MASKS)
+        return fail(SNAPS_UNSUPPORTED, "n_masks = %d > %d, the limit of the built-in scratch array (use snaps_knn_selfjoin with a workspace)",
+                    n_masks, SNAPS_STATIC_MAX_MASKS);
+    Engine E;
+    E.job = Job{d_X, N, n_feat, ld, h_masks, n_masks, 0, N, SNAPS_ENGINE_LATTICE, SNAPS_ENGINE_LATTICE};
+    E.st = static_cast<cudaStream_t>(stream);
+    snaps_status rc = check_job(E.job, k);
+    if (rc) return rc;
+    if (k < 1 || k > SNAPS_LATTICE_MAX_K || k > N - 1)
+        return fail(SNAPS_INVALID_ARG, "k = %d outside 1..min(N-1, %d)", k, SNAPS_LATTICE_MAX_K);
+    if (!out_idx && !out_dist && !out_kth && !out_mean && !out_indeg)
+        return fail(SNAPS_INVALID_ARG, "all outputs are NULL");
+    void* scratch = nullptr;
+    rc = static_scratch_address(&scratch);
+    if (rc) return rc;
+    rc = carve(scratch, SNAPS_STATIC_SCRATCH_BYTES, E.job, &E.w);
+    if (rc) return rc;
+    rc = engine_begin(&E);                  // rewrites every staged row and block the kernel reads
+    if (rc) return rc;
+    if (out_indeg)
+        CUDA_TRY(cudaMemsetAsync(out_indeg, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, E.st));
+    const KnnOut o = {out_idx, out_dist, out_kth, out_mean, out_indeg};
+    std::vector<snaps::BatchDesc> batches;
+    plan_lattice(h_masks, n_masks, nullptr, 0, &batches);
+    CUDA_TRY(cudaMemcpyAsync(E.w.batches, batches.data(), sizeof(snaps::BatchDesc) * batches.size(),
+                             cudaMemcpyHostToDevice, E.st));
+    return lattice_knn_enqueue(&E, E.w.batches, static_cast<int>(batches.size()), k, o);   // zeroes the work counter
 }
 
 snaps_status snaps_range_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t ld,
