@@ -424,7 +424,8 @@ snaps_status grid_knn_enqueue(Engine* E, int m0, int nm, int k, const KnnOut& o)
         snaps::GridJoinParams p;
         int d = 0;
         grid_params_common(E, m, &p, &d);
-        CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, &E->gi, E->st));
+        CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, k, &E->gi, E->st));
+        p.warp_order = E->gi.warp_order;
         const size_t r = static_cast<size_t>(m - m0);
         p.k = k;
         p.out_idx = o.idx ? o.idx + r * nq * k : nullptr;
@@ -449,7 +450,7 @@ snaps_status grid_range_enqueue(Engine* E, int m0, int nm, const float* h_eps2, 
         snaps::GridJoinParams p;
         int d = 0;
         grid_params_common(E, m, &p, &d);
-        CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, &E->gi, E->st));
+        CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, 0, &E->gi, E->st));
         const size_t r = static_cast<size_t>(m - m0);
         p.G = G;
         if (G > 0) p.eps2_grid = d_radii + static_cast<size_t>(m) * G;

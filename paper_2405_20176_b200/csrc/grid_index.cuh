@@ -48,6 +48,7 @@ struct GridIndex {             // per-mask state (rebuilt for every mask)
     int* cell_start;           // [n_cells + 1]
     float* Xs;                 // compact rows in cell order, two objects interleaved: [ceil(N/2)][4*ceil(d/4)][2] floats
     int* qlist;                // positions of the queries in [q_begin, q_end) (only when sharded)
+    int* warp_order;           // kNN: the join's warps (32 consecutive queries each), heaviest first
     void* cub_tmp;
     size_t cub_bytes;
 };
@@ -79,7 +80,8 @@ cudaError_t grid_plan_launch(const uint16_t* d_masks, int n_masks, int64_t N, co
 void grid_index_carve(unsigned char* region, size_t bytes, int64_t N, GridIndex* ix);
 
 // Per mask: cell keys -> stable sort -> compact rows, cell starts; optional query list for [q_begin, q_end).
+// knn_k > 0: also the order in which the kNN join takes its warps (ix->warp_order), heaviest first.
 cudaError_t grid_index_build(const GridTable& t, const GridPlan* d_plan, int N, int d, const int bits[kGridDims],
-                             int64_t q_begin, int64_t q_end, GridIndex* ix, cudaStream_t stream);
+                             int64_t q_begin, int64_t q_end, int knn_k, GridIndex* ix, cudaStream_t stream);
 
 }  // namespace snaps

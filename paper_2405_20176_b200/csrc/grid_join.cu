@@ -111,9 +111,10 @@ __global__ void __launch_bounds__(warps_per_cta(MODE) * 32) grid_join_kernel(con
     constexpr int G4 = DP / 2;                     // float4 per pair of candidates: two columns x two objects
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long wid = static_cast<long long>(blockIdx.x) * (blockDim.x >> 5) + warp;
+    const long long slot = static_cast<long long>(blockIdx.x) * (blockDim.x >> 5) + warp;
+    if (slot * 32 >= p.nq) return;                 // warps are independent: no block barrier exists
+    const long long wid = p.warp_order ? p.warp_order[slot] : slot;
     const long long qi0 = wid * 32;
-    if (qi0 >= p.nq) return;                       // warps are independent: no block barrier exists
     const int k = p.k;
     float* wsm = reinterpret_cast<float*>(smem_raw) + static_cast<size_t>(warp) * warp_words(D, MODE, k, p.G);
     float4* tile4 = reinterpret_cast<float4*>(wsm);

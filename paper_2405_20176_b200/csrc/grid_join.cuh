@@ -15,6 +15,7 @@ struct GridJoinParams {
     const int* perm;
     const int* cell_start;
     const int* qlist;          // sorted positions of the queries, or nullptr = every position
+    const int* warp_order;     // warp slot -> group of 32 queries (heaviest first), or nullptr = identity
     const float* edges;        // [15][kGridEdgeStride]
     const GridPlan* plan;      // device
     int bits[kGridDims];       // host copy of plan->bits
