@@ -626,7 +626,7 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
             del out
             torch.cuda.empty_cache()
             Xh = torch.from_numpy(X).pin_memory()
-            mpb = 2048
+            mpb = 4096           # 8 groups: a group's join overlaps the previous group's copy-out
             hws = torch.empty(snaps.workspace_bytes(N, n_feat, n_masks, k, x_on_host=True) +
                               snaps.stream_ring_bytes(N, N, k, mpb), dtype=torch.uint8, device=dev)
             hout = {"kth": torch.empty((n_masks, N), dtype=torch.float32, pin_memory=True),
