@@ -40,6 +40,19 @@ def test_workspace_and_plan_sizes():
     assert s.stream_ring_bytes(1000, 1000, 10, 4) >= 2 * 4 * 1000 * 23 * 4
 
 
+def test_static_scratch_matches_the_workspace_layout():
+    """snaps_knn_selfjoin_static carves its built-in array like a caller's workspace: the array must be
+    exactly what the largest admitted sizes need (include/snaps.h: SNAPS_STATIC_*)."""
+    import re
+    import paper_2405_20176_b200 as s
+    text = open(os.path.join(ROOT, "include", "snaps.h")).read()
+    val = {n: int(v) for n, v in re.findall(r"#define (SNAPS_STATIC_\w+) (\d+)", text)}
+    assert val["SNAPS_STATIC_MAX_N"] == s.STATIC_MAX_N and val["SNAPS_STATIC_MAX_MASKS"] == s.STATIC_MAX_MASKS
+    need = s.workspace_bytes(val["SNAPS_STATIC_MAX_N"], 15, val["SNAPS_STATIC_MAX_MASKS"], 32, engine="lattice")
+    assert need == val["SNAPS_STATIC_SCRATCH_BYTES"]
+    assert s.workspace_bytes(31693, 15, 2048, 10, engine="lattice") <= val["SNAPS_STATIC_SCRATCH_BYTES"]
+
+
 def test_no_torch_types_in_header():
     text = open(os.path.join(ROOT, "include", "snaps.h")).read()
     assert "torch" not in text.lower().replace("pytorch", "") or True
