@@ -388,6 +388,57 @@ def run_range(args, cfg, snaps, torch, D, steps, warmup, peakinfo, emit=True):
     return line
 
 
+def run_select_eps(args, cfg, snaps, torch, D):
+    """The DSSJ parameter selection of PAPER.md:181-189, 229-239 in one call per chunk of masks
+    (snaps_range_select_eps: eps_min / eps_max search -> |G| radii -> one join at eps_max -> ranks -> Eq. 2 -> Eq. 3)
+    at the paper's operating point on SNAPShot1: s_min = 0.001 |D|, s_max = 0.15 |D|, |G| = 22 (Fig. 2,
+    reading A22), top 1 %.  The paper's figure for this workload over all 32,752 feature spaces,
+    whole pipeline on 1 x A100 with o = 8: 2.64 h -- context, other hardware."""
+    X = workloads.make_table(cfg.n, cfg.seed, cols=list(range(cfg.n_feat)), outlier_frac=0.01)
+    N = len(X)
+    groups = {}
+    for m in cfg.masks():
+        groups.setdefault(int(m) >> 6, []).append(m)
+    keys = sorted(groups)
+    n_b = max(1, args.select_eps // 64)
+    masks = np.array([m for kk in keys[::max(1, len(keys) // n_b)][:n_b] for m in groups[kk]], dtype=np.uint16)
+    rng = np.random.default_rng(cfg.seed)
+    q = np.sort(rng.choice(N, 1000, replace=False)).astype(np.int32)
+    c = np.arange(N, dtype=np.int32)
+    G, n_top, s_min, s_max = 22, int(round(0.01 * N)), 0.001 * N, 0.15 * N
+    Xd = torch.from_numpy(X).to(D.dev)
+    chunk = 512
+
+    def step():
+        for m0 in range(0, len(masks), chunk):
+            out = snaps.range_select_eps(Xd, masks[m0:m0 + chunk], q, c, s_min, s_max, G, n_top, 4096, engine="lattice")
+        return out
+
+    for _ in range(max(1, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(D.dev.index or 0)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        out = step()
+    ev1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    print(json.dumps({
+        "metric": "feature spaces/sec (DSSJ parameter selection: eps search + 22-radius join at s_max + ranks + Eq. 2 + Eq. 3)",
+        "value": len(masks) / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(1, args.warmup),
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: N={N} x 15 (seed {cfg.seed}), {len(masks)} subspaces = {n_b} whole sub-lattice batches "
+                               f"spread over the 32,752, s_min={s_min:.0f}, s_max={s_max:.0f} neighbours, |G|={G}, top {n_top}"},
+        "ms_per_subspace": ms / len(masks), "seconds_for_all_32752": ms / len(masks) * 32752 / 1e3,
+        "selected_grid_index_histogram": np.bincount(out["j_count"].cpu().numpy(), minlength=G).tolist(),
+        "clocks": clocks,
+        "paper_context": "paper: DSSJ over all 32,752 feature spaces incl. eps^select and both rankings, 2.64 h on 1xA100 "
+                         "(o=8), whole pipeline with CPU post-processing and file output (PAPER.md:394)"}), flush=True)
+
+
 def run_c5(args, cfg, snaps, torch, D):
     """Config 5 (BASELINE.json configs[4]): N=5,000,000 x 15, 256 subspace masks sampled from the 32,752,
     kNNSJ k=16 plus DSSJ (eps_d for ~100 neighbours), outputs through the recycling sink (two pinned host
@@ -484,6 +535,9 @@ def main():
                     help="headline step on the first M masks only, for `ncu --set full` captures (ncu replays a launch "
                          "~40 times and saves / restores its 12.5 GB of outputs around each replay); the line is marked "
                          "`partial` and is NOT a bench value")
+    ap.add_argument("--select-eps", type=int, default=0, metavar="M",
+                    help="with --config c3_snapshot1_dssj: time the DSSJ parameter selection (snaps_range_select_eps) at the "
+                         "paper's operating point on M masks (whole sub-lattice batches spread over the mask list) instead of the join")
     ap.add_argument("--c5-n", type=int, default=0, help="config 5 with a reduced N (quick runs)")
     ap.add_argument("--c5-masks", type=int, default=0, help="config 5 on its first M masks only (quick runs)")
     args = ap.parse_args()
@@ -520,6 +574,9 @@ def main():
             return
         if cfg.join == "knn" and cfg.n >= 100000:
             run_lsst(args, cfg, snaps, torch, D, max(1, args.steps))
+            return
+        if cfg.join == "range" and args.select_eps > 0:
+            run_select_eps(args, cfg, snaps, torch, D)
             return
         if cfg.join == "range":
             run_range(args, cfg, snaps, torch, D, args.steps, args.warmup, peakinfo)

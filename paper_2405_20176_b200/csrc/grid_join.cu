@@ -204,6 +204,13 @@ __global__ void __launch_bounds__(warps_per_cta(MODE) * 32) grid_join_kernel(con
     }
     __syncwarp();
 
+    float g_first = 0.f, g_per_eps = 0.f;                    // radius grid: first radius and bins per unit of distance
+    if (MODE == MODE_RANGE_GRID) {
+        g_first = sqrtf(fmaxf(gthr[0], 0.f));
+        const float g_last = sqrtf(fmaxf(gthr[p.G - 1], 0.f));
+        g_per_eps = (p.G > 1 && g_last > g_first) ? static_cast<float>(p.G - 1) / (g_last - g_first) : 0.f;
+    }
+
     // ---- one candidate against this lane's query
     auto consider = [&](float acc, int cpos) {
         if (KNN) {
@@ -220,10 +227,18 @@ __global__ void __launch_bounds__(warps_per_cta(MODE) * 32) grid_join_kernel(con
             sum += sqrtf(acc);
         } else {
             if (cpos == pos) return;
-            int g = 0;
-            while (acc > gthr[g]) ++g;                       // smallest radius that contains the pair
+            // smallest radius that contains the pair: guessed as if the radii were evenly spaced (the library's own
+            // grids are, reading A22), settled against the exact thresholds on either side -- any grid stays exact
+            const float dd = sqrtf(acc);
+            int g = min(max(__float2int_ru((dd - g_first) * g_per_eps), 0), p.G - 1);
+            if (g > 0 && acc <= gthr[g - 1]) {
+                --g;
+                while (g > 0 && acc <= gthr[g - 1]) --g;
+            } else {
+                while (acc > gthr[g]) ++g;                   // ends: acc <= the largest threshold
+            }
             gcnt[g * 32 + lane] += 1;
-            gsum[g * 32 + lane] += sqrtf(acc);
+            gsum[g * 32 + lane] += dd;
         }
     };
 

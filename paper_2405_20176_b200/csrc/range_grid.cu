@@ -46,6 +46,13 @@ __device__ __noinline__ void range_grid_refine(float* ws, int G, bool with_sum, 
         __syncwarp();
         const int T = 32 * half + lane;
         const float thr = G_TMAX(T);
+        // A neighbour's bin = the smallest radius that contains it (radii ascend).  The bin is guessed from the
+        // distance itself, as if the list's radii were evenly spaced between the smallest and the largest (the
+        // library's own grids are, reading A22), and the guess is settled against the exact thresholds on
+        // either side: one shared-memory round trip per neighbour when the guess is right, any grid stays exact.
+        const float t_first = G_THR(T, 0);
+        const float e_first = sqrtf(fmaxf(t_first, 0.f)), e_last = sqrtf(fmaxf(thr, 0.f));
+        const float per_eps = (G > 1 && e_last > e_first) ? static_cast<float>(G - 1) / (e_last - e_first) : 0.f;
         unsigned mask = 0u;
 #pragma unroll
         for (int j4 = 0; j4 < 8; ++j4) {
@@ -60,10 +67,20 @@ __device__ __noinline__ void range_grid_refine(float* ws, int G, bool with_sum, 
             const int j = __ffs(mask) - 1;
             mask &= mask - 1u;
             const float d2 = G_MT(lane, j);
-            int g = 0;   // smallest radius that contains the neighbour (radii ascend)
-            while (!(d2 < G_THR(T, g))) ++g;
+            const float dd = sqrtf(d2);
+            int g = min(max(__float2int_ru((dd - e_first) * per_eps), 0), G - 1);
+            {
+                const float below = g > 0 ? G_THR(T, g - 1) : -1.f, here = G_THR(T, g);
+                if (d2 < below) {
+                    --g;
+                    while (g > 0 && d2 < G_THR(T, g - 1)) --g;
+                } else if (!(d2 < here)) {
+                    ++g;
+                    while (!(d2 < G_THR(T, g))) ++g;         // ends: d2 < the largest threshold
+                }
+            }
             G_HCNT(T, g) += 1;
-            if (with_sum) G_HSUM(T, g) += sqrtf(d2);
+            if (with_sum) G_HSUM(T, g) += dd;
         }
         __syncwarp();
     }
