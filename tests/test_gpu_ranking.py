@@ -147,6 +147,41 @@ def test_radius_grid_single_scan_matches_oracle_per_radius(snaps):
         snaps.range_selfjoin_grid(_t(X), masks, grid[:, ::-1].copy())   # not ascending
 
 
+@pytest.mark.parametrize("engine", ["lattice", "grid"])
+def test_radius_grid_irregular_radii(snaps, engine):
+    """The kernels guess a neighbour's radius bin as if the radii were evenly spaced and settle the guess against
+    the exact thresholds: grids that are anything but evenly spaced (geometric, clustered at either end, radii a few
+    ulps apart, G = 1, 2 and the maximum 32) must give, radius by radius, exactly the counts of the single-radius join
+    and its sums within the fp32 summation-order tolerance."""
+    import torch
+    rng = np.random.default_rng(77)
+    X = workloads.make_table(1300, 31, outlier_frac=0.02)
+    masks = np.array([0b11, 0x7FFF, (1 << 11) | (1 << 4) | 0b10, 0b1111100, (1 << 13) | (1 << 6), 0b101], dtype=np.uint16)
+    scale = np.array([1.0, 6.0, 2.0, 3.0, 1.5, 1.2], dtype=np.float32)
+    Xd = _t(X)
+    grids = {
+        "geometric": np.geomspace(0.004, 0.16, 12),
+        "clustered_low": np.concatenate([np.linspace(0.01, 0.012, 9), [0.05, 0.15]]),
+        "clustered_high": np.concatenate([[0.005, 0.03], np.linspace(0.140, 0.141, 10)]),
+        "adjacent_floats": np.array([0.02, 0.0200001, 0.0200002, 0.07, 0.0700001, 0.13]),
+        "one": np.array([0.06]),
+        "two": np.array([0.001, 0.2]),
+        "thirty_two": np.sort(rng.uniform(0.002, 0.18, 32)),
+    }
+    for name, base in grids.items():
+        grid = (base[None, :].astype(np.float32) * scale[:, None]).astype(np.float32)
+        out = snaps.range_selfjoin_grid(Xd, masks, grid, engine=engine)
+        torch.cuda.synchronize()
+        cnt, sm = out["count"].cpu().numpy(), out["sumdist"].cpu().numpy()
+        assert (np.diff(cnt, axis=1) >= 0).all(), name
+        for g in sorted({0, grid.shape[1] // 2, grid.shape[1] - 1}):
+            one = snaps.range_selfjoin(Xd, masks, grid[:, g], engine=engine)
+            torch.cuda.synchronize()
+            assert np.array_equal(one["count"].cpu().numpy(), cnt[:, g]), (name, g)
+            ref = one["sumdist"].cpu().numpy()
+            assert np.allclose(sm[:, g], ref, rtol=3e-5, atol=1e-6), (name, g)
+
+
 def test_select_k_pipeline_matches_oracle(snaps):
     """snaps_knn_select_k (one call: k grid -> scores -> ranks -> Eq. 2 -> Eq. 3) against the oracle
     procedure, mask by mask, on the SAME k_max lists: the oracle's own join, cast to the fp32 lists the
