@@ -12,7 +12,7 @@ CSRC = os.path.join(_HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(_HERE, "libsnaps.so")
 SOURCES = ["api.cu", "knn_lattice.cu", "range_lattice.cu", "misc_kernels.cu", "ranking.cu", "range_grid.cu",
-           "eps_search.cu", "grid_index.cu", "grid_join.cu"]
+           "eps_search.cu", "grid_index.cu", "grid_join.cu", "knn_bigk.cu"]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     # no implicit mul+add contraction: the kernels place their FMAs explicitly so that the

@@ -19,6 +19,7 @@
 #include "eps_search.cuh"
 #include "grid_index.cuh"
 #include "grid_join.cuh"
+#include "knn_bigk.cuh"
 #include "knn_lattice.cuh"
 #include "misc_kernels.cuh"
 #include "range_grid.cuh"
@@ -290,6 +291,8 @@ struct Engine {
     Job job;
     Workspace w;
     cudaStream_t st;
+    unsigned char* bigk = nullptr;   // what is left of the workspace for the long-list kNN path (knn_bigk.cu), if any
+    size_t bigk_bytes = 0;
     snaps::GridTable gt;
     snaps::GridIndex gi;
 };
@@ -424,7 +427,11 @@ snaps_status grid_knn_enqueue(Engine* E, int m0, int nm, int k, const KnnOut& o)
         snaps::GridJoinParams p;
         int d = 0;
         grid_params_common(E, m, &p, &d);
-        CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, k, &E->gi, E->st));
+        // long lists on a small table: radix selection over brute-force passes instead of per-query heaps, when the
+        // workspace has the room (snaps_workspace_bytes asks for it)
+        const bool bigk = k >= snaps::kBigKMinK && j.N <= snaps::kBigKMaxN && E->bigk &&
+                          E->bigk_bytes >= snaps::knn_bigk_scratch_bytes(j.nq(), k);
+        CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, bigk ? 0 : k, &E->gi, E->st));
         p.warp_order = E->gi.warp_order;
         const size_t r = static_cast<size_t>(m - m0);
         p.k = k;
@@ -434,7 +441,8 @@ snaps_status grid_knn_enqueue(Engine* E, int m0, int nm, int k, const KnnOut& o)
         p.out_mean = o.mean ? o.mean + r * nq : nullptr;
         p.out_indeg = o.indeg ? o.indeg + r * N : nullptr;
         const bool prof = prof_begin(E->st);
-        CUDA_TRY(snaps::grid_knn_launch(p, d, E->st));
+        if (bigk) CUDA_TRY(snaps::knn_bigk_launch(p, d, E->bigk, E->bigk_bytes, E->st));
+        else CUDA_TRY(snaps::grid_knn_launch(p, d, E->st));
         prof_end(prof, E->st);
     }
     return SNAPS_OK;
@@ -524,6 +532,8 @@ snaps_status run_batched(Batched* B, const std::vector<snaps::BatchDesc>* all_ba
             r += b;
             left -= b;
         }
+    E->bigk = r;                 // what the ring leaves
+    E->bigk_bytes = left;
     const bool knn = B->k > 0;
     const int indeg_arr = 4;
     struct Pending { int m0, nm, buf; };
@@ -811,7 +821,11 @@ size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k, int flag
         return 0;
     const int engine = resolve_engine(flags, N, k);
     if (engine != SNAPS_ENGINE_LATTICE && engine != SNAPS_ENGINE_GRID) return 0;
-    return base_workspace_bytes(N, n_feat, n_masks, engine, flags);
+    size_t b = base_workspace_bytes(N, n_feat, n_masks, engine, flags);
+    if (engine == SNAPS_ENGINE_GRID && k >= snaps::kBigKMinK && N <= snaps::kBigKMaxN &&
+        static_cast<long long>(N) * k <= 0x7fffffffLL)
+        b += snaps::knn_bigk_scratch_bytes(N, k);      // long lists on a small table: the selection path's keys
+    return b;
 }
 
 int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t* h_masks, int n_masks) {
@@ -844,6 +858,8 @@ snaps_status snaps_knn_selfjoin(const float* d_X, int64_t N, int n_feat, int64_t
     if (out_indeg)
         CUDA_TRY(cudaMemsetAsync(out_indeg, 0, sizeof(int32_t) * static_cast<size_t>(n_masks) * N, E.st));
     const KnnOut o = {out_idx, out_dist, out_kth, out_mean, out_indeg};
+    E.bigk = E.w.extra;
+    E.bigk_bytes = E.w.extra_bytes;
     if (E.job.engine == SNAPS_ENGINE_GRID) return grid_knn_enqueue(&E, 0, n_masks, k, o);
     std::vector<snaps::BatchDesc> batches;
     plan_lattice(h_masks, n_masks, nullptr, 0, &batches);

@@ -1,0 +1,19 @@
+// knn_bigk.cuh -- kNN self-join of one feature subspace for long lists on small tables
+// (512 < k <= 4096, N <= 131,072: the paper's k_max = 4096 on SNAPShot1).
+#pragma once
+#include "grid_join.cuh"
+
+namespace snaps {
+
+constexpr int kBigKMaxN = 1 << 17;     // ids take 17 bits of the 48-bit selection key
+constexpr int kBigKMinK = 513;         // below, the heaps of grid_join.cu are faster (the seven passes cost ~45 ms at N = 31,693)
+
+// Scratch the launch needs for nq queries and lists of k: two arrays of nq*k 64-bit keys, segment offsets, CUB's own.
+size_t knn_bigk_scratch_bytes(int64_t nq, int k);
+
+// Same inputs and outputs as grid_knn_launch (the index of grid_index.cu supplies the compact rows and the
+// sorted order; the cells themselves are not used).  The distances are formed by the same instruction sequence,
+// so the two paths give identical lists.
+cudaError_t knn_bigk_launch(const GridJoinParams& p, int d, void* scratch, size_t scratch_bytes, cudaStream_t stream);
+
+}  // namespace snaps

@@ -603,6 +603,44 @@ def test_paper_operating_point_k4096(snaps, oracle_mod):
     assert torch.equal(out["kth"], out["dist"][:, :, -1])
 
 
+@pytest.mark.parametrize("n,nf,k,seed", [(700, 15, 513, 0), (1200, 6, 1000, 1), (1537, 15, 700, 2), (600, 3, 599, 3)])
+def test_long_list_path_against_oracle(snaps, oracle_mod, n, nf, k, seed):
+    """k > 512 on a small table takes the selection path (knn_bigk.cu: radix selection over brute-force passes,
+    then one segmented sort): whole output against the oracle, incl. k = N - 1, plus a table with a block of
+    duplicate rows (every tie must go to the smaller id) and a query-range slice."""
+    import torch
+    X = workloads.make_table(n, 50 + seed, cols=list(range(nf)), outlier_frac=0.02)
+    if seed == 2:
+        X = workloads.duplicate_block_table(n, 50 + seed)
+    allm = workloads.all_masks(nf, 1)
+    masks = np.random.default_rng(seed).choice(allm, 5, replace=False).astype(np.uint16)
+    g, _ = _knn_case(snaps, oracle_mod, X, masks, k, engine="grid")
+    # a slice of the queries gives the same rows
+    q0, q1 = n // 3, n // 3 + 101
+    part = snaps.knn_selfjoin(_dev(X), masks, k, engine="grid", q_range=(q0, q1))
+    torch.cuda.synchronize()
+    assert np.array_equal(part["idx"].cpu().numpy(), g["idx"][:, q0:q1])
+    assert np.array_equal(part["dist"].cpu().numpy(), g["dist"][:, q0:q1])
+    assert np.array_equal(part["mean"].cpu().numpy(), g["mean"][:, q0:q1])
+
+
+def test_long_list_path_equals_heap_path(snaps):
+    """The two ways of building lists longer than 256 give identical outputs: a workspace without the selection
+    path's scratch (the size for k = 512) makes the same call fall back to the heaps in the output lists."""
+    import torch
+    X = workloads.make_table(2500, 91, outlier_frac=0.01)
+    masks = np.array([0b11, 0x7FFF, (1 << 10) | (1 << 5) | 0b100], dtype=np.uint16)
+    k = 777
+    Xd = _dev(X)
+    a = snaps.knn_selfjoin(Xd, masks, k, engine="grid")
+    small = torch.empty(snaps.workspace_bytes(len(X), 15, len(masks), 512, engine="grid"), dtype=torch.uint8, device="cuda")
+    assert small.numel() < a["_workspace"].numel()
+    b = snaps.knn_selfjoin(Xd, masks, k, engine="grid", workspace=small)
+    torch.cuda.synchronize()
+    for name in ("idx", "dist", "kth", "mean", "indeg"):
+        assert torch.equal(a[name], b[name]), name
+
+
 def test_radius_grid_sub_lattice_engine_full_size(snaps, oracle_mod):
     """The sub-lattice radius-grid kernel (range_grid.cu) at config 3's size: N = 31,693, two whole batches
     (128 lattice slots, 125 masks), four radii per mask up to config 3's stored eps_d; sampled queries of every
