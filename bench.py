@@ -388,6 +388,62 @@ def run_range(args, cfg, snaps, torch, D, steps, warmup, peakinfo, emit=True):
     return line
 
 
+def run_select_k(args, cfg, snaps, torch, D):
+    """The kNN parameter selection of PAPER.md:181-189, 258-260 at the paper's SNAPShot1 operating point: one join at
+    k_max = 4096 gives every smaller k's lists as prefixes; snaps_knn_select_k then forms the scores at
+    every k_j of the grid, ranks them, and takes Eq. 2 against the smallest and largest k and Eq. 3 -- for both kNN
+    metrics.  The paper's k grid is "unevenly sampled" and not printed (reading A17): powers of two 2 ... 4096 here."""
+    X = workloads.make_table(cfg.n, cfg.seed, cols=list(range(cfg.n_feat)), outlier_frac=0.01)
+    N = len(X)
+    masks_all = cfg.masks()
+    masks = masks_all[np.linspace(0, len(masks_all) - 1, args.select_k).astype(np.int64)]
+    k_max, n_top = 4096, int(round(0.01 * N))
+    k_grid = np.array([2, 4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048, 3072, 4096], dtype=np.int32)
+    Xd = torch.from_numpy(X).to(D.dev)
+    chunk = 8
+    first = snaps.knn_selfjoin(Xd, masks[:chunk], k_max, engine="grid")
+    ws = first.pop("_workspace")
+    snaps.profile_enable(True)
+    join_ms = []
+
+    def step():
+        for m0 in range(0, len(masks), chunk):
+            mm = masks[m0:m0 + chunk]
+            if len(mm) == chunk:
+                j = snaps.knn_selfjoin(Xd, mm, k_max, engine="grid", out=first, workspace=ws)
+            else:
+                j = snaps.knn_selfjoin(Xd, mm, k_max, engine="grid")
+            join_ms.append(snaps.profile_last_kernel_ms()[0])
+            sel = snaps.knn_select_k(j["idx"], j["dist"], k_grid, n_top)
+        return sel
+
+    for _ in range(max(1, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+    join_ms.clear()
+    sampler = ClockSampler(D.dev.index or 0)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        sel = step()
+    ev1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    print(json.dumps({
+        "metric": "feature spaces/sec (kNN parameter selection: join at k_max = 4096 + scores at 13 k + ranks + Eq. 2 + Eq. 3)",
+        "value": len(masks) / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(1, args.warmup),
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: N={N} x 15 (seed {cfg.seed}), {len(masks)} subspaces spread over the 32,752, "
+                               f"k_max={k_max}, k grid {k_grid.tolist()}, top {n_top}"},
+        "ms_per_subspace": ms / len(masks), "join_ms_per_subspace": float(np.sum(join_ms)) / args.steps / len(masks),
+        "seconds_for_all_32752": ms / len(masks) * 32752 / 1e3,
+        "selected_grid_index_histogram_last_chunk": np.bincount(sel["j_mean"].cpu().numpy(), minlength=len(k_grid)).tolist(),
+        "clocks": clocks,
+        "paper_context": "paper: kNNSJ more expensive than DSSJ (PAPER.md:398); absolute kNNSJ time on SNAPShot1 not in the "
+                         "text (Fig. 10 is an image)"}), flush=True)
+
+
 def run_select_eps(args, cfg, snaps, torch, D):
     """The DSSJ parameter selection of PAPER.md:181-189, 229-239 in one call per chunk of masks
     (snaps_range_select_eps: eps_min / eps_max search -> |G| radii -> one join at eps_max -> ranks -> Eq. 2 -> Eq. 3)
@@ -433,7 +489,7 @@ def run_select_eps(args, cfg, snaps, torch, D):
         "config": {"workload": f"{cfg.name}: N={N} x 15 (seed {cfg.seed}), {len(masks)} subspaces = {n_b} whole sub-lattice batches "
                                f"spread over the 32,752, s_min={s_min:.0f}, s_max={s_max:.0f} neighbours, |G|={G}, top {n_top}"},
         "ms_per_subspace": ms / len(masks), "seconds_for_all_32752": ms / len(masks) * 32752 / 1e3,
-        "selected_grid_index_histogram": np.bincount(out["j_count"].cpu().numpy(), minlength=G).tolist(),
+        "selected_grid_index_histogram_last_chunk": np.bincount(out["j_count"].cpu().numpy(), minlength=G).tolist(),
         "clocks": clocks,
         "paper_context": "paper: DSSJ over all 32,752 feature spaces incl. eps^select and both rankings, 2.64 h on 1xA100 "
                          "(o=8), whole pipeline with CPU post-processing and file output (PAPER.md:394)"}), flush=True)
@@ -538,6 +594,9 @@ def main():
     ap.add_argument("--select-eps", type=int, default=0, metavar="M",
                     help="with --config c3_snapshot1_dssj: time the DSSJ parameter selection (snaps_range_select_eps) at the "
                          "paper's operating point on M masks (whole sub-lattice batches spread over the mask list) instead of the join")
+    ap.add_argument("--select-k", type=int, default=0, metavar="M",
+                    help="with the default config: time the kNN parameter selection at the paper's operating point (join at "
+                         "k_max = 4096, then snaps_knn_select_k over a 13-point k grid) on M masks spread over the mask list")
     ap.add_argument("--c5-n", type=int, default=0, help="config 5 with a reduced N (quick runs)")
     ap.add_argument("--c5-masks", type=int, default=0, help="config 5 on its first M masks only (quick runs)")
     args = ap.parse_args()
@@ -574,6 +633,9 @@ def main():
             return
         if cfg.join == "knn" and cfg.n >= 100000:
             run_lsst(args, cfg, snaps, torch, D, max(1, args.steps))
+            return
+        if cfg.join == "knn" and args.select_k > 0:
+            run_select_k(args, cfg, snaps, torch, D)
             return
         if cfg.join == "range" and args.select_eps > 0:
             run_select_eps(args, cfg, snaps, torch, D)
