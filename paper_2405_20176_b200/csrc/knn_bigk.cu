@@ -2,13 +2,14 @@
 // (512 < k <= 4096, N <= 131,072): PAPER.md:258, k_max = 4096 on SNAPShot1's 31,693 objects.
 //
 // At k = 13 % of N no index prunes anything, and a per-query heap of 4096 entries in global memory spends its
-// time in divergent sifts (grid_join.cu's in-place mode: 400-490 ms per subspace at k = 4096; here 50-64 ms):
+// time in divergent sifts (grid_join.cu's in-place mode: 400-490 ms per subspace at k = 4096; here 28-37 ms):
 //   * SELECT: one warp = 32 queries (lane = query) streams ALL candidates through a shared-memory tile, the
 //     distance of a pair formed by the same instruction sequence as in grid_join.cu (so both paths give the
-//     same lists), and finds the query's k-th smallest key (d^2 bits << 17 | id) by radix selection: six passes
+//     same lists), and finds the query's k-th smallest key (d^2 bits << 17 | id) by radix selection: up to six passes
 //     over the candidates, each a 256-bin per-lane histogram of the next 8 key bits among the candidates that
 //     match the prefix so far.  Keys are unique (ids are), so the k-th key is exact and ties go to the smaller id
-//     (reading A3).  A seventh pass writes the k keys <= the k-th, unordered;
+//     (reading A3); the passes stop once every lane's k-th key is the last of its bin (typically after three or
+//     four).  A last pass writes the k keys <= the k-th, unordered;
 //   * SORT: one CUB segmented radix sort of the nq segments of k keys (48 significant bits);
 //   * FINALISE (a7): ids, sqrt, k-th and mean distance (summed in list order, as everywhere), in-degree.
 // Every pass recomputes the distances: 7 N^2 d flops per subspace is milliseconds at this N, far less than
@@ -27,11 +28,13 @@ constexpr int kBins = 256;
 constexpr int kIdBits = 17;
 
 __host__ __device__ constexpr int dpb(int d) { return (d + 3) / 4 * 4; }
-__host__ __device__ constexpr int warp_words_b(int d) { return kTileB * dpb(d) + kTileB + kBins * 32; }
+// per-warp shared-memory words; the per-lane histogram counts in 16 bits when no bin can overflow them (N < 65,536):
+// half the footprint, twice the warps per SM
+__host__ __device__ constexpr int warp_words_b(int d, int counter_bytes) { return kTileB * dpb(d) + kTileB + kBins * 8 * counter_bytes; }
 
 typedef unsigned long long u64;
 
-template <int D>
+template <int D, typename C>
 __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoinParams p, u64* __restrict__ keys_out) {
     constexpr int DP = dpb(D);
     constexpr int G4 = DP / 2;                     // float4 per pair of candidates
@@ -40,10 +43,10 @@ __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoi
     const long long wid = static_cast<long long>(blockIdx.x) * kWarpsB + warp;
     const long long qi0 = wid * 32;
     if (qi0 >= p.nq) return;                       // warps are independent: no block barrier exists
-    float* wsm = reinterpret_cast<float*>(smem_raw) + static_cast<size_t>(warp) * warp_words_b(D);
+    float* wsm = reinterpret_cast<float*>(smem_raw) + static_cast<size_t>(warp) * warp_words_b(D, sizeof(C));
     float4* tile4 = reinterpret_cast<float4*>(wsm);
     int* tile_id = reinterpret_cast<int*>(wsm + kTileB * DP);
-    unsigned* hist = reinterpret_cast<unsigned*>(wsm + kTileB * DP + kTileB);
+    C* hist = reinterpret_cast<C*>(wsm + kTileB * DP + kTileB);
     const GridPlan* pl = p.plan;
     const int N = p.N, k = p.k;
     const bool valid = qi0 + lane < p.nq;
@@ -97,23 +100,34 @@ __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoi
     // ---- radix selection of the k-th smallest key, 8 bits per pass from the top of the 48
     u64 prefix = 0;
     int need = k;
+    bool done = !valid;            // the k-th key is pinned down as far as the emit pass needs
 #pragma unroll 1
     for (int pass = 0; pass < 6; ++pass) {
+        if (__all_sync(kFull, done)) break;
         const int shift = 40 - 8 * pass;
-        for (int i = lane; i < kBins * 32; i += 32) hist[i] = 0u;
+        for (int i = lane; i < kBins * 32; i += 32) hist[i] = 0;
         const u64 want = prefix >> (shift + 8);
         stream([&](u64 key) {
-            if (pass == 0 || (key >> (shift + 8)) == want) hist[static_cast<unsigned>((key >> shift) & 255u) * 32 + lane] += 1u;
+            if (!done && (pass == 0 || (key >> (shift + 8)) == want))
+                hist[static_cast<unsigned>((key >> shift) & 255u) * 32 + lane] += 1;
         });
-        int cum = 0, sel = kBins - 1;
-        bool found = false;
-        for (int b = 0; b < kBins; ++b) {
-            const int c = static_cast<int>(hist[b * 32 + lane]);
-            if (!found && cum + c >= need) { sel = b; found = true; }
-            if (!found) cum += c;
+        if (!done) {
+            int cum = 0, sel = kBins - 1, csel = 0;
+            bool found = false;
+            for (int b = 0; b < kBins; ++b) {
+                const int c = static_cast<int>(hist[b * 32 + lane]);
+                if (!found && cum + c >= need) { sel = b; csel = c; found = true; }
+                if (!found) cum += c;
+            }
+            prefix |= static_cast<u64>(sel) << shift;
+            need -= cum;
+            // the k-th is the last of its bin: every key with this prefix is among the k smallest, the lower bits
+            // need not be resolved (the usual case once the bins are narrower than the gaps between distances)
+            if (found && need == csel) {
+                prefix |= (static_cast<u64>(1) << shift) - 1;
+                done = true;
+            }
         }
-        prefix |= static_cast<u64>(sel) << shift;
-        need -= cum;
     }
     // ---- the k keys up to the k-th, in stream order
     int cnt = 0;
@@ -166,15 +180,20 @@ size_t cub_bytes_for(int64_t nq, int k) {
     return al256(b);
 }
 
-template <int D>
-cudaError_t launch_d(const GridJoinParams& p, u64* keys, cudaStream_t st) {
-    const size_t smem = static_cast<size_t>(kWarpsB) * warp_words_b(D) * 4;
-    auto kernel = bigk_select_kernel<D>;
+template <int D, typename C>
+cudaError_t launch_dc(const GridJoinParams& p, u64* keys, cudaStream_t st) {
+    const size_t smem = static_cast<size_t>(kWarpsB) * warp_words_b(D, sizeof(C)) * 4;
+    auto kernel = bigk_select_kernel<D, C>;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
     const long long warps = (static_cast<long long>(p.nq) + 31) / 32;
     kernel<<<static_cast<int>((warps + kWarpsB - 1) / kWarpsB), kWarpsB * 32, smem, st>>>(p, keys);
     return cudaGetLastError();
+}
+
+template <int D>
+cudaError_t launch_d(const GridJoinParams& p, u64* keys, cudaStream_t st) {
+    return p.N < 65536 ? launch_dc<D, unsigned short>(p, keys, st) : launch_dc<D, unsigned>(p, keys, st);
 }
 
 }  // namespace

@@ -6,7 +6,7 @@
 namespace snaps {
 
 constexpr int kBigKMaxN = 1 << 17;     // ids take 17 bits of the 48-bit selection key
-constexpr int kBigKMinK = 513;         // below, the heaps of grid_join.cu are faster (the seven passes cost ~45 ms at N = 31,693)
+constexpr int kBigKMinK = 513;         // below, the heaps of grid_join.cu are faster (the passes and the sort cost ~25 ms at N = 31,693)
 
 // Scratch the launch needs for nq queries and lists of k: two arrays of nq*k 64-bit keys, segment offsets, CUB's own.
 size_t knn_bigk_scratch_bytes(int64_t nq, int k);

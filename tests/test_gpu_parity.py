@@ -624,6 +624,23 @@ def test_long_list_path_against_oracle(snaps, oracle_mod, n, nf, k, seed):
     assert np.array_equal(part["mean"].cpu().numpy(), g["mean"][:, q0:q1])
 
 
+def test_long_list_path_above_65535_objects(snaps, oracle_mod):
+    """N >= 65,536: the selection path counts in 32 bits (a histogram bin can hold more than 65,535 candidates).
+    Sampled queries against the oracle, whole-output invariants."""
+    import torch
+    N, k = 70001, 600
+    X = workloads.make_table(N, 66, outlier_frac=0.001)
+    masks = np.array([0b11, (1 << 12) | (1 << 8) | (1 << 3) | 1, 0x7FFF], dtype=np.uint16)
+    out = snaps.knn_selfjoin(_dev(X), masks, k, engine="grid")
+    torch.cuda.synchronize()
+    qs = np.sort(np.random.default_rng(6).choice(N, 6, replace=False))
+    oi, od = oracle_mod.knn_selfjoin(X, masks, k + 1, queries=qs)
+    check_knn(out["idx"][:, qs].cpu().numpy(), out["dist"][:, qs].cpu().numpy(), oi, od, queries=qs)
+    assert bool((out["indeg"].sum(dim=1) == N * k).all())
+    assert bool((out["dist"][:, :, 1:] >= out["dist"][:, :, :-1]).all())
+    assert torch.equal(out["kth"], out["dist"][:, :, -1])
+
+
 def test_long_list_path_equals_heap_path(snaps):
     """The two ways of building lists longer than 256 give identical outputs: a workspace without the selection
     path's scratch (the size for k = 512) makes the same call fall back to the heaps in the output lists."""
