@@ -108,7 +108,7 @@ int64_t snaps_planned_evals(int64_t N, int n_feat, const uint16_t *h_masks, int 
  *              including columns no mask uses
  *   h_masks    host, [n_masks] uint16
  *   k          1 <= k <= min(N-1, SNAPS_MAX_K); the sub-lattice engine holds k <= 32; k > 256 needs
- *              out_idx and out_dist (the lists are built in place, or, for k > 512 on N <= 131,072 with the
+ *              out_idx and out_dist (the lists are built in place, or, for k > 384 on N <= 131,072 with the
  *              workspace snaps_workspace_bytes reports for that k, by radix selection: same lists, faster)
  *   q_begin, q_end   the queries: 0 <= q_begin < q_end <= N; nq = q_end - q_begin.  A rank of a
  *              multi-GPU run owns one slice (no exchange step);

@@ -1,5 +1,5 @@
 // knn_bigk.cu -- kNN self-join of ONE feature subspace for long lists on small tables
-// (512 < k <= 4096, N <= 131,072): PAPER.md:258, k_max = 4096 on SNAPShot1's 31,693 objects.
+// (384 < k <= 4096, N <= 131,072): PAPER.md:258, k_max = 4096 on SNAPShot1's 31,693 objects.
 //
 // At k = 13 % of N no index prunes anything, and a per-query heap of 4096 entries in global memory spends its
 // time in divergent sifts (grid_join.cu's in-place mode: 400-490 ms per subspace at k = 4096; here 28-37 ms):

@@ -1,12 +1,13 @@
 // knn_bigk.cuh -- kNN self-join of one feature subspace for long lists on small tables
-// (512 < k <= 4096, N <= 131,072: the paper's k_max = 4096 on SNAPShot1).
+// (384 < k <= 4096, N <= 131,072: the paper's k_max = 4096 on SNAPShot1).
 #pragma once
 #include "grid_join.cuh"
 
 namespace snaps {
 
 constexpr int kBigKMaxN = 1 << 17;     // ids take 17 bits of the 48-bit selection key
-constexpr int kBigKMinK = 513;         // below, the heaps of grid_join.cu are faster (the passes and the sort cost ~25 ms at N = 31,693)
+constexpr int kBigKMinK = 385;         // below, the heaps of grid_join.cu are faster for most masks (measured at N = 31,693:
+                                       // k = 400: heaps 14-40 ms for d = 2 ... 15, selection 23-28 ms; k = 300: 10-32 ms)
 
 // Scratch the launch needs for nq queries and lists of k: two arrays of nq*k 64-bit keys, segment offsets, CUB's own.
 size_t knn_bigk_scratch_bytes(int64_t nq, int k);

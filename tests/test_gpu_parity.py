@@ -603,9 +603,9 @@ def test_paper_operating_point_k4096(snaps, oracle_mod):
     assert torch.equal(out["kth"], out["dist"][:, :, -1])
 
 
-@pytest.mark.parametrize("n,nf,k,seed", [(700, 15, 513, 0), (1200, 6, 1000, 1), (1537, 15, 700, 2), (600, 3, 599, 3)])
+@pytest.mark.parametrize("n,nf,k,seed", [(700, 15, 385, 0), (1200, 6, 1000, 1), (1537, 15, 700, 2), (600, 3, 599, 3)])
 def test_long_list_path_against_oracle(snaps, oracle_mod, n, nf, k, seed):
-    """k > 512 on a small table takes the selection path (knn_bigk.cu: radix selection over brute-force passes,
+    """k > 384 on a small table takes the selection path (knn_bigk.cu: radix selection over brute-force passes,
     then one segmented sort): whole output against the oracle, incl. k = N - 1, plus a table with a block of
     duplicate rows (every tie must go to the smaller id) and a query-range slice."""
     import torch
@@ -643,14 +643,14 @@ def test_long_list_path_above_65535_objects(snaps, oracle_mod):
 
 def test_long_list_path_equals_heap_path(snaps):
     """The two ways of building lists longer than 256 give identical outputs: a workspace without the selection
-    path's scratch (the size for k = 512) makes the same call fall back to the heaps in the output lists."""
+    path's scratch (the size for k = 384) makes the same call fall back to the heaps in the output lists."""
     import torch
     X = workloads.make_table(2500, 91, outlier_frac=0.01)
     masks = np.array([0b11, 0x7FFF, (1 << 10) | (1 << 5) | 0b100], dtype=np.uint16)
     k = 777
     Xd = _dev(X)
     a = snaps.knn_selfjoin(Xd, masks, k, engine="grid")
-    small = torch.empty(snaps.workspace_bytes(len(X), 15, len(masks), 512, engine="grid"), dtype=torch.uint8, device="cuda")
+    small = torch.empty(snaps.workspace_bytes(len(X), 15, len(masks), 384, engine="grid"), dtype=torch.uint8, device="cuda")
     assert small.numel() < a["_workspace"].numel()
     b = snaps.knn_selfjoin(Xd, masks, k, engine="grid", workspace=small)
     torch.cuda.synchronize()
