@@ -63,13 +63,29 @@ __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoi
     auto stream = [&](auto&& fn) {
         const int n_pairs = (N + 1) >> 1;
         constexpr int kTilePairs = kTileB / 2;
+        constexpr int PF = (kTilePairs * G4 + 31) / 32;      // float4 per lane per tile
+        float4 nx[PF];                                       // the next tile, in flight while this one is evaluated
+        int nid0 = -1, nid1 = -1;
+        auto fetch = [&](int t0) {
+            const int n4 = min(kTilePairs, n_pairs - t0) * G4;
+            const float4* src = reinterpret_cast<const float4*>(p.Xs) + static_cast<size_t>(t0) * G4;
+#pragma unroll
+            for (int u = 0; u < PF; ++u)
+                if (lane + 32 * u < n4) nx[u] = __ldg(src + lane + 32 * u);
+            nid0 = 2 * t0 + lane < N ? __ldg(p.perm + 2 * t0 + lane) : -1;
+            nid1 = 2 * t0 + 32 + lane < N ? __ldg(p.perm + 2 * t0 + 32 + lane) : -1;
+        };
+        fetch(0);
         for (int t0 = 0; t0 < n_pairs; t0 += kTilePairs) {
             const int n = min(kTilePairs, n_pairs - t0);
             __syncwarp();
-            const float4* src = reinterpret_cast<const float4*>(p.Xs) + static_cast<size_t>(t0) * G4;
-            for (int i = lane; i < n * G4; i += 32) tile4[i] = __ldg(src + i);
-            for (int i = lane; i < 2 * n; i += 32) tile_id[i] = 2 * t0 + i < N ? __ldg(p.perm + 2 * t0 + i) : -1;
+#pragma unroll
+            for (int u = 0; u < PF; ++u)
+                if (lane + 32 * u < n * G4) tile4[lane + 32 * u] = nx[u];
+            tile_id[lane] = nid0;
+            tile_id[32 + lane] = nid1;
             __syncwarp();
+            if (t0 + kTilePairs < n_pairs) fetch(t0 + kTilePairs);
 #pragma unroll 2
             for (int r = 0; r < n; ++r) {
                 f32x2 acc = 0ull;
