@@ -2,8 +2,8 @@
 // (384 < k <= 4096, N <= 131,072): PAPER.md:258, k_max = 4096 on SNAPShot1's 31,693 objects.
 //
 // At k = 13 % of N no index prunes anything, and a per-query heap of 4096 entries in global memory spends its
-// time in divergent sifts (grid_join.cu's in-place mode: 400-490 ms per subspace at k = 4096; here 28-37 ms):
-//   * SELECT: one warp = 32 queries (lane = query) streams ALL candidates through a shared-memory tile, the
+// time in divergent sifts (grid_join.cu's in-place mode: 400-490 ms per subspace at k = 4096; here 21-31 ms):
+//   * SELECT: one CTA = 32 queries (lane = query; its four warps take alternate tiles) streams ALL candidates, the
 //     distance of a pair formed by the same instruction sequence as in grid_join.cu (so both paths give the
 //     same lists), and finds the query's k-th smallest key (d^2 bits << 17 | id) by radix selection: up to six passes
 //     over the candidates, each a 256-bin per-lane histogram of the next 8 key bits among the candidates that
@@ -22,7 +22,7 @@ namespace snaps {
 
 namespace {
 
-constexpr int kWarpsB = 2;            // warps per CTA (independent)
+constexpr int kWarpsB = 4;            // warps per CTA = per group of 32 queries (they share the candidates out)
 constexpr int kTileB = 64;            // candidates per tile
 constexpr int kBins = 256;
 constexpr int kIdBits = 17;
@@ -40,10 +40,11 @@ __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoi
     constexpr int G4 = DP / 2;                     // float4 per pair of candidates
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const long long wid = static_cast<long long>(blockIdx.x) * kWarpsB + warp;
-    const long long qi0 = wid * 32;
-    if (qi0 >= p.nq) return;                       // warps are independent: no block barrier exists
+    // one CTA = one group of 32 queries; its kWarpsB warps take alternate candidate tiles and add up their
+    // histograms (31,693 queries are only 991 groups: one warp each would leave the SMs half empty)
+    const long long qi0 = static_cast<long long>(blockIdx.x) * 32;
     float* wsm = reinterpret_cast<float*>(smem_raw) + static_cast<size_t>(warp) * warp_words_b(D, sizeof(C));
+    int* emit_cnt = reinterpret_cast<int*>(reinterpret_cast<float*>(smem_raw) + static_cast<size_t>(kWarpsB) * warp_words_b(D, sizeof(C)));
     float4* tile4 = reinterpret_cast<float4*>(wsm);
     int* tile_id = reinterpret_cast<int*>(wsm + kTileB * DP);
     C* hist = reinterpret_cast<C*>(wsm + kTileB * DP + kTileB);
@@ -75,8 +76,8 @@ __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoi
             nid0 = 2 * t0 + lane < N ? __ldg(p.perm + 2 * t0 + lane) : -1;
             nid1 = 2 * t0 + 32 + lane < N ? __ldg(p.perm + 2 * t0 + 32 + lane) : -1;
         };
-        fetch(0);
-        for (int t0 = 0; t0 < n_pairs; t0 += kTilePairs) {
+        if (warp * kTilePairs < n_pairs) fetch(warp * kTilePairs);
+        for (int t0 = warp * kTilePairs; t0 < n_pairs; t0 += kWarpsB * kTilePairs) {
             const int n = min(kTilePairs, n_pairs - t0);
             __syncwarp();
 #pragma unroll
@@ -85,7 +86,7 @@ __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoi
             tile_id[lane] = nid0;
             tile_id[32 + lane] = nid1;
             __syncwarp();
-            if (t0 + kTilePairs < n_pairs) fetch(t0 + kTilePairs);
+            if (t0 + kWarpsB * kTilePairs < n_pairs) fetch(t0 + kWarpsB * kTilePairs);
 #pragma unroll 2
             for (int r = 0; r < n; ++r) {
                 f32x2 acc = 0ull;
@@ -119,19 +120,26 @@ __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoi
     bool done = !valid;            // the k-th key is pinned down as far as the emit pass needs
 #pragma unroll 1
     for (int pass = 0; pass < 6; ++pass) {
-        if (__all_sync(kFull, done)) break;
+        if (__all_sync(kFull, done)) break;       // the same in every warp of the CTA: they select identically
         const int shift = 40 - 8 * pass;
+        __syncthreads();                           // the other warps have read this histogram
         for (int i = lane; i < kBins * 32; i += 32) hist[i] = 0;
         const u64 want = prefix >> (shift + 8);
         stream([&](u64 key) {
             if (!done && (pass == 0 || (key >> (shift + 8)) == want))
                 hist[static_cast<unsigned>((key >> shift) & 255u) * 32 + lane] += 1;
         });
+        __syncthreads();
         if (!done) {
             int cum = 0, sel = kBins - 1, csel = 0;
             bool found = false;
             for (int b = 0; b < kBins; ++b) {
-                const int c = static_cast<int>(hist[b * 32 + lane]);
+                int c = 0;
+#pragma unroll
+                for (int w = 0; w < kWarpsB; ++w)
+                    c += static_cast<int>(reinterpret_cast<const C*>(reinterpret_cast<const float*>(smem_raw) +
+                                                                     static_cast<size_t>(w) * warp_words_b(D, sizeof(C)) +
+                                                                     kTileB * DP + kTileB)[b * 32 + lane]);
                 if (!found && cum + c >= need) { sel = b; csel = c; found = true; }
                 if (!found) cum += c;
             }
@@ -146,10 +154,14 @@ __global__ void __launch_bounds__(kWarpsB * 32) bigk_select_kernel(const GridJoi
         }
     }
     // ---- the k keys up to the k-th, in stream order
-    int cnt = 0;
+    if (warp == 0) emit_cnt[lane] = 0;
+    __syncthreads();
     u64* mine = keys_out + static_cast<size_t>(valid ? my_id - p.q_begin : 0) * k;
     stream([&](u64 key) {
-        if (key <= prefix && cnt < k) mine[cnt++] = key;
+        if (key <= prefix) {
+            const int at = atomicAdd(&emit_cnt[lane], 1);    // any order: the segments are sorted afterwards
+            if (at < k) mine[at] = key;
+        }
     });
 }
 
@@ -198,12 +210,12 @@ size_t cub_bytes_for(int64_t nq, int k) {
 
 template <int D, typename C>
 cudaError_t launch_dc(const GridJoinParams& p, u64* keys, cudaStream_t st) {
-    const size_t smem = static_cast<size_t>(kWarpsB) * warp_words_b(D, sizeof(C)) * 4;
+    const size_t smem = (static_cast<size_t>(kWarpsB) * warp_words_b(D, sizeof(C)) + 32) * 4;
     auto kernel = bigk_select_kernel<D, C>;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    const long long warps = (static_cast<long long>(p.nq) + 31) / 32;
-    kernel<<<static_cast<int>((warps + kWarpsB - 1) / kWarpsB), kWarpsB * 32, smem, st>>>(p, keys);
+    const long long groups = (static_cast<long long>(p.nq) + 31) / 32;
+    kernel<<<static_cast<int>(groups), kWarpsB * 32, smem, st>>>(p, keys);
     return cudaGetLastError();
 }
 
