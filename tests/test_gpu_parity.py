@@ -641,6 +641,24 @@ def test_long_list_path_above_65535_objects(snaps, oracle_mod):
     assert torch.equal(out["kth"], out["dist"][:, :, -1])
 
 
+def test_long_list_path_through_the_batched_calls(snaps):
+    """Long lists through the streamed call (staging ring + side-stream copies) and through a query-range slice of
+    it: the same outputs as the resident call."""
+    import torch
+    X = workloads.make_table(1800, 93, outlier_frac=0.01)
+    masks = np.array([0b101, 0x7FFF, (1 << 9) | (1 << 2), 0b1111000, (1 << 14) | 1], dtype=np.uint16)
+    k = 450
+    Xd = _dev(X)
+    ref = snaps.knn_selfjoin(Xd, masks, k, engine="grid")
+    st = snaps.knn_selfjoin_streamed(Xd, masks, k, masks_per_batch=2, engine="grid")
+    part = snaps.knn_selfjoin_streamed(Xd, masks, k, masks_per_batch=3, engine="grid", q_range=(500, 1301))
+    torch.cuda.synchronize()
+    for name in ("idx", "dist", "kth", "mean", "indeg"):
+        assert torch.equal(st[name], ref[name].cpu()), name
+    for name in ("idx", "dist", "kth", "mean"):
+        assert torch.equal(part[name], ref[name][:, 500:1301].cpu()), name
+
+
 def test_long_list_path_equals_heap_path(snaps):
     """The two ways of building lists longer than 256 give identical outputs: a workspace without the selection
     path's scratch (the size for k = 384) makes the same call fall back to the heaps in the output lists."""
