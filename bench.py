@@ -388,7 +388,7 @@ def run_range(args, cfg, snaps, torch, D, steps, warmup, peakinfo, emit=True):
     return line
 
 
-def run_select_k(args, cfg, snaps, torch, D):
+def run_select_k(args, cfg, snaps, torch, D, n_masks=None, steps=None, warmup=None, emit=True):
     """The kNN parameter selection of PAPER.md:181-189, 258-260 at the paper's SNAPShot1 operating point: one join at
     k_max = 4096 gives every smaller k's lists as prefixes; snaps_knn_select_k then forms the scores at
     every k_j of the grid, ranks them, and takes Eq. 2 against the smallest and largest k and Eq. 3 -- for both kNN
@@ -396,7 +396,8 @@ def run_select_k(args, cfg, snaps, torch, D):
     X = workloads.make_table(cfg.n, cfg.seed, cols=list(range(cfg.n_feat)), outlier_frac=0.01)
     N = len(X)
     masks_all = cfg.masks()
-    masks = masks_all[np.linspace(0, len(masks_all) - 1, args.select_k).astype(np.int64)]
+    n_steps, n_warm = steps or args.steps, warmup if warmup is not None else max(1, args.warmup)
+    masks = masks_all[np.linspace(0, len(masks_all) - 1, n_masks or args.select_k).astype(np.int64)]
     k_max, n_top = 4096, int(round(0.01 * N))
     k_grid = np.array([2, 4, 8, 16, 32, 64, 128, 256, 512, 1024, 2048, 3072, 4096], dtype=np.int32)
     Xd = torch.from_numpy(X).to(D.dev)
@@ -417,34 +418,37 @@ def run_select_k(args, cfg, snaps, torch, D):
             sel = snaps.knn_select_k(j["idx"], j["dist"], k_grid, n_top)
         return sel
 
-    for _ in range(max(1, args.warmup)):
+    for _ in range(n_warm):
         step()
     torch.cuda.synchronize()
     join_ms.clear()
     sampler = ClockSampler(D.dev.index or 0)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
-    for _ in range(args.steps):
+    for _ in range(n_steps):
         sel = step()
     ev1.record()
     torch.cuda.synchronize()
     clocks = sampler.stop()
-    ms = ev0.elapsed_time(ev1) / args.steps
-    print(json.dumps({
+    ms = ev0.elapsed_time(ev1) / n_steps
+    line = {
         "metric": "feature spaces/sec (kNN parameter selection: join at k_max = 4096 + scores at 13 k + ranks + Eq. 2 + Eq. 3)",
-        "value": len(masks) / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(1, args.warmup),
+        "value": len(masks) / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": n_steps, "warmup": n_warm,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{cfg.name}: N={N} x 15 (seed {cfg.seed}), {len(masks)} subspaces spread over the 32,752, "
                                f"k_max={k_max}, k grid {k_grid.tolist()}, top {n_top}"},
-        "ms_per_subspace": ms / len(masks), "join_ms_per_subspace": float(np.sum(join_ms)) / args.steps / len(masks),
+        "ms_per_subspace": ms / len(masks), "join_ms_per_subspace": float(np.sum(join_ms)) / n_steps / len(masks),
         "seconds_for_all_32752": ms / len(masks) * 32752 / 1e3,
         "selected_grid_index_histogram_last_chunk": np.bincount(sel["j_mean"].cpu().numpy(), minlength=len(k_grid)).tolist(),
         "clocks": clocks,
         "paper_context": "paper: kNNSJ more expensive than DSSJ (PAPER.md:398); absolute kNNSJ time on SNAPShot1 not in the "
-                         "text (Fig. 10 is an image)"}), flush=True)
+                         "text (Fig. 10 is an image)"}
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
 
 
-def run_select_eps(args, cfg, snaps, torch, D):
+def run_select_eps(args, cfg, snaps, torch, D, n_masks=None, steps=None, warmup=None, emit=True):
     """The DSSJ parameter selection of PAPER.md:181-189, 229-239 in one call per chunk of masks
     (snaps_range_select_eps: eps_min / eps_max search -> |G| radii -> one join at eps_max -> ranks -> Eq. 2 -> Eq. 3)
     at the paper's operating point on SNAPShot1: s_min = 0.001 |D|, s_max = 0.15 |D|, |G| = 22 (Fig. 2,
@@ -456,7 +460,8 @@ def run_select_eps(args, cfg, snaps, torch, D):
     for m in cfg.masks():
         groups.setdefault(int(m) >> 6, []).append(m)
     keys = sorted(groups)
-    n_b = max(1, args.select_eps // 64)
+    n_steps, n_warm = steps or args.steps, warmup if warmup is not None else max(1, args.warmup)
+    n_b = max(1, (n_masks or args.select_eps) // 64)
     masks = np.array([m for kk in keys[::max(1, len(keys) // n_b)][:n_b] for m in groups[kk]], dtype=np.uint16)
     rng = np.random.default_rng(cfg.seed)
     q = np.sort(rng.choice(N, 1000, replace=False)).astype(np.int32)
@@ -470,21 +475,21 @@ def run_select_eps(args, cfg, snaps, torch, D):
             out = snaps.range_select_eps(Xd, masks[m0:m0 + chunk], q, c, s_min, s_max, G, n_top, 4096, engine="lattice")
         return out
 
-    for _ in range(max(1, args.warmup)):
+    for _ in range(n_warm):
         step()
     torch.cuda.synchronize()
     sampler = ClockSampler(D.dev.index or 0)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record()
-    for _ in range(args.steps):
+    for _ in range(n_steps):
         out = step()
     ev1.record()
     torch.cuda.synchronize()
     clocks = sampler.stop()
-    ms = ev0.elapsed_time(ev1) / args.steps
-    print(json.dumps({
+    ms = ev0.elapsed_time(ev1) / n_steps
+    line = {
         "metric": "feature spaces/sec (DSSJ parameter selection: eps search + 22-radius join at s_max + ranks + Eq. 2 + Eq. 3)",
-        "value": len(masks) / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(1, args.warmup),
+        "value": len(masks) / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": n_steps, "warmup": n_warm,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"{cfg.name}: N={N} x 15 (seed {cfg.seed}), {len(masks)} subspaces = {n_b} whole sub-lattice batches "
                                f"spread over the 32,752, s_min={s_min:.0f}, s_max={s_max:.0f} neighbours, |G|={G}, top {n_top}"},
@@ -492,7 +497,10 @@ def run_select_eps(args, cfg, snaps, torch, D):
         "selected_grid_index_histogram_last_chunk": np.bincount(out["j_count"].cpu().numpy(), minlength=G).tolist(),
         "clocks": clocks,
         "paper_context": "paper: DSSJ over all 32,752 feature spaces incl. eps^select and both rankings, 2.64 h on 1xA100 "
-                         "(o=8), whole pipeline with CPU post-processing and file output (PAPER.md:394)"}), flush=True)
+                         "(o=8), whole pipeline with CPU post-processing and file output (PAPER.md:394)"}
+    if emit:
+        print(json.dumps(line), flush=True)
+    return line
 
 
 def run_c5(args, cfg, snaps, torch, D):
@@ -587,6 +595,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-lsst", action="store_true", help="skip the LSST-scale leg (config 4) of the default run")
     ap.add_argument("--no-dssj", action="store_true", help="skip the DSSJ leg (config 3) of the default run")
+    ap.add_argument("--no-select", action="store_true", help="skip the parameter-selection legs of the default run")
     ap.add_argument("--masks-limit", type=int, default=0,
                     help="headline step on the first M masks only, for `ncu --set full` captures (ncu replays a launch "
                          "~40 times and saves / restores its 12.5 GB of outputs around each replay); the line is marked "
@@ -816,6 +825,21 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
         except Exception as e:
             lsst = {"error": repr(e)[:200]}
 
+    select = None
+    if default_run and not args.no_select:
+        # the paper's own operating points, a few seconds each: parameter selection for DSSJ at
+        # s_max = 0.15 N over 22 radii, and for kNN at k_max = 4096
+        select = {}
+        for name, fn, cfgname, nm in (("eps", run_select_eps, "c3_snapshot1_dssj", 512), ("k", run_select_k, "c2_snapshot1_knn", 16)):
+            try:
+                torch.cuda.empty_cache()
+                full = fn(args, workloads.get_config(cfgname), snaps, torch, D, n_masks=nm, steps=2, warmup=1, emit=False)
+                select[name] = {k_: full[k_] for k_ in ("metric", "value", "unit", "steps", "ms_per_step", "ms_per_subspace",
+                                                        "seconds_for_all_32752", "clocks")}
+                select[name]["workload"] = full["config"]["workload"]
+            except Exception as e:
+                select[name] = {"error": repr(e)[:200]}
+
     if rank == 0:
         line = {
             **({"partial": f"first {args.masks_limit} masks only (--masks-limit): not a bench value"} if args.masks_limit > 0 else {}),
@@ -831,7 +855,7 @@ def run_headline(args, cfg, snaps, torch, D, shard_masks, peakinfo):
                                     "one catalogue; masks dealt to ranks by sub-lattice batch, no collective") if (world > 1 or dynamic) else "none"},
             "evals_per_s": evals_per_s, "fp32_peak_frac": roofline["frac"],
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches,
-            "dssj": dssj, "lsst_scale": lsst,
+            "dssj": dssj, "lsst_scale": lsst, "parameter_selection": select,
             "clocks": clocks,
             "paper_context": "paper: DSSJ all 32,752 spaces 2.64 h on 1xA100 (o=8) incl. CPU "
                              "post-processing; LSST5M kNNSJ ~100 s/feature space (PAPER.md:394, Table 4)",
