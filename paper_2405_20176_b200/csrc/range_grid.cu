@@ -62,25 +62,43 @@ __device__ __noinline__ void range_grid_refine(float* ws, int G, bool with_sum, 
             mask |= (m.z < thr ? 1u : 0u) << (4 * j4 + 2);
             mask |= (m.w < thr ? 1u : 0u) << (4 * j4 + 3);
         }
+        // bin of one neighbour: guess, then settle against the exact thresholds on either side
+        auto bin_of = [&](float d2, float dd) -> int {
+            int g = min(max(__float2int_ru((dd - e_first) * per_eps), 0), G - 1);
+            const float below = g > 0 ? G_THR(T, g - 1) : -1.f, here = G_THR(T, g);
+            if (d2 < below) {
+                --g;
+                while (g > 0 && d2 < G_THR(T, g - 1)) --g;
+            } else if (!(d2 < here)) {
+                ++g;
+                while (!(d2 < G_THR(T, g))) ++g;             // ends: d2 < the largest threshold
+            }
+            return g;
+        };
+        // two neighbours per trip: their bin searches and histogram reads overlap; the updates keep candidate order
 #pragma unroll 1
         while (mask) {
-            const int j = __ffs(mask) - 1;
+            const int j0 = __ffs(mask) - 1;
             mask &= mask - 1u;
-            const float d2 = G_MT(lane, j);
-            const float dd = sqrtf(d2);
-            int g = min(max(__float2int_ru((dd - e_first) * per_eps), 0), G - 1);
-            {
-                const float below = g > 0 ? G_THR(T, g - 1) : -1.f, here = G_THR(T, g);
-                if (d2 < below) {
-                    --g;
-                    while (g > 0 && d2 < G_THR(T, g - 1)) --g;
-                } else if (!(d2 < here)) {
-                    ++g;
-                    while (!(d2 < G_THR(T, g))) ++g;         // ends: d2 < the largest threshold
+            const bool two = mask != 0u;
+            const int j1 = two ? __ffs(mask) - 1 : j0;
+            if (two) mask &= mask - 1u;
+            const float d2a = G_MT(lane, j0), d2b = G_MT(lane, j1);
+            const float dda = sqrtf(d2a), ddb = sqrtf(d2b);
+            const int ga = bin_of(d2a, dda), gb = bin_of(d2b, ddb);
+            const int ca = G_HCNT(T, ga), cb = G_HCNT(T, gb);
+            const float sa = with_sum ? G_HSUM(T, ga) : 0.f, sb = with_sum ? G_HSUM(T, gb) : 0.f;
+            if (two && ga == gb) {
+                G_HCNT(T, ga) = ca + 2;
+                if (with_sum) G_HSUM(T, ga) = (sa + dda) + ddb;
+            } else {
+                G_HCNT(T, ga) = ca + 1;
+                if (with_sum) G_HSUM(T, ga) = sa + dda;
+                if (two) {
+                    G_HCNT(T, gb) = cb + 1;
+                    if (with_sum) G_HSUM(T, gb) = sb + ddb;
                 }
             }
-            G_HCNT(T, g) += 1;
-            if (with_sum) G_HSUM(T, g) += dd;
         }
         __syncwarp();
     }
