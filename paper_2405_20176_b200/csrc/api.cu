@@ -429,7 +429,7 @@ snaps_status grid_knn_enqueue(Engine* E, int m0, int nm, int k, const KnnOut& o)
         grid_params_common(E, m, &p, &d);
         // long lists on a small table: radix selection over brute-force passes instead of per-query heaps, when the
         // workspace has the room (snaps_workspace_bytes asks for it)
-        const bool bigk = k >= snaps::kBigKMinK && j.N <= snaps::kBigKMaxN && E->bigk &&
+        const bool bigk = snaps::knn_bigk_pays(j.N, k) && E->bigk &&
                           E->bigk_bytes >= snaps::knn_bigk_scratch_bytes(j.nq(), k);
         CUDA_TRY(snaps::grid_index_build(E->gt, p.plan, p.N, d, p.bits, j.q_begin, j.q_end, bigk ? 0 : k, &E->gi, E->st));
         p.warp_order = E->gi.warp_order;
@@ -822,7 +822,7 @@ size_t snaps_workspace_bytes(int64_t N, int n_feat, int n_masks, int k, int flag
     const int engine = resolve_engine(flags, N, k);
     if (engine != SNAPS_ENGINE_LATTICE && engine != SNAPS_ENGINE_GRID) return 0;
     size_t b = base_workspace_bytes(N, n_feat, n_masks, engine, flags);
-    if (engine == SNAPS_ENGINE_GRID && k >= snaps::kBigKMinK && N <= snaps::kBigKMaxN &&
+    if (engine == SNAPS_ENGINE_GRID && snaps::knn_bigk_pays(N, k) &&
         static_cast<long long>(N) * k <= 0x7fffffffLL)
         b += snaps::knn_bigk_scratch_bytes(N, k);      // long lists on a small table: the selection path's keys
     return b;
